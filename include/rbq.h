@@ -1,0 +1,168 @@
+/*
+ * rbq.h -- C ABI of the B200-native RaBitQCache decode hot path (arxiv/paper_2606_31519).
+ *
+ * One library, librbq_b200.so, of hand-written sm_100a CUDA kernels.  Citations are lines of
+ * /root/reference/PAPER.md ("L<n>") plus the section / equation / algorithm they fall in.
+ *
+ * Conventions (all entry points)
+ *   - Every call returns int: RBQ_OK (0) or a negative rbq_status.  No exceptions, no exit().
+ *     rbq_last_error(ctx) returns a ctx-owned, NUL-terminated description of the last failure.
+ *   - ALL tensor arguments are caller-owned DEVICE pointers (allocated by the caller, e.g. with
+ *     PyTorch) unless the parameter name ends in `_host`.  The library allocates no device memory
+ *     per call; scratch comes from the caller-provided workspace (rbq_workspace_bytes /
+ *     rbq_set_workspace).  rbq_config and the rbq_kv / rbq_index structs themselves are HOST
+ *     structs holding device pointers; they are read during the call only.
+ *   - Calls only ENQUEUE work on the given stream (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and never synchronise the device.  Token counts are read from device
+ *     memory (rbq_index.n_indexed / n_total), so no host read-back happens inside a decode step.
+ *   - Layouts are row-major and contiguous except K/V, which carry element strides.  head_dim must
+ *     be 128 (64/256: RBQ_ERR_UNSUPPORTED).  n_q_heads must be a multiple of n_kv_heads, with
+ *     group size G = n_q_heads/n_kv_heads in {1, 2, 4, 8}.  Inputs are assumed finite.
+ *   - There is no CPU fallback and no backend dispatch: without a CUDA device every compute call
+ *     fails with RBQ_ERR_CUDA.
+ *
+ * Notation: B sequences, Hq query heads, Hkv KV heads, D = head_dim, Lcap = max_tokens,
+ * n_indexed[b] = tokens of sequence b that have codes, n_total[b] = n_indexed[b] + pending.
+ */
+#ifndef RBQ_H_
+#define RBQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rbq_ctx rbq_ctx;
+
+typedef enum {
+  RBQ_OK = 0,
+  RBQ_ERR_INVALID_ARG = -1,
+  RBQ_ERR_UNSUPPORTED = -2,
+  RBQ_ERR_WORKSPACE = -3,   /* workspace missing or too small */
+  RBQ_ERR_CUDA = -4
+} rbq_status;
+
+typedef enum { RBQ_F32 = 0, RBQ_BF16 = 1 } rbq_dtype;
+typedef enum { RBQ_ROT_DENSE = 0, RBQ_ROT_WH = 1 } rbq_rot_kind;
+/* EXACT: canonical fp32 order (R1) -> codes/factors bit-identical to the oracle.
+ * FAST : tensor-core rotation (bf16 hi/lo split, fp32 accumulate); codes may differ only where
+ *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative. */
+typedef enum { RBQ_ENC_EXACT = 0, RBQ_ENC_FAST = 1 } rbq_enc_mode;
+
+/* flags of rbq_encode_keys */
+#define RBQ_CK_GIVEN 1u     /* idx->c_k already holds the centroids: do not recompute (L66) */
+
+typedef struct {
+  int32_t batch, n_q_heads, n_kv_heads, head_dim;
+  int32_t max_tokens;        /* Lcap: capacity per sequence (multiple of 4)                      */
+  int32_t flush_tokens;      /* W: pending-window capacity (L215); 0 = never flush              */
+  int32_t kv_dtype;          /* rbq_dtype of K/V cache rows                                      */
+  int32_t q_dtype;           /* rbq_dtype of q                                                   */
+  int32_t out_dtype;         /* rbq_dtype of the attention output                                */
+  float sm_scale;            /* softmax scale; 0 => 1/sqrt(head_dim)  (Alg.2 line 12, L184)      */
+  int32_t rot_kind;          /* rbq_rot_kind                                                     */
+  const float* rot;          /* DEVICE. DENSE: P[D][D] row-major, y_j = sum_i x_i P[i][j] (L149); */
+                             /*         WH   : s[D] in {-1,+1}, y = H(s.*x)/sqrt(D), H Sylvester  */
+  int32_t enc_mode;          /* rbq_enc_mode                                                     */
+} rbq_config;
+
+typedef struct {             /* K/V cache; strides in ELEMENTS; one row = D contiguous elements  */
+  void* k;                   /* [B][Hkv][Lcap][D] by default                                      */
+  void* v;
+  int64_t stride_b, stride_h, stride_t;   /* stride_t must be >= D and a multiple of 8           */
+} rbq_kv;
+
+typedef struct {
+  uint32_t* codes;           /* [B][Hkv][Lcap][D/32]; bit (j%32) of word j/32 = [y_j > 0] (L270, L485) */
+  float*    f_scale;         /* [B][Hkv][Lcap] = ||k-c_k||^2 / ||(k-c_k)P||_1 = ||k-c_k|| / <c',P^T k_c> */
+                             /*   (Eq.18); 0 when k == c_k                             */
+  float*    f_bias;          /* [B][Hq][Lcap] = <c_q[b,h], k_t> (L89); NULL iff c_q is NULL      */
+  float*    c_k;             /* [B][Hkv][D] key centroids (Alg.1 line 4, L116)                   */
+  const float* c_q;          /* [B][Hq][D] query centroids or NULL (= zero centroid)             */
+  int32_t*  n_indexed;       /* [B]                                                              */
+  int32_t*  n_total;         /* [B]                                                              */
+} rbq_index;
+
+/* ---- context ------------------------------------------------------------------------------ */
+/* Validates the config and creates a context (host object; owns two CUDA events and a small
+ * device block of per-query constants carved from the workspace).                              */
+int rbq_create(const rbq_config* cfg_host, rbq_ctx** out);
+int rbq_destroy(rbq_ctx* ctx);
+/* Bytes of device scratch the calls below need for this config (query constants, Top-p state,
+ * split-K attention partials, scores of the fused step).                                       */
+int rbq_workspace_bytes(const rbq_ctx* ctx, size_t* bytes);
+/* `dev` must stay valid and 256-byte aligned until rbq_destroy or the next rbq_set_workspace.  */
+int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes);
+const char* rbq_last_error(const rbq_ctx* ctx);
+
+/* ---- S1  Alg.1 index construction (L106-147, L149-151, L485-487) ---------------------------- */
+/* For every (b, kv head) encodes tokens [0, seq_lens[b]): c_k = mean of those keys (unless
+ * RBQ_CK_GIVEN), x = k - c_k, y = x P, codes = packed [y > 0], f_scale = ||x||^2/||y||_1,
+ * f_bias = <c_q, k> when c_q != NULL.  Sets n_indexed = n_total = seq_lens.  seq_lens: DEVICE [B]. */
+int rbq_encode_keys(rbq_ctx* ctx, const rbq_kv* cache, const int32_t* seq_lens, uint32_t flags,
+                    rbq_index* idx, void* stream);
+
+/* ---- S2/S8  lazy decode updates (L215; R14) --------------------------------------- */
+/* k_new, v_new: [B][Hkv][n_new][D] contiguous, kv_dtype.  (1) if an earlier call enqueued a flush,
+ * `stream` waits for it and n_indexed += flushed; (2) rows are copied to cache rows
+ * [n_total, n_total+n_new), n_total += n_new; (3) if pending >= W, the oldest floor(pending/W)*W
+ * pending rows are encoded with the frozen c_k on `side_stream` (ordered after the copy by an
+ * event); they stay pending until the next rbq_append_tokens call.  side_stream may equal stream. */
+int rbq_append_tokens(rbq_ctx* ctx, const void* k_new, const void* v_new, int32_t n_new,
+                      rbq_kv* cache, rbq_index* idx, void* stream, void* side_stream);
+
+/* ---- S3  query pre-processing + INT4 quantisation (Alg.2 lines 4-6, L168-172; Eq.5; L524) */
+/* q: [B][Hq][D] q_dtype.  Optional outputs (each may be NULL): qu uint8 [B][Hq][D] in [0,15];
+ * qparams float [B][Hq][6] = {||q-c_q||, q_l, Delta, sum(qu), <q,c_k>, <c_q,c_k>}.
+ * Always refreshes the context's private query constants used by S4/S5.                        */
+int rbq_query_quantize(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu,
+                       float* qparams, void* stream);
+
+/* ---- S4  Int4_Dot_Binary (Alg.2 line 8, L176; L268-274; L534) -------------------------------- */
+/* dot[b][h][t] = <c_b[t], qu[b][h]> (exact integer), pop[b][g][t] = popcount(c_b[t]) for
+ * t < n_indexed[b]; int32 [B][Hq][Lcap] / [B][Hkv][Lcap].  Includes S3.                         */
+int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32_t* dot,
+                        int32_t* pop, void* stream);
+
+/* ---- S3-S5  estimated logits (Alg.2 lines 4-10; Eq.20, Eq.18, Eq.2) ------------ */
+/* scores[b][h][t] = sm_scale * ( ||q-c_q|| f_scale[t] (2 Delta dot + 2 q_l pop - Delta sum(qu)
+ * - D q_l) + <q,c_k> + f_bias[t] - <c_q,c_k> ) for t < n_indexed[b]; float [B][Hq][Lcap].       */
+int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float* scores,
+                        void* stream);
+
+/* ---- S6  adaptive Top-p selection (Alg.2 line 12, L184, L201) -------------------------------- */
+/* Per row (b,h): the minimal set I whose softmax mass over t < n_indexed[b] is >= p, ties broken
+ * towards the lowest index; p >= 1 selects every indexed token.  sel_idx int32 [B][Hq][Lcap]
+ * (first sel_cnt[b][h] entries valid, ascending token order), sel_cnt int32 [B][Hq].            */
+int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p,
+                    int32_t* sel_idx, int32_t* sel_cnt, void* stream);
+
+/* ---- S7  hybrid attention over selected U pending tokens (Alg.2 lines 14-15, L188-190, L215) -- */
+/* out[b][h] = sum_{t in A} softmax_A(<q,k_t> sm_scale)_t v_t, A = sel_idx[b][h][0..cnt) U
+ * [n_indexed[b], n_total[b]); out_dtype [B][Hq][D]; lse float [B][Hq] or NULL (log-sum-exp over A).
+ * Empty A gives out = 0, lse = -inf.                                                           */
+int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx,
+                         const int32_t* sel_idx, const int32_t* sel_cnt, void* out, float* lse,
+                         void* stream);
+
+/* ---- fused decode step: S3 -> S4/S5 -> S6 -> S7 (Alg.2) ---------------------------- */
+/* sel_idx / sel_cnt are optional outputs (NULL = keep them in the workspace).                   */
+int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, float p,
+                    void* out, int32_t* sel_idx, int32_t* sel_cnt, void* stream);
+
+/* ---- host-buffer convenience used by the end-to-end measurement ------------------------------ */
+/* Same as rbq_decode_step but q_host / out_host are HOST buffers (pinned recommended): copies q
+ * host->device, runs the step, copies out device->host, all on `stream`; staging device buffers
+ * come from the workspace.  Does not synchronise; the caller synchronises the stream.           */
+int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, const rbq_index* idx,
+                         float p, void* out_host, void* stream);
+
+/* Number of kernel launches the library has enqueued through this context so far.              */
+int64_t rbq_launch_count(const rbq_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RBQ_H_ */

@@ -1,0 +1,265 @@
+// rbq_api.cu -- host side of the C ABI declared in include/rbq.h: argument checks, workspace
+// carve-up, stream/event ordering of the lazy flush.  Every entry point only enqueues kernels.
+#include <new>
+#include <string.h>
+
+#include "rbq_common.cuh"
+
+namespace {
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+void layout_workspace(rbq_ctx* c) {
+  const rbq_config& g = c->cfg;
+  const size_t B = g.batch, Hq = g.n_q_heads, Hkv = g.n_kv_heads, L = g.max_tokens;
+  const size_t rows = B * Hq;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  c->off_qconst = take(B * Hkv * sizeof(RbqQConst));
+  c->off_rowstat = take(rows * 16);
+  c->off_scores = take(rows * L * sizeof(float));
+  c->off_selidx = take(rows * L * sizeof(int32_t));
+  c->off_selcnt = take(rows * sizeof(int32_t));
+  c->max_chunks = (int)(rows * ((L + 255) / 256 + 1));
+  c->off_part = take((size_t)c->max_chunks * (RBQ_D + 2) * sizeof(float));
+  c->off_part_meta = take((rows + 1) * sizeof(int));
+  c->off_stage_q = take(rows * RBQ_D * sizeof(float));
+  c->off_stage_out = take(rows * RBQ_D * sizeof(float));
+  c->off_centroid = take(B * Hkv * 64 * RBQ_D * sizeof(double));
+  c->off_counters = take(256);
+  c->off_cand = off;
+  c->total_bytes = off;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int check_kv(rbq_ctx* ctx, const rbq_kv* kv) {
+  if (!kv || !kv->k || !kv->v) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: null pointer");
+  if (kv->stride_t < RBQ_D || (kv->stride_t % 8) || (kv->stride_h % 8) || (kv->stride_b % 8))
+    RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: strides must be multiples of 8 elements and stride_t >= head_dim");
+  if (!aligned16(kv->k) || !aligned16(kv->v)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: k/v must be 16-byte aligned");
+  return RBQ_OK;
+}
+
+int check_idx(rbq_ctx* ctx, const rbq_index* idx, bool need_codes) {
+  if (!idx || !idx->c_k || !idx->n_indexed || !idx->n_total) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_index: null pointer");
+  if (need_codes && (!idx->codes || !idx->f_scale)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_index: codes/f_scale null");
+  if (need_codes && (!aligned16(idx->codes) || !aligned16(idx->f_scale)))
+    RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_index: codes/f_scale must be 16-byte aligned");
+  if ((idx->c_q != nullptr) != (idx->f_bias != nullptr))
+    RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_index: f_bias must be non-NULL exactly when c_q is");
+  return RBQ_OK;
+}
+
+int need_ws(rbq_ctx* ctx) {
+  if (!ctx->ws || ctx->ws_bytes < ctx->total_bytes)
+    RBQ_FAIL(ctx, RBQ_ERR_WORKSPACE, "workspace missing or smaller than rbq_workspace_bytes (%zu)", ctx->total_bytes);
+  return RBQ_OK;
+}
+
+RbqKV dev_kv(const rbq_kv* kv) { return RbqKV{kv->k, kv->v, (long long)kv->stride_b, (long long)kv->stride_h, (long long)kv->stride_t}; }
+
+template <typename T>
+T* ws_ptr(rbq_ctx* ctx, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(ctx->ws) + off); }
+
+}  // namespace
+
+#define RBQ_TRY(expr) do { int rc_ = (expr); if (rc_ != RBQ_OK) return rc_; } while (0)
+#define RBQ_CTX(ctx) do { if (!(ctx)) return RBQ_ERR_INVALID_ARG; (ctx)->err[0] = 0; } while (0)
+
+extern "C" {
+
+int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
+  if (!cfg || !out) return RBQ_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (cfg->batch <= 0 || cfg->n_q_heads <= 0 || cfg->n_kv_heads <= 0 || cfg->max_tokens <= 0) return RBQ_ERR_INVALID_ARG;
+  if (cfg->n_q_heads % cfg->n_kv_heads) return RBQ_ERR_INVALID_ARG;
+  if (cfg->head_dim != RBQ_D) return (cfg->head_dim == 64 || cfg->head_dim == 256) ? RBQ_ERR_UNSUPPORTED : RBQ_ERR_INVALID_ARG;
+  const int G = cfg->n_q_heads / cfg->n_kv_heads;
+  if (G != 1 && G != 2 && G != 4) return RBQ_ERR_UNSUPPORTED;
+  if (cfg->max_tokens % 4) return RBQ_ERR_INVALID_ARG;
+  if (cfg->flush_tokens < 0) return RBQ_ERR_INVALID_ARG;
+  for (int d : {cfg->kv_dtype, cfg->q_dtype, cfg->out_dtype})
+    if (d != RBQ_F32 && d != RBQ_BF16) return RBQ_ERR_INVALID_ARG;
+  if (cfg->rot_kind != RBQ_ROT_DENSE && cfg->rot_kind != RBQ_ROT_WH) return RBQ_ERR_INVALID_ARG;
+  if (cfg->enc_mode != RBQ_ENC_EXACT && cfg->enc_mode != RBQ_ENC_FAST) return RBQ_ERR_INVALID_ARG;
+  if (!cfg->rot || !(cfg->sm_scale >= 0.0f)) return RBQ_ERR_INVALID_ARG;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return RBQ_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return RBQ_ERR_CUDA;
+  rbq_ctx* c = new (std::nothrow) rbq_ctx();
+  if (!c) return RBQ_ERR_INVALID_ARG;
+  memset(c, 0, sizeof(*c));
+  c->cfg = *cfg;
+  c->G = G;
+  c->sm_scale = cfg->sm_scale > 0.0f ? cfg->sm_scale : (float)(1.0 / sqrt((double)cfg->head_dim));
+  c->sm_count = sms;
+  if (cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_flush, cudaEventDisableTiming) != cudaSuccess) {
+    delete c;
+    return RBQ_ERR_CUDA;
+  }
+  layout_workspace(c);
+  *out = c;
+  return RBQ_OK;
+}
+
+int rbq_destroy(rbq_ctx* ctx) {
+  if (!ctx) return RBQ_ERR_INVALID_ARG;
+  cudaEventDestroy(ctx->ev_copy);
+  cudaEventDestroy(ctx->ev_flush);
+  delete ctx;
+  return RBQ_OK;
+}
+
+int rbq_workspace_bytes(const rbq_ctx* ctx, size_t* bytes) {
+  if (!ctx || !bytes) return RBQ_ERR_INVALID_ARG;
+  *bytes = ctx->total_bytes;
+  return RBQ_OK;
+}
+
+int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes) {
+  RBQ_CTX(ctx);
+  if (!dev || (reinterpret_cast<uintptr_t>(dev) & 255u)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+  if (bytes < ctx->total_bytes) RBQ_FAIL(ctx, RBQ_ERR_WORKSPACE, "workspace too small: %zu < %zu", bytes, ctx->total_bytes);
+  ctx->ws = dev;
+  ctx->ws_bytes = bytes;
+  return RBQ_OK;
+}
+
+const char* rbq_last_error(const rbq_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int64_t rbq_launch_count(const rbq_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int rbq_encode_keys(rbq_ctx* ctx, const rbq_kv* cache, const int32_t* seq_lens, uint32_t flags, rbq_index* idx, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_kv(ctx, cache));
+  RBQ_TRY(check_idx(ctx, idx, true));
+  RBQ_TRY(need_ws(ctx));
+  if (!seq_lens) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "seq_lens null");
+  cudaStream_t s = (cudaStream_t)stream;
+  const RbqKV kv = dev_kv(cache);
+  if (!(flags & RBQ_CK_GIVEN)) RBQ_TRY(rbq_launch_centroid(ctx, kv, seq_lens, idx->c_k, s));
+  RBQ_TRY(rbq_launch_encode(ctx, kv, nullptr, seq_lens, 0, ctx->cfg.max_tokens, idx, s));
+  RBQ_TRY(rbq_launch_set_counts(ctx, seq_lens, idx->n_indexed, idx->n_total, s));
+  ctx->pending = 0;
+  ctx->in_flight = 0;
+  return RBQ_OK;
+}
+
+int rbq_append_tokens(rbq_ctx* ctx, const void* k_new, const void* v_new, int32_t n_new, rbq_kv* cache, rbq_index* idx,
+                      void* stream, void* side_stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_kv(ctx, cache));
+  RBQ_TRY(check_idx(ctx, idx, true));
+  RBQ_TRY(need_ws(ctx));
+  if (n_new < 0 || (n_new > 0 && (!k_new || !v_new))) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "k_new/v_new null or n_new < 0");
+  if (n_new > 0 && (!aligned16(k_new) || !aligned16(v_new))) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "k_new/v_new must be 16-byte aligned");
+  cudaStream_t s = (cudaStream_t)stream, side = (cudaStream_t)side_stream;
+  const RbqKV kv = dev_kv(cache);
+  int commit = 0;
+  if (ctx->in_flight > 0) {                       // (1) commit the flush enqueued by an earlier call
+    if (side != s) RBQ_CUDA_OK(ctx, cudaStreamWaitEvent(s, ctx->ev_flush, 0));
+    commit = ctx->in_flight;
+    ctx->pending -= commit;
+    ctx->in_flight = 0;
+  }
+  RBQ_TRY(rbq_launch_append_copy(ctx, k_new, v_new, n_new, kv, idx->n_indexed, idx->n_total, commit, s));   // (2)
+  ctx->pending += n_new;
+  const int W = ctx->cfg.flush_tokens;
+  if (W > 0 && ctx->pending >= W) {               // (3) batched encode of the oldest whole windows
+    const int nf = ctx->pending / W * W;
+    if (side != s) {
+      RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->ev_copy, s));
+      RBQ_CUDA_OK(ctx, cudaStreamWaitEvent(side, ctx->ev_copy, 0));
+    }
+    RBQ_TRY(rbq_launch_encode(ctx, kv, idx->n_indexed, nullptr, nf, nf, idx, side));
+    if (side != s) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->ev_flush, side));
+    ctx->in_flight = nf;
+  }
+  return RBQ_OK;
+}
+
+int rbq_query_quantize(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, false));
+  RBQ_TRY(need_ws(ctx));
+  if (!q) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q null");
+  return rbq_launch_query(ctx, q, idx, qu, qparams, (cudaStream_t)stream);
+}
+
+int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32_t* dot, int32_t* pop, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, true));
+  RBQ_TRY(need_ws(ctx));
+  if (!q || !dot || !pop) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/dot/pop null");
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, (cudaStream_t)stream));
+  return rbq_launch_estimate(ctx, idx, nullptr, dot, pop, (cudaStream_t)stream);
+}
+
+int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float* scores, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, true));
+  RBQ_TRY(need_ws(ctx));
+  if (!q || !scores) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/scores null");
+  if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, (cudaStream_t)stream));
+  return rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
+                    void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, false));
+  if (!scores || !sel_idx || !sel_cnt) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores/sel_idx/sel_cnt null");
+  if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
+  if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
+  return rbq_launch_topp(ctx, scores, idx->n_indexed, p, sel_idx, sel_cnt, (cudaStream_t)stream);
+}
+
+int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, const int32_t* sel_idx,
+                         const int32_t* sel_cnt, void* out, float* lse, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_kv(ctx, cache));
+  RBQ_TRY(check_idx(ctx, idx, false));
+  RBQ_TRY(need_ws(ctx));
+  if (!q || !sel_idx || !sel_cnt || !out) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/sel_idx/sel_cnt/out null");
+  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, sel_idx, sel_cnt, out, lse, (cudaStream_t)stream);
+}
+
+int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, float p, void* out,
+                    int32_t* sel_idx, int32_t* sel_cnt, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_kv(ctx, cache));
+  RBQ_TRY(check_idx(ctx, idx, true));
+  RBQ_TRY(need_ws(ctx));
+  if (!q || !out) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/out null");
+  if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
+  cudaStream_t s = (cudaStream_t)stream;
+  float* scores = ws_ptr<float>(ctx, ctx->off_scores);
+  int32_t* si = sel_idx ? sel_idx : ws_ptr<int32_t>(ctx, ctx->off_selidx);
+  int32_t* sn = sel_cnt ? sel_cnt : ws_ptr<int32_t>(ctx, ctx->off_selcnt);
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, s));
+  RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, idx->n_indexed, p, si, sn, s));
+  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, si, sn, out, nullptr, s);
+}
+
+int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, const rbq_index* idx, float p,
+                         void* out_host, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(need_ws(ctx));
+  if (!q_host || !out_host) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q_host/out_host null");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads;
+  const size_t qb = rows * RBQ_D * (ctx->cfg.q_dtype == RBQ_BF16 ? 2 : 4);
+  const size_t ob = rows * RBQ_D * (ctx->cfg.out_dtype == RBQ_BF16 ? 2 : 4);
+  void* dq = ws_ptr<char>(ctx, ctx->off_stage_q);
+  void* dout = ws_ptr<char>(ctx, ctx->off_stage_out);
+  RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
+  RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, dout, nullptr, nullptr, stream));
+  RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
+  return RBQ_OK;
+}
+
+}  // extern "C"

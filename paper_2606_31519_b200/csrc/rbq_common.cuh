@@ -1,0 +1,108 @@
+// rbq_common.cuh -- shared host/device declarations of the B200 RaBitQCache library.
+// CUDA path only: nothing here is shared with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/rbq.h"
+
+#define RBQ_D 128            // head_dim supported by every kernel
+#define RBQ_WORDS 4          // D/32 code words per token
+#define RBQ_MAX_G 4          // query heads per KV head (N=8 MMA columns: G heads + G ones-columns)
+
+// Private per-(sequence, KV head) query constants produced by S3 and consumed by S4/S5.
+// bfrag: B-operand fragments of mma.m16n8k32.u8 in register order [k-step][lane][2]
+//        (column 2j = query head j of the group, column 2j+1 = all-ones -> popcount),
+//        pre-scaled by 2^(3-n) so that the masked code bytes (value 2^n) need no shift.
+struct __align__(16) RbqQConst {
+  uint32_t bfrag[4][32][2];
+  float cA[RBQ_MAX_G];       // sm_scale * ||q-c_q|| * Delta / 4
+  float cB[RBQ_MAX_G];       // sm_scale * ||q-c_q|| * q_l   / 4
+  float cD[RBQ_MAX_G];       // sm_scale * (<q,c_k> - <c_q,c_k>)
+  int32_t init_d[RBQ_MAX_G]; // 0x4B400000 - 4*sum(qu): accumulator start (float-magic biased)
+  int32_t init_p;            // 0x4B400000 - 4*D
+  int32_t pad[3];
+};
+
+struct RbqKV {               // device view of rbq_kv
+  const void* k;
+  const void* v;
+  long long sb, sh, st;      // element strides
+};
+
+struct rbq_ctx {
+  rbq_config cfg;
+  int G;
+  float sm_scale;
+  int sm_count;
+  void* ws;
+  size_t ws_bytes;
+  // workspace carve-up (byte offsets), filled by rbq_layout_workspace
+  size_t off_qconst, off_rowstat, off_scores, off_selidx, off_selcnt, off_part, off_part_meta,
+      off_stage_q, off_stage_out, off_centroid, off_counters, off_cand, total_bytes;
+  int max_chunks;
+  cudaEvent_t ev_copy, ev_flush;
+  int pending;               // host shadow of n_total - n_indexed (uniform over the batch)
+  int in_flight;             // rows encoded by an enqueued flush, not yet committed
+  long long launches;
+  char err[256];
+};
+
+#define RBQ_FAIL(ctx, code, ...)                                   \
+  do {                                                             \
+    if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__); \
+    return (code);                                                 \
+  } while (0)
+
+#define RBQ_CUDA_OK(ctx, expr)                                                      \
+  do {                                                                              \
+    cudaError_t e_ = (expr);                                                        \
+    if (e_ != cudaSuccess) RBQ_FAIL(ctx, RBQ_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+#define RBQ_LAUNCH_OK(ctx)                                                          \
+  do {                                                                              \
+    cudaError_t e_ = cudaGetLastError();                                            \
+    if (e_ != cudaSuccess) RBQ_FAIL(ctx, RBQ_ERR_CUDA, "launch failed at %s:%d: %s", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+    (ctx)->launches++;                                                              \
+  } while (0)
+
+// ---- device helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ float rbq_ld_elem(const float* p, long long i) { return p[i]; }
+__device__ __forceinline__ float rbq_ld_elem(const __nv_bfloat16* p, long long i) {
+  return __bfloat162float(p[i]);
+}
+__device__ __forceinline__ void rbq_st_elem(float* p, long long i, float v) { p[i] = v; }
+__device__ __forceinline__ void rbq_st_elem(__nv_bfloat16* p, long long i, float v) {
+  p[i] = __float2bfloat16_rn(v);
+}
+__device__ __forceinline__ float rbq_bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float rbq_bf16hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+
+// order-preserving map float -> uint32 (larger float <=> larger key)
+__device__ __forceinline__ uint32_t rbq_fkey(float f) {
+  uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float rbq_fkey_inv(uint32_t k) {
+  uint32_t u = (k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k;
+  return __uint_as_float(u);
+}
+
+// ---- kernel launchers (defined in the .cu files, called from rbq_api.cu) ------------------------
+int rbq_launch_centroid(rbq_ctx*, const RbqKV&, const int32_t* seq_lens, float* c_k, cudaStream_t);
+int rbq_launch_encode(rbq_ctx*, const RbqKV&, const int32_t* t_begin, const int32_t* t_count_or_null,
+                      int fixed_count, int max_count, const rbq_index*, cudaStream_t);
+int rbq_launch_set_counts(rbq_ctx*, const int32_t* seq_lens, int32_t* n_indexed, int32_t* n_total,
+                          cudaStream_t);
+int rbq_launch_append_copy(rbq_ctx*, const void* k_new, const void* v_new, int n_new, const RbqKV&,
+                           int32_t* n_indexed, int32_t* n_total, int commit, cudaStream_t);
+int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, float* qparams, cudaStream_t);
+int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop,
+                        cudaStream_t);
+int rbq_launch_topp(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx,
+                    int32_t* sel_cnt, cudaStream_t);
+int rbq_launch_attention(rbq_ctx*, const void* q, const RbqKV&, const rbq_index*, const int32_t* sel_idx,
+                         const int32_t* sel_cnt, void* out, float* lse, cudaStream_t);

@@ -1,0 +1,294 @@
+// rbq_encode.cu -- S1/S2: centroid, Alg.1 index construction (PAPER.md:L106-147, L149-151,
+// L485-487), cache-tail append (L215).
+//
+// RBQ_ENC_EXACT reproduces the canonical fp32 order of DESIGN.md R1 bit for bit:
+//   x_i = fl32(k_i) - c_k,i ; n2 <- fmaf(x_i, x_i, n2), i ascending ;
+//   dense: y_j <- fmaf(x_i, P[i][j], y_j), i ascending, one accumulator per j
+//          (a non-split-K SGEMM inner loop, here register-tiled 4 tokens x 8 outputs per thread);
+//   WH   : u = s.*x ; butterflies h = 1,2,..,D/2, (a,b) -> (a+b, a-b) ; y = u * fl32(1/sqrt(D)) ;
+//   l1 <- l1 + |y_j| (WH: |u_j|, then * fl32(1/sqrt(D))), j ascending ; f_scale = n2 / l1 (IEEE).
+// The file is compiled with -fmad=false; every fused multiply-add below is an explicit fmaf().
+#include "rbq_common.cuh"
+
+namespace {
+
+constexpr int ENC_TOK = 64;        // tokens per CTA tile
+constexpr int ENC_THREADS = 256;
+constexpr int XS = RBQ_D + 1;      // padded row stride of the x / y tile (bank-conflict-free per-token access)
+
+// ---- centroid: c_k = mean over t < n of K[b][g][t][:] , fp64 accumulation ------------------------
+// Partial sums over CEN_SPLIT contiguous token ranges, then a fixed-order final sum.  fp64 sums of
+// bf16 / fp32 inputs of this size are exact (or within 1 ulp of fp64), so the fp32 result is the
+// correctly rounded mean irrespective of the order.
+constexpr int CEN_SPLIT = 64;
+
+template <typename T>
+__global__ void centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
+                                        const int32_t* __restrict__ seq_lens, int Hkv, double* __restrict__ part) {
+  const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv, s = blockIdx.y, d = threadIdx.x;
+  const int n = seq_lens[b];
+  const int per = (n + CEN_SPLIT - 1) / CEN_SPLIT;
+  const int t0 = s * per, t1 = min(n, t0 + per);
+  const T* base = K + (long long)b * sb + (long long)g * sh;
+  double acc = 0.0;
+  for (int t = t0; t < t1; ++t) acc += (double)rbq_ld_elem(base, (long long)t * st + d);
+  part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + d] = acc;
+}
+
+__global__ void centroid_final_kernel(const double* __restrict__ part, const int32_t* __restrict__ seq_lens,
+                                      int Hkv, float* __restrict__ c_k) {
+  const int bg = blockIdx.x, b = bg / Hkv, d = threadIdx.x;
+  const int n = seq_lens[b];
+  double acc = 0.0;
+  for (int s = 0; s < CEN_SPLIT; ++s) acc += part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + d];
+  c_k[(size_t)bg * RBQ_D + d] = (n > 0) ? (float)(acc / (double)n) : 0.0f;
+}
+
+// ---- Alg.1 tile kernel --------------------------------------------------------------------------
+// grid = (ceil(max_count / ENC_TOK), B*Hkv).  Tokens [t_begin[b], t_begin[b]+count[b]).
+// smem: x tile [ENC_TOK][XS] fp32 (becomes the y tile), P [D][D] fp32 (dense only), n2[ENC_TOK].
+template <typename T, int ROT>
+__global__ void __launch_bounds__(ENC_THREADS)
+encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
+              const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count, int fixed_count,
+              int Hkv, int Lcap, const float* __restrict__ rot, const float* __restrict__ c_k,
+              uint32_t* __restrict__ codes, float* __restrict__ f_scale) {
+  extern __shared__ __align__(16) float smem[];
+  float* xs = smem;                                 // [ENC_TOK][XS]
+  float* n2s = xs + ENC_TOK * XS;                   // [ENC_TOK]
+  float* rs = n2s + ENC_TOK;                        // dense: [D][D]; WH: [D] signs
+
+  const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
+  const int tb = t_begin ? t_begin[b] : 0;
+  const int cnt = t_count ? t_count[b] : fixed_count;
+  const int tile0 = blockIdx.x * ENC_TOK;
+  if (tile0 >= cnt) return;
+  const int ntok = min(ENC_TOK, cnt - tile0);
+  const int tid = threadIdx.x;
+  const T* base = K + (long long)b * sb + (long long)g * sh + (long long)(tb + tile0) * st;
+  const float* ck = c_k + (size_t)bg * RBQ_D;
+
+  // x = fl32(k) - c_k
+  for (int e = tid; e < ENC_TOK * RBQ_D; e += ENC_THREADS) {
+    const int r = e >> 7, d = e & 127;
+    float x = 0.0f;
+    if (r < ntok) x = __fsub_rn(rbq_ld_elem(base, (long long)r * st + d), ck[d]);
+    xs[r * XS + d] = x;
+  }
+  if (ROT == RBQ_ROT_DENSE) {
+    for (int e = tid; e < RBQ_D * RBQ_D / 4; e += ENC_THREADS)
+      reinterpret_cast<float4*>(rs)[e] = reinterpret_cast<const float4*>(rot)[e];
+  } else {
+    if (tid < RBQ_D) rs[tid] = rot[tid];
+  }
+  __syncthreads();
+
+  // n2: one thread per token, sequential fma chain (i ascending)
+  if (tid < ENC_TOK) {
+    float n2 = 0.0f;
+    const float* xr = xs + tid * XS;
+#pragma unroll 8
+    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(xr[i], xr[i], n2);
+    n2s[tid] = n2;
+  }
+
+  if (ROT == RBQ_ROT_DENSE) {
+    // thread -> 4 tokens (tt*4..+3) x 8 outputs (tj*4..+3 and 64+tj*4..+3)
+    const int tj = tid & 15, tt = tid >> 4;
+    float acc[4][8];
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = 0; n < 8; ++n) acc[m][n] = 0.0f;
+    const float* x0 = xs + (tt * 4) * XS;
+#pragma unroll 4
+    for (int i = 0; i < RBQ_D; ++i) {
+      const float4 r0 = *reinterpret_cast<const float4*>(rs + i * RBQ_D + tj * 4);
+      const float4 r1 = *reinterpret_cast<const float4*>(rs + i * RBQ_D + 64 + tj * 4);
+      const float rr[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const float xv = x0[m * XS + i];
+#pragma unroll
+        for (int n = 0; n < 8; ++n) acc[m][n] = fmaf(xv, rr[n], acc[m][n]);
+      }
+    }
+    __syncthreads();                                 // everyone done reading x (n2 included)
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = 0; n < 8; ++n)
+        xs[(tt * 4 + m) * XS + (n < 4 ? tj * 4 + n : 64 + tj * 4 + (n - 4))] = acc[m][n];
+  } else {
+    __syncthreads();
+    // WH: warp w handles tokens w, w+8, ...; lane holds elements 4*lane..4*lane+3
+    const int warp = tid >> 5, lane = tid & 31;
+    for (int r = warp; r < ENC_TOK; r += ENC_THREADS / 32) {
+      float* xr = xs + r * XS + lane * 4;
+      float u0 = __fmul_rn(rs[lane * 4 + 0], xr[0]), u1 = __fmul_rn(rs[lane * 4 + 1], xr[1]);
+      float u2 = __fmul_rn(rs[lane * 4 + 2], xr[2]), u3 = __fmul_rn(rs[lane * 4 + 3], xr[3]);
+      float a, c;
+      a = __fadd_rn(u0, u1); c = __fsub_rn(u0, u1); u0 = a; u1 = c;          // h = 1
+      a = __fadd_rn(u2, u3); c = __fsub_rn(u2, u3); u2 = a; u3 = c;
+      a = __fadd_rn(u0, u2); c = __fsub_rn(u0, u2); u0 = a; u2 = c;          // h = 2
+      a = __fadd_rn(u1, u3); c = __fsub_rn(u1, u3); u1 = a; u3 = c;
+#pragma unroll
+      for (int m = 1; m < 32; m <<= 1) {                                      // h = 4*m
+        const bool up = (lane & m) != 0;
+        float p0 = __shfl_xor_sync(0xffffffffu, u0, m), p1 = __shfl_xor_sync(0xffffffffu, u1, m);
+        float p2 = __shfl_xor_sync(0xffffffffu, u2, m), p3 = __shfl_xor_sync(0xffffffffu, u3, m);
+        u0 = up ? __fsub_rn(p0, u0) : __fadd_rn(u0, p0);
+        u1 = up ? __fsub_rn(p1, u1) : __fadd_rn(u1, p1);
+        u2 = up ? __fsub_rn(p2, u2) : __fadd_rn(u2, p2);
+        u3 = up ? __fsub_rn(p3, u3) : __fadd_rn(u3, p3);
+      }
+      __syncwarp();
+      xr[0] = u0; xr[1] = u1; xr[2] = u2; xr[3] = u3;                         // unscaled u
+    }
+  }
+  __syncthreads();
+
+  // epilogue: one thread per token: l1 (sequential), sign bits, f_scale
+  if (tid < ntok) {
+    const float* yr = xs + tid * XS;
+    float l1 = 0.0f;
+    uint32_t w[RBQ_WORDS];
+    const float c = (float)(1.0 / sqrt((double)RBQ_D));
+#pragma unroll
+    for (int ww = 0; ww < RBQ_WORDS; ++ww) {
+      uint32_t word = 0;
+#pragma unroll 8
+      for (int j = 0; j < 32; ++j) {
+        const float yv = yr[ww * 32 + j];
+        l1 = __fadd_rn(l1, fabsf(yv));
+        const float ys = (ROT == RBQ_ROT_DENSE) ? yv : __fmul_rn(yv, c);
+        word |= (ys > 0.0f ? 1u : 0u) << j;
+      }
+      w[ww] = word;
+    }
+    if (ROT == RBQ_ROT_WH) l1 = __fmul_rn(l1, c);
+    const size_t tok = (size_t)bg * Lcap + tb + tile0 + tid;
+    reinterpret_cast<uint4*>(codes)[tok] = make_uint4(w[0], w[1], w[2], w[3]);
+    f_scale[tok] = (l1 == 0.0f) ? 0.0f : __fdiv_rn(n2s[tid], l1);
+  }
+}
+
+// f_bias[b][hq][t] = <c_q[b][hq], k_t>, fma chain i ascending.  Parity-only path.
+template <typename T>
+__global__ void fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
+                             const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count,
+                             int fixed_count, int Hq, int Hkv, int Lcap, const float* __restrict__ c_q,
+                             float* __restrict__ f_bias) {
+  const int bh = blockIdx.y, b = bh / Hq, h = bh % Hq, g = h / (Hq / Hkv);
+  const int tb = t_begin ? t_begin[b] : 0;
+  const int cnt = t_count ? t_count[b] : fixed_count;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= cnt) return;
+  const T* k = K + (long long)b * sb + (long long)g * sh + (long long)(tb + r) * st;
+  const float* cq = c_q + (size_t)bh * RBQ_D;
+  float acc = 0.0f;
+  for (int i = 0; i < RBQ_D; ++i) acc = fmaf(cq[i], rbq_ld_elem(k, i), acc);
+  f_bias[(size_t)bh * Lcap + tb + r] = acc;
+}
+
+__global__ void set_counts_kernel(const int32_t* __restrict__ seq_lens, int32_t* n_indexed, int32_t* n_total, int B) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < B) { n_indexed[b] = seq_lens[b]; n_total[b] = seq_lens[b]; }
+}
+
+// S2: commit an earlier flush (n_indexed += commit), copy n_new rows per (b, kv head) to the cache
+// tail [n_total, n_total + n_new), then n_total += n_new (done by the last block via a second launch
+// of this kernel family: see append_bump_kernel).  16-byte vector copies.
+__global__ void append_copy_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, int n_new,
+                                   int row_vec, char* __restrict__ kc, char* __restrict__ vc, long long sb_bytes,
+                                   long long sh_bytes, long long st_bytes, int Hkv,
+                                   const int32_t* __restrict__ n_total) {
+  const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_new * row_vec) return;
+  const int r = e / row_vec, c = e % row_vec;
+  const long long dst = (long long)b * sb_bytes + (long long)g * sh_bytes + (long long)(n_total[b] + r) * st_bytes + c * 16;
+  const size_t src = ((size_t)bg * n_new + r) * row_vec + c;
+  *reinterpret_cast<uint4*>(kc + dst) = k_new[src];
+  *reinterpret_cast<uint4*>(vc + dst) = v_new[src];
+}
+
+__global__ void append_bump_kernel(int32_t* n_indexed, int32_t* n_total, int B, int commit, int n_new) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < B) { n_indexed[b] += commit; n_total[b] += n_new; }
+}
+
+}  // namespace
+
+int rbq_launch_centroid(rbq_ctx* ctx, const RbqKV& kv, const int32_t* seq_lens, float* c_k, cudaStream_t s) {
+  const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
+  double* part = reinterpret_cast<double*>(static_cast<char*>(ctx->ws) + ctx->off_centroid);
+  dim3 grid(BG, CEN_SPLIT);
+  if (ctx->cfg.kv_dtype == RBQ_BF16)
+    centroid_partial_kernel<<<grid, RBQ_D, 0, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
+                                                    ctx->cfg.n_kv_heads, part);
+  else
+    centroid_partial_kernel<<<grid, RBQ_D, 0, s>>>((const float*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
+                                                    ctx->cfg.n_kv_heads, part);
+  RBQ_LAUNCH_OK(ctx);
+  centroid_final_kernel<<<BG, RBQ_D, 0, s>>>(part, seq_lens, ctx->cfg.n_kv_heads, c_k);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
+
+template <typename T, int ROT>
+static int launch_encode_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
+                           int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
+  const size_t smem = (size_t)(ENC_TOK * XS + ENC_TOK + (ROT == RBQ_ROT_DENSE ? RBQ_D * RBQ_D : RBQ_D)) * sizeof(float);
+  auto kern = encode_kernel<T, ROT>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set = true;
+  }
+  dim3 grid((max_count + ENC_TOK - 1) / ENC_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
+  kern<<<grid, ENC_THREADS, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
+                                       ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->cfg.rot, idx->c_k,
+                                       idx->codes, idx->f_scale);
+  RBQ_LAUNCH_OK(ctx);
+  if (idx->c_q) {
+    dim3 g2((max_count + 127) / 128, ctx->cfg.batch * ctx->cfg.n_q_heads);
+    fbias_kernel<T><<<g2, 128, 0, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
+                                       ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, idx->c_q,
+                                       idx->f_bias);
+    RBQ_LAUNCH_OK(ctx);
+  }
+  return RBQ_OK;
+}
+
+int rbq_launch_encode(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
+                      int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
+  if (max_count <= 0) return RBQ_OK;
+  const bool bf = ctx->cfg.kv_dtype == RBQ_BF16, wh = ctx->cfg.rot_kind == RBQ_ROT_WH;
+  if (bf && !wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  if (bf && wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  if (!bf && !wh) return launch_encode_t<float, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  return launch_encode_t<float, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+}
+
+int rbq_launch_set_counts(rbq_ctx* ctx, const int32_t* seq_lens, int32_t* n_indexed, int32_t* n_total, cudaStream_t s) {
+  set_counts_kernel<<<(ctx->cfg.batch + 127) / 128, 128, 0, s>>>(seq_lens, n_indexed, n_total, ctx->cfg.batch);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
+
+int rbq_launch_append_copy(rbq_ctx* ctx, const void* k_new, const void* v_new, int n_new, const RbqKV& kv,
+                           int32_t* n_indexed, int32_t* n_total, int commit, cudaStream_t s) {
+  const int esz = ctx->cfg.kv_dtype == RBQ_BF16 ? 2 : 4;
+  const int row_vec = RBQ_D * esz / 16;
+  if (n_new > 0) {
+    dim3 grid((n_new * row_vec + 127) / 128, ctx->cfg.batch * ctx->cfg.n_kv_heads);
+    append_copy_kernel<<<grid, 128, 0, s>>>((const uint4*)k_new, (const uint4*)v_new, n_new, row_vec,
+                                            (char*)kv.k, (char*)kv.v, kv.sb * esz, kv.sh * esz, kv.st * esz,
+                                            ctx->cfg.n_kv_heads, n_total);
+    RBQ_LAUNCH_OK(ctx);
+  }
+  append_bump_kernel<<<(ctx->cfg.batch + 127) / 128, 128, 0, s>>>(n_indexed, n_total, ctx->cfg.batch, commit, n_new);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}

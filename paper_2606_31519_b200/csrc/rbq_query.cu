@@ -1,0 +1,179 @@
+// rbq_query.cu -- S3: query pre-processing and INT4 quantisation
+// (Alg.2 lines 4-6, L168-172; Eq.5; L524; readings R5/R6/R12 of DESIGN.md).
+//
+//   xq = q - c_q ; qn = ||xq||_2 ; u = xq/qn ; q' = u P (canonical fp32 order, as S1) ;
+//   q_l = min q', q_r = max q', Delta = (q_r - q_l)/15 ; qu_j = clamp(floor((q'_j-q_l)/Delta + 1/2), 0, 15).
+// One CTA per (sequence, KV head), one 128-thread slice per query head of the group.  Besides the
+// optional public outputs (qu, qparams) it writes the private RbqQConst block: the u8 B-operand
+// fragments of the estimator MMA and the per-head reconstruction constants of Eq.20 / Eq.2.
+#include "rbq_common.cuh"
+
+namespace {
+
+template <typename TQ>
+__global__ void __launch_bounds__(RBQ_MAX_G * RBQ_D)
+query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const float* __restrict__ c_k,
+             const float* __restrict__ rot, int rot_kind, int Hq, int Hkv, float sm_scale,
+             uint8_t* __restrict__ qu_out, float* __restrict__ qparams, RbqQConst* __restrict__ qc_out) {
+  const int G = Hq / Hkv;
+  const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv;
+  const int hs = threadIdx.x >> 7, j = threadIdx.x & 127;      // head slice, dim
+  const int h = g * G + min(hs, G - 1);              // slices beyond G recompute head G-1, write nothing
+  const size_t row = (size_t)b * Hq + h;
+
+  __shared__ float s_x[RBQ_MAX_G][RBQ_D];      // xq, then u
+  __shared__ float s_y[RBQ_MAX_G][RBQ_D];      // q'
+  __shared__ float s_red[RBQ_MAX_G][8];        // per-warp min / max
+  __shared__ int s_isum[RBQ_MAX_G][4];
+  __shared__ float s_qn[RBQ_MAX_G];
+  __shared__ double s_dot[RBQ_MAX_G][2];
+  __shared__ uint8_t s_qu[RBQ_MAX_G][RBQ_D];
+
+  const float qv = rbq_ld_elem(q, row * RBQ_D + j);
+  const float cqv = c_q ? c_q[row * RBQ_D + j] : 0.0f;
+  const float ckv = c_k[(size_t)bg * RBQ_D + j];
+  const float xq = c_q ? __fsub_rn(qv, cqv) : qv;
+  s_x[hs][j] = xq;
+  s_y[hs][j] = qv;                               // staged for the fp64 dot chains below
+  __syncthreads();
+  // three sequential chains per head, on three different threads (orders of DESIGN.md R1)
+  if (j == 0) {
+    float n2 = 0.0f;
+    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(s_x[hs][i], s_x[hs][i], n2);
+    s_qn[hs] = __fsqrt_rn(n2);
+  } else if (j == 32) {                          // <q, c_k> : fp64, i ascending
+    double a = 0.0;
+    const float* ck = c_k + (size_t)bg * RBQ_D;
+    for (int i = 0; i < RBQ_D; ++i) a = fma((double)s_y[hs][i], (double)ck[i], a);
+    s_dot[hs][0] = a;
+  } else if (j == 64) {                          // <c_q, c_k>
+    double a = 0.0;
+    if (c_q) {
+      const float* ck = c_k + (size_t)bg * RBQ_D;
+      const float* cq = c_q + row * RBQ_D;
+      for (int i = 0; i < RBQ_D; ++i) a = fma((double)cq[i], (double)ck[i], a);
+    }
+    s_dot[hs][1] = a;
+  }
+  __syncthreads();
+  const float qn = s_qn[hs];
+  const float u = (qn > 0.0f) ? __fdiv_rn(xq, qn) : 0.0f;
+  s_x[hs][j] = u;
+  __syncthreads();
+
+  float qp;
+  if (rot_kind == RBQ_ROT_DENSE) {
+    float acc = 0.0f;
+#pragma unroll 8
+    for (int i = 0; i < RBQ_D; ++i) acc = fmaf(s_x[hs][i], rot[i * RBQ_D + j], acc);
+    qp = acc;
+  } else {
+    // warp 0 of the slice runs the 128-point butterflies (4 elements per lane), as in S1
+    if (j < 32) {
+      const int lane = j;
+      float u0 = __fmul_rn(rot[lane * 4 + 0], s_x[hs][lane * 4 + 0]);
+      float u1 = __fmul_rn(rot[lane * 4 + 1], s_x[hs][lane * 4 + 1]);
+      float u2 = __fmul_rn(rot[lane * 4 + 2], s_x[hs][lane * 4 + 2]);
+      float u3 = __fmul_rn(rot[lane * 4 + 3], s_x[hs][lane * 4 + 3]);
+      float a, c;
+      a = __fadd_rn(u0, u1); c = __fsub_rn(u0, u1); u0 = a; u1 = c;
+      a = __fadd_rn(u2, u3); c = __fsub_rn(u2, u3); u2 = a; u3 = c;
+      a = __fadd_rn(u0, u2); c = __fsub_rn(u0, u2); u0 = a; u2 = c;
+      a = __fadd_rn(u1, u3); c = __fsub_rn(u1, u3); u1 = a; u3 = c;
+#pragma unroll
+      for (int m = 1; m < 32; m <<= 1) {
+        const bool up = (lane & m) != 0;
+        float p0 = __shfl_xor_sync(0xffffffffu, u0, m), p1 = __shfl_xor_sync(0xffffffffu, u1, m);
+        float p2 = __shfl_xor_sync(0xffffffffu, u2, m), p3 = __shfl_xor_sync(0xffffffffu, u3, m);
+        u0 = up ? __fsub_rn(p0, u0) : __fadd_rn(u0, p0);
+        u1 = up ? __fsub_rn(p1, u1) : __fadd_rn(u1, p1);
+        u2 = up ? __fsub_rn(p2, u2) : __fadd_rn(u2, p2);
+        u3 = up ? __fsub_rn(p3, u3) : __fadd_rn(u3, p3);
+      }
+      const float c1 = (float)(1.0 / sqrt((double)RBQ_D));
+      s_y[hs][lane * 4 + 0] = __fmul_rn(u0, c1);
+      s_y[hs][lane * 4 + 1] = __fmul_rn(u1, c1);
+      s_y[hs][lane * 4 + 2] = __fmul_rn(u2, c1);
+      s_y[hs][lane * 4 + 3] = __fmul_rn(u3, c1);
+    }
+    __syncthreads();
+    qp = s_y[hs][j];
+  }
+
+  // min / max over the 128 dims of the slice
+  float mn = qp, mx = qp;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+    mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  }
+  const int wslice = (j >> 5);
+  if ((j & 31) == 0) { s_red[hs][wslice] = mn; s_red[hs][4 + wslice] = mx; }
+  __syncthreads();
+  const float ql = fminf(fminf(s_red[hs][0], s_red[hs][1]), fminf(s_red[hs][2], s_red[hs][3]));
+  const float qr = fmaxf(fmaxf(s_red[hs][4], s_red[hs][5]), fmaxf(s_red[hs][6], s_red[hs][7]));
+  const float delta = __fdiv_rn(__fsub_rn(qr, ql), 15.0f);
+  int v = 0;
+  if (delta > 0.0f) {
+    const float t = __fdiv_rn(__fsub_rn(qp, ql), delta);
+    v = (int)floorf(__fadd_rn(t, 0.5f));
+    v = min(15, max(0, v));
+  }
+  s_qu[hs][j] = (uint8_t)v;
+  int sv = v;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sv += __shfl_xor_sync(0xffffffffu, sv, o);
+  if ((j & 31) == 0) s_isum[hs][wslice] = sv;
+  __syncthreads();
+  const int sumq = s_isum[hs][0] + s_isum[hs][1] + s_isum[hs][2] + s_isum[hs][3];
+
+  if (hs < G) {
+    if (qu_out) qu_out[row * RBQ_D + j] = (uint8_t)v;
+    if (j == 0) {
+      const float q_ck = (float)s_dot[hs][0], cq_ck = (float)s_dot[hs][1];
+      if (qparams) {
+        float* o = qparams + row * 6;
+        o[0] = qn; o[1] = ql; o[2] = delta; o[3] = (float)sumq; o[4] = q_ck; o[5] = cq_ck;
+      }
+      RbqQConst* qc = qc_out + bg;
+      qc->cA[hs] = (float)((double)sm_scale * (double)qn * (double)delta * 0.25);
+      qc->cB[hs] = (float)((double)sm_scale * (double)qn * (double)ql * 0.25);
+      qc->cD[hs] = (float)((double)sm_scale * ((double)q_ck - (double)cq_ck));
+      qc->init_d[hs] = 0x4B400000 - 4 * sumq;
+      if (hs == 0) qc->init_p = 0x4B400000 - 4 * RBQ_D;
+    }
+  }
+  // B-operand fragments: word (s, lane, r): byte i <-> k = 4*t' + i (+16 for r = 1), column n = g'
+  //   dim = 32*t' + 8*i + 2*s + r, value = (n odd ? 1 : qu[head n/2][dim]) << (3 - ((2*s + r) & 3))
+  if (threadIdx.x < 256) {
+    const int w = threadIdx.x, s = w >> 6, lane = (w >> 1) & 31, r = w & 1;
+    const int gp = lane >> 2, tp = lane & 3;
+    const int e = 2 * s + r, sh = 3 - (e & 3);
+    uint32_t word = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int dim = 32 * tp + 8 * i + e;
+      uint32_t val = 0;
+      if (gp & 1) val = ((gp >> 1) < G) ? 1u : 0u;
+      else if ((gp >> 1) < G) val = s_qu[gp >> 1][dim];
+      word |= (val << sh) << (8 * i);
+    }
+    qc_out[bg].bfrag[s][lane][r] = word;
+  }
+}
+
+}  // namespace
+
+int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, cudaStream_t s) {
+  const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
+  RbqQConst* qc = reinterpret_cast<RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
+  const int threads = max(256, ctx->G * RBQ_D);
+  if (ctx->cfg.q_dtype == RBQ_BF16)
+    query_kernel<<<BG, threads, 0, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
+                                        ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+  else
+    query_kernel<<<BG, threads, 0, s>>>((const float*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
+                                        ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
