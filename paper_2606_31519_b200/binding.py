@@ -28,7 +28,9 @@ RBQ_CK_GIVEN = 1
 EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspace", "rbq_last_error",
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
            "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_sparse_attention",
-           "rbq_decode_step", "rbq_decode_step_host"]
+           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read"]
+N_STAGES = 5
+STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_chunks", "attn_merge"]
 
 
 class RbqError(RuntimeError):
@@ -78,6 +80,8 @@ def load():
         "rbq_sparse_attention": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), vp, vp, vp, vp, vp], C.c_int),
         "rbq_decode_step": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), f32, vp, vp, vp, vp], C.c_int),
         "rbq_decode_step_host": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), f32, vp, vp], C.c_int),
+        "rbq_profile_enable": ([vp, C.c_int], C.c_int),
+        "rbq_profile_read": ([vp, C.POINTER(C.c_float), C.POINTER(i32)], C.c_int),
     }
     for name, (args, res) in sig.items():
         fn = getattr(lib, name)
@@ -191,6 +195,18 @@ def rbq_decode_step_host(ctx, q_host, kv: rbq_kv, idx: rbq_index, p, out_host, s
                                             _stream(stream)), "rbq_decode_step_host")
 
 
+def rbq_profile_enable(ctx, enable: bool):
+    _check(ctx, load().rbq_profile_enable(ctx, int(bool(enable))), "rbq_profile_enable")
+
+
+def rbq_profile_read(ctx):
+    """Blocks until the recorded steps finished; returns ({stage: total ms}, n_steps)."""
+    ms = (C.c_float * N_STAGES)()
+    n = C.c_int32()
+    _check(ctx, load().rbq_profile_read(ctx, ms, C.byref(n)), "rbq_profile_read")
+    return dict(zip(STAGE_NAMES, [float(x) for x in ms])), n.value
+
+
 # ---- convenience bundle ----------------------------------------------------------------------------
 class RaBitQCache:
     """Context + workspace + caller-owned tensors (K/V cache, index) for one attention layer."""
@@ -278,3 +294,9 @@ class RaBitQCache:
 
     def launch_count(self):
         return rbq_launch_count(self.ctx)
+
+    def profile_enable(self, on=True):
+        rbq_profile_enable(self.ctx, on)
+
+    def profile_read(self):
+        return rbq_profile_read(self.ctx)

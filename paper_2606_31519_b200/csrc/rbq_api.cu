@@ -108,6 +108,10 @@ int rbq_destroy(rbq_ctx* ctx) {
   if (!ctx) return RBQ_ERR_INVALID_ARG;
   cudaEventDestroy(ctx->ev_copy);
   cudaEventDestroy(ctx->ev_flush);
+  if (ctx->prof_ev) {
+    for (int i = 0; i < RBQ_PROFILE_MAX_STEPS * (RBQ_N_STAGES + 1); ++i) cudaEventDestroy(ctx->prof_ev[i]);
+    delete[] ctx->prof_ev;
+  }
   delete ctx;
   return RBQ_OK;
 }
@@ -239,10 +243,51 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
   float* scores = ws_ptr<float>(ctx, ctx->off_scores);
   int32_t* si = sel_idx ? sel_idx : ws_ptr<int32_t>(ctx, ctx->off_selidx);
   int32_t* sn = sel_cnt ? sel_cnt : ws_ptr<int32_t>(ctx, ctx->off_selcnt);
+  cudaEvent_t* ev = nullptr;                       // stage timing events of this step, if profiling
+  if (ctx->prof_on && ctx->prof_steps < RBQ_PROFILE_MAX_STEPS) ev = ctx->prof_ev + (size_t)ctx->prof_steps++ * (RBQ_N_STAGES + 1);
+  ctx->stage_ev = ev;
+  if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[0], s));
   RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, s));
+  if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
+  if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
   RBQ_TRY(rbq_launch_topp(ctx, scores, idx->n_indexed, p, si, sn, s));
-  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, si, sn, out, nullptr, s);
+  if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
+  const int rc = rbq_launch_attention(ctx, q, dev_kv(cache), idx, si, sn, out, nullptr, s);   // records ev[4] before the merge
+  ctx->stage_ev = nullptr;
+  if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[5], s));
+  return rc;
+}
+
+int rbq_profile_enable(rbq_ctx* ctx, int enable) {
+  RBQ_CTX(ctx);
+  if (enable && !ctx->prof_ev) {
+    const int n = RBQ_PROFILE_MAX_STEPS * (RBQ_N_STAGES + 1);
+    ctx->prof_ev = new (std::nothrow) cudaEvent_t[n];
+    if (!ctx->prof_ev) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "out of host memory");
+    for (int i = 0; i < n; ++i) RBQ_CUDA_OK(ctx, cudaEventCreate(&ctx->prof_ev[i]));
+  }
+  ctx->prof_on = enable ? 1 : 0;
+  ctx->prof_steps = 0;
+  return RBQ_OK;
+}
+
+int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host) {
+  RBQ_CTX(ctx);
+  if (!ms_host || !n_steps_host) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "ms_host/n_steps_host null");
+  for (int k = 0; k < RBQ_N_STAGES; ++k) ms_host[k] = 0.0f;
+  *n_steps_host = ctx->prof_steps;
+  for (int i = 0; i < ctx->prof_steps; ++i) {
+    cudaEvent_t* ev = ctx->prof_ev + (size_t)i * (RBQ_N_STAGES + 1);
+    RBQ_CUDA_OK(ctx, cudaEventSynchronize(ev[RBQ_N_STAGES]));
+    for (int k = 0; k < RBQ_N_STAGES; ++k) {
+      float ms = 0.0f;
+      RBQ_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ev[k], ev[k + 1]));
+      ms_host[k] += ms;
+    }
+  }
+  ctx->prof_steps = 0;
+  return RBQ_OK;
 }
 
 int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, const rbq_index* idx, float p,

@@ -240,6 +240,7 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   else if (qbf) rc = launch_chunks<float, __nv_bfloat16>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
   else rc = launch_chunks<float, float>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
   if (rc != RBQ_OK) return rc;
+  if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   if (ctx->cfg.out_dtype == RBQ_BF16)
     attn_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, chunk_start, (__nv_bfloat16*)out, lse);
   else

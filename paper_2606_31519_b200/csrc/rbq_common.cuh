@@ -47,6 +47,9 @@ struct rbq_ctx {
   int pending;               // host shadow of n_total - n_indexed (uniform over the batch)
   int in_flight;             // rows encoded by an enqueued flush, not yet committed
   long long launches;
+  int prof_on, prof_steps;                                   // stage timing (rbq_profile_*)
+  cudaEvent_t* stage_ev;                                     // events of the step being enqueued, or NULL
+  cudaEvent_t* prof_ev;                                      // [RBQ_PROFILE_MAX_STEPS][RBQ_N_STAGES + 1], lazily created
   char err[256];
 };
 

@@ -1,0 +1,218 @@
+"""Chained GPU parity: the whole path on the GPU (encode -> query -> estimate -> Top-p -> attention,
+and the fused rbq_decode_step), against the oracle end to end; p = 1 against dense attention (P6);
+lazy append / flush state machine (L215) against the oracle's LazyIndex, with and without a side stream.
+
+In the chained runs the GPU's own fp32 logits feed its Top-p, so a set difference is additionally
+allowed for tokens whose logit lies within the 1e-5 band of the boundary logit: the check used here is
+"oracle Top-p applied to the GPU's logits" (exact rule) plus the end-to-end output tolerance.
+"""
+import numpy as np
+import pytest
+
+from tests import gpu_util as U
+
+pytestmark = pytest.mark.gpu
+
+ROT_DENSE, ROT_WH = 0, 1
+
+
+def _chained(orc, w, rot, kind, p, with_cq=False):
+    import torch
+    o = U.oracle_full(orc, w, rot, kind, with_cq, p=p)
+    c = U.make_cache(w, rot, rot_kind=kind, with_cq=with_cq)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    q = U.to_dev(w.q, U.torch_dtype(w))
+    # staged calls
+    scores = c.new_scores()
+    sel_idx, sel_cnt = c.new_sel()
+    out, out2 = c.new_out(), c.new_out()
+    c.estimate_scores(q, scores)
+    c.topp_select(scores, p, sel_idx, sel_cnt)
+    c.sparse_attention(q, sel_idx, sel_cnt, out)
+    # fused call
+    sel_idx2, sel_cnt2 = c.new_sel()
+    c.decode_step(q, p, out2, sel_idx2, sel_cnt2)
+    torch.cuda.synchronize()
+    s = scores.cpu().numpy()
+    U.assert_logits_close(s, o["scores"], w.seq_lens, w.Hq)
+    idx, cnt = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy()
+    assert (cnt == sel_cnt2.cpu().numpy()).all()
+    n_rows = np.repeat(w.seq_lens, w.Hq)
+    ref_idx, ref_cnt = orc.topp(s.reshape(w.B * w.Hq, w.Lcap), n_rows, p)     # exact rule on the GPU's logits
+    ref_idx, ref_cnt = ref_idx.reshape(w.B, w.Hq, w.Lcap), ref_cnt.reshape(w.B, w.Hq)
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        for h in range(w.Hq):
+            g = idx[b, h, :cnt[b, h]]
+            assert (g == sel_idx2.cpu().numpy()[b, h, :cnt[b, h]]).all(), "fused and staged selections differ"
+            U.assert_topp_row(s[b, h, :n], g, ref_idx[b, h, :ref_cnt[b, h]], p)
+    # budgets of the oracle chain and the GPU chain agree closely (boundary tokens only)
+    assert np.abs(cnt.astype(np.int64) - o["sel_cnt"]).max() <= max(2, int(0.002 * o["sel_cnt"].max()))
+    U.assert_attention_close(out.cpu().numpy(), o["out"], w.kv_dtype)
+    assert (out.cpu().numpy().view(np.uint32) == out2.cpu().numpy().view(np.uint32)).all(), "fused != staged output"
+    c.close()
+    return o
+
+
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+@pytest.mark.parametrize("cfg,kw,p", [(0, {}, 0.9), (1, dict(L=5003), 0.8), (1, dict(L=5003), 0.95),
+                                      (2, dict(L=6150, n_heavy=32), 0.9), (3, dict(L=3001, B=3), 0.9)])
+def test_decode_step_chained(orc, rot128, cfg, kw, p, kind):
+    from paper_2606_31519_b200 import synth
+    rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
+    _chained(orc, U.workload(cfg, **kw), rot, kind, p)
+
+
+def test_decode_step_chained_with_cq(orc, rot128):
+    _chained(orc, U.workload(0, with_cq=True), rot128[0], ROT_DENSE, 0.9, with_cq=True)
+
+
+@pytest.mark.parametrize("cfg,kw", [(0, {}), (1, dict(L=2051)), (3, dict(L=1500, B=3))])
+def test_p1_is_dense_attention(orc, rot128, cfg, kw):
+    """P6: rbq_decode_step(p = 1) == textbook softmax attention over all tokens (oracle with the full index
+    set, and torch SDPA in fp32 on the same device as an independent library definition)."""
+    import torch
+    w = U.workload(cfg, **kw)
+    c = U.make_cache(w, rot128[0])
+    c.encode_keys(U.to_dev(w.seq_lens))
+    q = U.to_dev(w.q, U.torch_dtype(w))
+    out = c.new_out()
+    sel_idx, sel_cnt = c.new_sel()
+    c.decode_step(q, 1.0, out, sel_idx, sel_cnt)
+    torch.cuda.synchronize()
+    assert (sel_cnt.cpu().numpy() == w.seq_lens[:, None]).all()
+    all_idx = np.broadcast_to(np.arange(w.Lcap, dtype=np.int32), (w.B, w.Hq, w.Lcap)).copy()
+    all_cnt = np.broadcast_to(w.seq_lens[:, None], (w.B, w.Hq)).astype(np.int32).copy()
+    ref, _ = orc.attention(w.q, w.K, w.V, all_idx, all_cnt, w.seq_lens, w.seq_lens, U.SM_SCALE)
+    U.assert_attention_close(out.cpu().numpy(), ref, w.kv_dtype)
+    G = w.Hq // w.Hkv
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        kk = c.K[b, :, :n].float().repeat_interleave(G, dim=0)
+        vv = c.V[b, :, :n].float().repeat_interleave(G, dim=0)
+        sd = torch.nn.functional.scaled_dot_product_attention(q[b].float()[:, None, :], kk, vv)[:, 0]
+        U.assert_attention_close(out[b].cpu().numpy(), sd.cpu().numpy(), w.kv_dtype)
+    c.close()
+
+
+@pytest.mark.parametrize("use_side", [False, True])
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+def test_append_flush_state_machine(orc, rot128, use_side, kind):
+    """L215 lazy updates (R14): 1 token per step, W = 8; flush enqueued when pending reaches W, committed by
+    the next append; codes of flushed rows bit-exact, decode output checked at steps around each flush."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    W, steps = 8, 21
+    w = U.workload(3, L=900, B=3, extra_cap=64)
+    rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, kind, rot, W)
+    c = U.make_cache(w, rot, rot_kind=kind, flush_tokens=W)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    main = torch.cuda.current_stream()
+    side = torch.cuda.Stream() if use_side else None
+    pool = synth.query_pool(w, 4)
+    out = c.new_out()
+    sel_idx, sel_cnt = c.new_sel()
+    for s in range(steps):
+        k_new, v_new = synth.append_rows(3, s, w.B, w.Hkv, 1)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16), stream=main, side_stream=side)
+        q_np = pool[s % 4]
+        c.decode_step(U.to_dev(q_np, torch.bfloat16), 0.9, out, sel_idx, sel_cnt)
+        torch.cuda.synchronize()
+        assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all(), f"step {s}: n_indexed"
+        assert (c.n_total.cpu().numpy() == lazy.n_total).all(), f"step {s}: n_total"
+        if s in (0, W - 2, W - 1, W, W + 1, 2 * W - 1, 2 * W, steps - 1):
+            ref = orc.decode_step(q_np, lazy.K, lazy.V, lazy.codes, lazy.f_scale, None, lazy.c_k, None, lazy.n_indexed,
+                                  lazy.n_total, kind, rot, 0.9, U.SM_SCALE)
+            U.assert_attention_close(out.cpu().numpy(), ref["out"], "bf16")
+            assert np.abs(sel_cnt.cpu().numpy().astype(np.int64) - ref["sel_cnt"]).max() <= 2
+    # every committed or in-flight row carries the oracle's code and factor; K/V rows were copied verbatim
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    for b in range(w.B):
+        n = int(lazy.n_indexed[b]) + lazy.in_flight
+        assert (codes[b, :, :n] == lazy.codes[b, :, :n]).all()
+        assert (fs[b, :, :n].view(np.uint32) == lazy.f_scale[b, :, :n].view(np.uint32)).all()
+        nt = int(lazy.n_total[b])
+        assert (c.K[b, :, :nt].float().cpu().numpy() == lazy.K[b, :, :nt]).all()
+        assert (c.V[b, :, :nt].float().cpu().numpy() == lazy.V[b, :, :nt]).all()
+    c.close()
+
+
+def test_append_many_tokens_per_call(orc, rot128):
+    """n_new = 5 per call with W = 8 (flush of whole windows only), and n_new >= W in one call."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    W = 8
+    w = U.workload(3, L=700, B=2, extra_cap=128)
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, ROT_DENSE, rot128[0], W)
+    c = U.make_cache(w, rot128[0], flush_tokens=W)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    out = c.new_out()
+    for s, n_new in enumerate([5, 5, 5, 19, 1, 8]):
+        k_new, v_new = synth.append_rows(3, 50 + s, w.B, w.Hkv, n_new)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16))
+        c.decode_step(U.to_dev(w.q, torch.bfloat16), 0.9, out)
+        torch.cuda.synchronize()
+        assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all() and (c.n_total.cpu().numpy() == lazy.n_total).all()
+        ref = orc.decode_step(w.q, lazy.K, lazy.V, lazy.codes, lazy.f_scale, None, lazy.c_k, None, lazy.n_indexed,
+                              lazy.n_total, ROT_DENSE, rot128[0], 0.9, U.SM_SCALE)
+        U.assert_attention_close(out.cpu().numpy(), ref["out"], "bf16")
+    c.close()
+
+
+def test_decode_step_host_buffers(orc, rot128):
+    """rbq_decode_step_host: pinned host q in, host out; same bits as the device-buffer call."""
+    import torch
+    w = U.workload(1, L=2051)
+    c = U.make_cache(w, rot128[0])
+    c.encode_keys(U.to_dev(w.seq_lens))
+    q_host = torch.from_numpy(w.q).to(torch.bfloat16).pin_memory()
+    out_host = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32).pin_memory()
+    c.decode_step_host(q_host, 0.9, out_host)
+    out = c.new_out()
+    c.decode_step(q_host.cuda(), 0.9, out)
+    torch.cuda.synchronize()
+    assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+    assert c.launch_count() > 0
+    c.close()
+
+
+def test_error_codes(rot128):
+    """Argument checks return negative status codes with a message; nothing is enqueued."""
+    import ctypes as C
+    import torch
+    from paper_2606_31519_b200 import binding as rb
+    rot = torch.from_numpy(rot128[0]).cuda()
+    lib = rb.load()
+
+    def create(**kw):
+        base = dict(batch=1, n_q_heads=4, n_kv_heads=1, head_dim=128, max_tokens=256, flush_tokens=0, kv_dtype=1, q_dtype=1,
+                    out_dtype=0, sm_scale=0.0, rot_kind=0, rot=rot.data_ptr(), enc_mode=0)
+        base.update(kw)
+        cfg = rb.rbq_config(**base)
+        h = C.c_void_p()
+        return lib.rbq_create(C.byref(cfg), C.byref(h)), h
+
+    assert create(head_dim=64)[0] == -2 and create(head_dim=256)[0] == -2          # RBQ_ERR_UNSUPPORTED
+    assert create(head_dim=100)[0] == -1 and create(n_q_heads=3, n_kv_heads=2)[0] == -1
+    assert create(max_tokens=0)[0] == -1 and create(rot=None)[0] == -1
+    rc, h = create()
+    assert rc == 0
+    n = rb.rbq_workspace_bytes(h)
+    assert n > 0
+    # no workspace yet
+    q = torch.zeros(1, 4, 128, dtype=torch.bfloat16, device="cuda")
+    idx = rb.rbq_index(None, None, None, rot.data_ptr(), None, rot.data_ptr(), rot.data_ptr())
+    assert lib.rbq_query_quantize(h, q.data_ptr(), C.byref(idx), None, None, None) == -3      # RBQ_ERR_WORKSPACE
+    assert b"workspace" in lib.rbq_last_error(h)
+    small = torch.zeros(256, dtype=torch.uint8, device="cuda")
+    assert lib.rbq_set_workspace(h, small.data_ptr(), 256) == -3
+    ws = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    assert lib.rbq_set_workspace(h, ws.data_ptr(), n) == 0
+    assert lib.rbq_estimate_scores(h, q.data_ptr(), C.byref(idx), None, None) == -1           # codes / scores null
+    with pytest.raises(rb.RbqError):
+        rb.rbq_topp_select(h, q, idx, 0.0, q, q)                                              # p must be > 0
+    assert lib.rbq_destroy(h) == 0
