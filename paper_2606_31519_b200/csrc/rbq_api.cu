@@ -16,18 +16,15 @@ void layout_workspace(rbq_ctx* c) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   c->off_qconst = take(B * Hkv * sizeof(RbqQConst));
-  c->off_rowstat = take(rows * 16);
   c->off_scores = take(rows * L * sizeof(float));
-  c->off_selidx = take(rows * L * sizeof(int32_t));
+  c->off_selbits = take(rows * (size_t)rbq_words_per_row(c) * sizeof(uint32_t));
   c->off_selcnt = take(rows * sizeof(int32_t));
-  c->max_chunks = (int)(rows * ((L + 255) / 256 + 1));
-  c->off_part = take((size_t)c->max_chunks * (RBQ_D + 2) * sizeof(float));
-  c->off_part_meta = take((rows + 1) * sizeof(int));
+  c->off_ulist = take(B * Hkv * L * sizeof(uint32_t));
+  c->off_ucount = take(B * Hkv * sizeof(int32_t));
+  c->off_part = take(rbq_attention_part_bytes(c));
   c->off_stage_q = take(rows * RBQ_D * sizeof(float));
   c->off_stage_out = take(rows * RBQ_D * sizeof(float));
   c->off_centroid = take(B * Hkv * 64 * RBQ_D * sizeof(double));
-  c->off_counters = take(256);
-  c->off_cand = off;
   c->total_bytes = off;
 }
 
@@ -215,10 +212,12 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
                     void* stream) {
   RBQ_CTX(ctx);
   RBQ_TRY(check_idx(ctx, idx, false));
+  RBQ_TRY(need_ws(ctx));
   if (!scores || !sel_idx || !sel_cnt) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores/sel_idx/sel_cnt null");
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
   if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
-  return rbq_launch_topp(ctx, scores, idx->n_indexed, p, sel_idx, sel_cnt, (cudaStream_t)stream);
+  return rbq_launch_topp(ctx, scores, idx->n_indexed, p, ws_ptr<uint32_t>(ctx, ctx->off_selbits), sel_idx, sel_cnt,
+                         (cudaStream_t)stream);
 }
 
 int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, const int32_t* sel_idx,
@@ -228,7 +227,9 @@ int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const
   RBQ_TRY(check_idx(ctx, idx, false));
   RBQ_TRY(need_ws(ctx));
   if (!q || !sel_idx || !sel_cnt || !out) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/sel_idx/sel_cnt/out null");
-  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, sel_idx, sel_cnt, out, lse, (cudaStream_t)stream);
+  uint32_t* bits = ws_ptr<uint32_t>(ctx, ctx->off_selbits);
+  RBQ_TRY(rbq_launch_bits_from_lists(ctx, idx, sel_idx, sel_cnt, bits, (cudaStream_t)stream));
+  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, lse, (cudaStream_t)stream);
 }
 
 int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, float p, void* out,
@@ -241,7 +242,7 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
   if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
   cudaStream_t s = (cudaStream_t)stream;
   float* scores = ws_ptr<float>(ctx, ctx->off_scores);
-  int32_t* si = sel_idx ? sel_idx : ws_ptr<int32_t>(ctx, ctx->off_selidx);
+  uint32_t* bits = ws_ptr<uint32_t>(ctx, ctx->off_selbits);
   int32_t* sn = sel_cnt ? sel_cnt : ws_ptr<int32_t>(ctx, ctx->off_selcnt);
   cudaEvent_t* ev = nullptr;                       // stage timing events of this step, if profiling
   if (ctx->prof_on && ctx->prof_steps < RBQ_PROFILE_MAX_STEPS) ev = ctx->prof_ev + (size_t)ctx->prof_steps++ * (RBQ_N_STAGES + 1);
@@ -251,11 +252,11 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  RBQ_TRY(rbq_launch_topp(ctx, scores, idx->n_indexed, p, si, sn, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
-  const int rc = rbq_launch_attention(ctx, q, dev_kv(cache), idx, si, sn, out, nullptr, s);   // records ev[4] before the merge
+  const int rc = rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
   ctx->stage_ev = nullptr;
-  if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[5], s));
+  if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[RBQ_N_STAGES], s));
   return rc;
 }
 

@@ -2,21 +2,438 @@
 // (Alg.2 lines 14-15, L188-190; L215 "K_local ... participate in the hybrid attention";
 // renormalised over the attended set, R7).
 //
-// HBM-bound gather of 2*D*sizeof(T) bytes per attended (token, q head) with ~4*D FLOP per row:
-// far below any compute roof, so the contraction stays on the FP32 pipe (no tensor cores) and the
-// design is about bytes in flight: flash-decoding split-K over the per-row index list, work = fixed
-// 256-token chunks of (sel_idx[row] ++ pending), distributed over a persistent grid sized from the
-// SM count; each half-warp reads one 256-byte K (then V) row per 128-bit load instruction, 8 rows
-// per warp in flight per operand; (m, l, o) partials per chunk, then a per-row merge.
+// The stage is an HBM-bound gather: 2*D*sizeof(T) bytes per attended (token, KV head).  The G query
+// heads of a KV group select different but overlapping sets, so the least the method must move is the
+// UNION of the group's sets -- that is what this path fetches, once:
+//   attn_plan_kernel   per KV group: OR of the G per-head selection bitmaps (written by S6) ->
+//                      compact ascending union list, entry = token | (head mask << 28), + its length.
+//   attn_gather_kernel persistent, one CTA per SM.  The concatenated union lists (+ pending windows) of
+//                      all groups are cut into equal contiguous ranges, one per CTA; inside a CTA each
+//                      warp runs a private 3-stage cp.async pipeline of 16-row K/V tiles (swizzled
+//                      shared memory, 128 KB in flight per SM) and contracts them on the tensor pipe:
+//                      S[head, token] = Q K^T and O += P V with mma.sync.m16n8k16.bf16 (heads on M, so
+//                      softmax statistics stay inside a quad, as in FlashAttention-2), head masks applied
+//                      to S.  The dot products are tiny (4*D FLOP per row and head); the tensor pipe is used
+//                      because it leaves the issue slots to the address generation of the gather.
+//   attn_merge_kernel  (m, l, o) partials of the CTAs that touched a group -> out, lse.
+// fp32 K/V or q (parity config 0) take the FP32-pipe kernel attn_simt_kernel over the same union lists.
 #include "rbq_common.cuh"
 
 namespace {
 
+// ---- bitmaps from caller-provided index lists (stand-alone rbq_sparse_attention) --------------------------------
+__global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, const int32_t* __restrict__ sel_cnt,
+                                       const int32_t* __restrict__ n_indexed, int Hq, int Lcap, int wpr,
+                                       uint32_t* __restrict__ bits) {
+  const int row = blockIdx.y, b = row / Hq;
+  const int cnt = min(sel_cnt[row], Lcap), n = n_indexed[b];
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += gridDim.x * blockDim.x) {
+    const int t = sel_idx[(size_t)row * Lcap + i];
+    if (t >= 0 && t < n) atomicOr(&bits[(size_t)row * wpr + (t >> 5)], 1u << (t & 31));
+  }
+}
+
+// ---- plan: union list per KV group ---------------------------------------------------------------------------------
+constexpr int PL_THREADS = 1024;
+constexpr int PL_SPLIT = 8;
+
+// grid = (PL_SPLIT, B*Hkv).  Every CTA of a group recomputes the prefix over the 128-token blocks (one block per
+// thread: 4 words x G heads), then its warps expand the blocks with blk % PL_SPLIT == blockIdx.x cooperatively
+// (lane = token bit of a word, position by popcount prefix).
+__global__ void __launch_bounds__(PL_THREADS)
+attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total,
+                 int Hq, int Hkv, int Lcap, int wpr, uint32_t* __restrict__ ulist, int32_t* __restrict__ ucount) {
+  __shared__ uint32_t s_warp[PL_THREADS / 32];
+  __shared__ uint32_t s_pre[PL_THREADS], s_cntb[PL_THREADS];
+  __shared__ uint32_t s_base;
+  const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nidx = max(0, n_indexed[b]);
+  const int nw = (nidx + 31) >> 5, nblk = (nw + 3) >> 2;
+  const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
+  uint32_t* out = ulist + (size_t)gi * Lcap;
+  if (tid == 0) s_base = 0;
+  __syncthreads();
+  for (int blk0 = 0; blk0 < nblk; blk0 += PL_THREADS) {
+    const int blk = blk0 + tid;
+    uint32_t uw[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int h = 0; h < RBQ_MAX_G; ++h) {
+      uint4 v = make_uint4(0u, 0u, 0u, 0u);
+      if (h < G && blk < nblk) v = *reinterpret_cast<const uint4*>(rows0 + (size_t)h * wpr + 4 * blk);
+      uw[0] |= v.x; uw[1] |= v.y; uw[2] |= v.z; uw[3] |= v.w;
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) if (4 * blk + k >= nw) uw[k] = 0u;   // words beyond the indexed prefix were never written
+    const uint32_t c = __popc(uw[0]) + __popc(uw[1]) + __popc(uw[2]) + __popc(uw[3]);
+    uint32_t si = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, si, o);
+      if (lane >= o) si += v;
+    }
+    if (lane == 31) s_warp[warp] = si;
+    __syncthreads();
+    uint32_t wp = 0, tot = 0;
+    for (int w = 0; w < PL_THREADS / 32; ++w) { if (w < warp) wp += s_warp[w]; tot += s_warp[w]; }
+    s_pre[tid] = s_base + wp + si - c;
+    s_cntb[tid] = c;
+    __syncthreads();
+    const unsigned lt = (1u << lane) - 1u;
+    for (int lb = (int)blockIdx.x + PL_SPLIT * warp; lb < PL_THREADS; lb += PL_SPLIT * (PL_THREADS / 32)) {
+      const int bk = blk0 + lb;
+      if (bk >= nblk || s_cntb[lb] == 0) continue;
+      uint32_t pos = s_pre[lb];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int wi = 4 * bk + k;
+        if (wi < nw) {
+          uint32_t u = 0, mask = 0;
+#pragma unroll
+          for (int h = 0; h < RBQ_MAX_G; ++h) {
+            if (h < G) {
+              const uint32_t hwv = rows0[(size_t)h * wpr + wi];
+              u |= hwv;
+              mask |= ((hwv >> lane) & 1u) << h;
+            }
+          }
+          if ((u >> lane) & 1u) out[pos + __popc(u & lt)] = (uint32_t)(wi * 32 + lane) | (mask << 28);
+          pos += __popc(u);
+        }
+      }
+    }
+    __syncthreads();
+    if (tid == 0) s_base += tot;
+    __syncthreads();
+  }
+  if (blockIdx.x == 0 && tid == 0) ucount[gi] = (int32_t)s_base;
+}
+
+// ---- shared by the gather kernels: exclusive prefix of attended rows per group ----------------------------------
+constexpr int AT_MAX_GROUPS = 2048;
+
+// s_start[gi] = sum over groups < gi of (ucount + pending); s_start[ngroups] = total.  Every CTA computes the same table.
+__device__ void build_group_table(const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
+                                  const int32_t* __restrict__ n_total, int ngroups, int Hkv, int* s_start, int* s_warp,
+                                  int nthreads) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  const int per = (ngroups + nthreads - 1) / nthreads;
+  const int g0 = tid * per;
+  int local = 0;
+  for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
+    const int b = gi / Hkv;
+    local += ucount[gi] + max(0, n_total[b] - max(0, n_indexed[b]));
+  }
+  int incl = local;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  int woff = 0, total = 0;
+  for (int w = 0; w < nwarps; ++w) { if (w < warp) woff += s_warp[w]; total += s_warp[w]; }
+  int run = woff + incl - local;
+  for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
+    const int b = gi / Hkv;
+    s_start[gi] = run;
+    run += ucount[gi] + max(0, n_total[b] - max(0, n_indexed[b]));
+  }
+  if (tid == 0) s_start[ngroups] = total;
+  __syncthreads();
+}
+
+__device__ __forceinline__ long long cta_begin(long long total, int c, int nc) { return total * c / nc; }
+
+// ---- tensor-pipe gather attention (bf16 K/V and q) ----------------------------------------------------------------------
+constexpr int GA_WARPS = 8;
+constexpr int GA_THREADS = GA_WARPS * 32;
+constexpr int GA_STAGES = 3;
+constexpr int GA_TILE = 16;                                   // rows per warp tile
+constexpr int GA_TILE_BYTES = GA_TILE * RBQ_D * 2;            // 4 KB per operand
+constexpr int GA_STAGE_BYTES = 2 * GA_TILE_BYTES;             // K + V
+constexpr int GA_SMEM = GA_WARPS * GA_STAGES * GA_STAGE_BYTES;   // 192 KB
+constexpr int GA_PART = RBQ_D + 2;                            // floats per (partial, head): o[128], m (base-2 units), l
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma_bf16(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&v);
+}
+
+// grid = number of SMs (persistent), GA_THREADS threads, GA_SMEM dynamic shared memory.
+// part: [gridDim.x + ngroups][G][GA_PART]; the partial of (CTA c, group gi) lives in slot c + gi.
+__global__ void __launch_bounds__(GA_THREADS, 1)
+attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ K, const __nv_bfloat16* __restrict__ V,
+                   long long sb, long long sh, long long st, const uint32_t* __restrict__ ulist,
+                   const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
+                   const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int Lcap, float scale_log2,
+                   float* __restrict__ part) {
+  extern __shared__ __align__(128) unsigned char ga_smem[];
+  __shared__ int s_start[AT_MAX_GROUPS + 1];
+  __shared__ int s_warp[GA_WARPS];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
+  const int G = Hq / Hkv;
+
+  build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
+  const long long total = s_start[ngroups];
+  const long long r0 = cta_begin(total, blockIdx.x, gridDim.x), r1 = cta_begin(total, blockIdx.x + 1, gridDim.x);
+  if (r0 >= r1) return;
+  // first group with s_start[gi + 1] > r0
+  int gi = 0;
+  {
+    int lo = 0, hi = ngroups - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if ((long long)s_start[mid + 1] > r0) hi = mid; else lo = mid + 1;
+    }
+    gi = lo;
+  }
+  unsigned char* my_smem = ga_smem + (size_t)warp * GA_STAGES * GA_STAGE_BYTES;
+  const uint32_t my_base = smem_u32(my_smem);
+
+  for (; gi < ngroups && (long long)s_start[gi] < r1; ++gi) {
+    const long long ga = s_start[gi], gb = s_start[gi + 1];
+    const int a = (int)(max(r0, ga) - ga), e = (int)(min(r1, gb) - ga);   // group-local rank range of this CTA
+    if (a >= e) continue;
+    const int b = gi / Hkv, g = gi % Hkv;
+    const int usel = ucount[gi], nidx = max(0, n_indexed[b]);
+    const __nv_bfloat16* Kb = K + (long long)b * sb + (long long)g * sh;
+    const __nv_bfloat16* Vb = V + (long long)b * sb + (long long)g * sh;
+    const uint32_t* ul = ulist + (size_t)gi * Lcap;
+
+    // A operand: Q rows of the group's heads (rows >= G are zero)
+    uint32_t qa[8][2];
+    {
+      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * RBQ_D);
+#pragma unroll
+      for (int ks = 0; ks < 8; ++ks) {
+        qa[ks][0] = (g4 < G) ? qp[8 * ks + t4] : 0u;
+        qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
+      }
+    }
+    float m_run = -INFINITY, l_run = 0.0f;
+    float o[16][4];
+#pragma unroll
+    for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.0f; o[nt][1] = 0.0f; o[nt][2] = 0.0f; o[nt][3] = 0.0f; }
+
+    const int ntiles = (e - a + GA_TILE - 1) / GA_TILE;
+    const int my_tiles = (ntiles > warp) ? (ntiles - warp + GA_WARPS - 1) / GA_WARPS : 0;
+
+    // entry of row `lane` (lanes 0..15) of tile i of this warp: token | mask << 28 (mask 0 = padding row)
+    auto tile_entry = [&](int i) -> uint32_t {
+      const int r = a + (warp + i * GA_WARPS) * GA_TILE + lane;
+      uint32_t ent = 0u;
+      if (lane < GA_TILE && r < e) ent = (r < usel) ? ul[r] : ((uint32_t)(nidx + (r - usel)) | (0xFu << 28));
+      return ent;
+    };
+    auto issue = [&](int i, uint32_t ent) {
+      const uint32_t sbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES);
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int row = 2 * k + (lane >> 4), ch = lane & 15;
+        const uint32_t re = __shfl_sync(0xffffffffu, ent, row);
+        const long long off = (long long)(re & 0x0FFFFFFFu) * st + ch * 8;
+        const uint32_t d = sbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4));
+        cp_async16(d, Kb + off);
+        cp_async16(d + GA_TILE_BYTES, Vb + off);
+      }
+    };
+    uint32_t ent_next[GA_STAGES - 1];
+#pragma unroll
+    for (int s = 0; s < GA_STAGES - 1; ++s) {
+      ent_next[s] = 0u;
+      if (s < my_tiles) { ent_next[s] = tile_entry(s); issue(s, ent_next[s]); }
+      cp_async_commit();
+    }
+    for (int i = 0; i < my_tiles; ++i) {
+      const uint32_t ent = ent_next[0];
+#pragma unroll
+      for (int s = 0; s + 1 < GA_STAGES - 1; ++s) ent_next[s] = ent_next[s + 1];
+      const int nx = i + GA_STAGES - 1;
+      ent_next[GA_STAGES - 2] = 0u;
+      if (nx < my_tiles) { ent_next[GA_STAGES - 2] = tile_entry(nx); issue(nx, ent_next[GA_STAGES - 2]); }
+      cp_async_commit();
+      cp_async_wait<GA_STAGES - 1>();
+      __syncwarp();
+      const uint32_t kbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES), vbase = kbase + GA_TILE_BYTES;
+
+      // S = Q K^T : two n-tiles of 8 tokens
+      float s[2][4];
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        s[nt][0] = 0.0f; s[nt][1] = 0.0f; s[nt][2] = 0.0f; s[nt][3] = 0.0f;
+        const int row = nt * 8 + (lane & 7);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          uint32_t bf[4];
+          const int ch = 4 * j + (lane >> 3);
+          ldsm_x4(bf, kbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4)));
+          mma_bf16(s[nt], qa[2 * j][0], 0u, qa[2 * j][1], 0u, bf[0], bf[1]);
+          mma_bf16(s[nt], qa[2 * j + 1][0], 0u, qa[2 * j + 1][1], 0u, bf[2], bf[3]);
+        }
+      }
+      // head masks, online softmax (row = head g4; this lane: tokens nt*8 + 2*t4, +1)
+      float tmax = -INFINITY;
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        const uint32_t e0 = __shfl_sync(0xffffffffu, ent, nt * 8 + 2 * t4);
+        const uint32_t e1 = __shfl_sync(0xffffffffu, ent, nt * 8 + 2 * t4 + 1);
+        const bool ok0 = (e0 >> (28 + (g4 & 3))) & 1u, ok1 = (e1 >> (28 + (g4 & 3))) & 1u;
+        s[nt][0] = (ok0 && g4 < G) ? s[nt][0] * scale_log2 : -INFINITY;
+        s[nt][1] = (ok1 && g4 < G) ? s[nt][1] * scale_log2 : -INFINITY;
+        tmax = fmaxf(tmax, fmaxf(s[nt][0], s[nt][1]));
+      }
+      tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+      tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+      const float m_new = fmaxf(m_run, tmax);
+      const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+      const float resc = exp2f(m_run - m_use);                 // m_run = -inf -> 0
+      m_run = m_new;
+      const float p00 = exp2f(s[0][0] - m_use), p01 = exp2f(s[0][1] - m_use);
+      const float p10 = exp2f(s[1][0] - m_use), p11 = exp2f(s[1][1] - m_use);
+      l_run = l_run * resc + ((p00 + p01) + (p10 + p11));
+      // P as bf16 hi + lo parts (two MMAs per V tile): keeps ~16 mantissa bits of the probabilities
+      const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+      const uint32_t pb0 = pack_bf16(p00 - rbq_bf16lo(pa0), p01 - rbq_bf16hi(pa0));
+      const uint32_t pb2 = pack_bf16(p10 - rbq_bf16lo(pa2), p11 - rbq_bf16hi(pa2));
+      // O = O * resc + P V
+#pragma unroll
+      for (int c2 = 0; c2 < 8; ++c2) {
+        uint32_t bf[4];
+        const int row = (lane & 7) + ((lane >> 3) & 1) * 8, ch = 2 * c2 + (lane >> 4);
+        ldsm_x4_t(bf, vbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4)));
+        o[2 * c2][0] *= resc; o[2 * c2][1] *= resc;
+        o[2 * c2 + 1][0] *= resc; o[2 * c2 + 1][1] *= resc;
+        mma_bf16(o[2 * c2], pa0, 0u, pa2, 0u, bf[0], bf[1]);
+        mma_bf16(o[2 * c2 + 1], pa0, 0u, pa2, 0u, bf[2], bf[3]);
+        mma_bf16(o[2 * c2], pb0, 0u, pb2, 0u, bf[0], bf[1]);
+        mma_bf16(o[2 * c2 + 1], pb0, 0u, pb2, 0u, bf[2], bf[3]);
+      }
+      __syncwarp();                                            // tile consumed before its stage is refilled
+    }
+    cp_async_wait<0>();
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
+
+    // merge the warps of the CTA (staging area aliases the drained pipeline buffers)
+    __syncthreads();
+    float* stg = reinterpret_cast<float*>(ga_smem);            // [GA_WARPS][G][GA_PART]
+    if (g4 < G) {
+      float* dst = stg + ((size_t)warp * G + g4) * GA_PART;
+#pragma unroll
+      for (int nt = 0; nt < 16; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
+      if (t4 == 0) { dst[RBQ_D] = m_run; dst[RBQ_D + 1] = l_run; }
+    }
+    __syncthreads();
+    float* pdst = part + (size_t)(blockIdx.x + gi) * G * GA_PART;
+    for (int idx = tid; idx < G * RBQ_D; idx += GA_THREADS) {
+      const int h = idx / RBQ_D, d = idx % RBQ_D;
+      float mm = -INFINITY;
+#pragma unroll
+      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[((size_t)w * G + h) * GA_PART + RBQ_D]);
+      float oo = 0.0f, ll = 0.0f;
+#pragma unroll
+      for (int w = 0; w < GA_WARPS; ++w) {
+        const float* sp = stg + ((size_t)w * G + h) * GA_PART;
+        const float f = (sp[RBQ_D] == -INFINITY) ? 0.0f : exp2f(sp[RBQ_D] - mm);
+        oo = fmaf(f, sp[d], oo);
+        ll = fmaf(f, sp[RBQ_D + 1], ll);
+      }
+      pdst[(size_t)h * GA_PART + d] = oo;
+      if (d == 0) { pdst[(size_t)h * GA_PART + RBQ_D] = mm; pdst[(size_t)h * GA_PART + RBQ_D + 1] = ll; }
+    }
+    __syncthreads();                                           // staging area free before the next group's pipeline
+  }
+}
+
+// grid = B*Hq rows, 256 threads = 2 slices x 128 dims.  Partial slots of the row's group: every CTA c whose range
+// intersects the group, slot c + gi.  m is in base-2 units (scaled by log2 e).  (m, l) of all slots are staged
+// first so that the o loop has independent loads.
+constexpr int MG_MAX_SLOTS = 256;
+
+template <typename TO>
+__global__ void __launch_bounds__(256)
+attn_merge_kernel(const float* __restrict__ part, const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
+                  const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int nc, TO* __restrict__ out,
+                  float* __restrict__ lse) {
+  __shared__ int s_start[AT_MAX_GROUPS + 1];
+  __shared__ int s_warp[8];
+  __shared__ float s_m[MG_MAX_SLOTS], s_f[MG_MAX_SLOTS], s_l[MG_MAX_SLOTS];
+  __shared__ float s_o[RBQ_D];
+  const int row = blockIdx.x, b = row / Hq, h = row % Hq, G = Hq / Hkv;
+  const int gi = b * Hkv + h / G, hl = h % G;
+  const int tid = threadIdx.x, d = tid & 127, slice = tid >> 7;
+  build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, 256);
+  const long long total = s_start[ngroups], ga = s_start[gi], gb = s_start[gi + 1];
+  int c0 = 0, nslots = 0;
+  if (gb > ga) {
+    c0 = (int)min((long long)nc - 1, ga * nc / max(total, 1ll));
+    while (c0 > 0 && cta_begin(total, c0, nc) > ga) --c0;
+    while (c0 + 1 < nc && cta_begin(total, c0 + 1, nc) <= ga) ++c0;
+    int c1 = (int)min((long long)nc - 1, (gb - 1) * nc / max(total, 1ll));
+    while (c1 > 0 && cta_begin(total, c1, nc) > gb - 1) --c1;
+    while (c1 + 1 < nc && cta_begin(total, c1 + 1, nc) <= gb - 1) ++c1;
+    nslots = c1 - c0 + 1;
+  }
+  const float* pbase = part + ((size_t)(c0 + gi) * G + hl) * GA_PART;
+  const size_t pstride = (size_t)G * GA_PART;
+  for (int i = tid; i < nslots; i += 256) {
+    const int c = c0 + i;
+    const long long x0 = max(cta_begin(total, c, nc), ga), x1 = min(cta_begin(total, c + 1, nc), gb);
+    float pm = -INFINITY, pl = 0.0f;
+    if (x0 < x1) { pm = pbase[i * pstride + RBQ_D]; pl = pbase[i * pstride + RBQ_D + 1]; }
+    s_m[i] = pm; s_l[i] = pl;
+  }
+  __syncthreads();
+  float mm = -INFINITY;
+  for (int i = 0; i < nslots; ++i) mm = fmaxf(mm, s_m[i]);
+  for (int i = tid; i < nslots; i += 256) s_f[i] = (s_m[i] == -INFINITY) ? 0.0f : exp2f(s_m[i] - mm);
+  __syncthreads();
+  float o = 0.0f, l = 0.0f;
+#pragma unroll 8
+  for (int i = slice; i < nslots; i += 2) {
+    const float f = s_f[i];
+    const float v = (f != 0.0f) ? pbase[i * pstride + d] : 0.0f;
+    o = fmaf(f, v, o);
+  }
+  for (int i = 0; i < nslots; ++i) l = fmaf(s_f[i], s_l[i], l);
+  if (slice == 1) s_o[d] = o;
+  __syncthreads();
+  if (slice == 0) {
+    o += s_o[d];
+    const bool empty = !(l > 0.0f);
+    rbq_st_elem(out, (long long)row * RBQ_D + d, empty ? 0.0f : o / l);
+    if (lse && d == 0) lse[row] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(l);
+  }
+}
+
+// ---- FP32-pipe kernel for fp32 K/V or q (parity config 0): split-K over the group's union list ---------------------
 constexpr int AT_THREADS = 256;
 constexpr int AT_WARPS = AT_THREADS / 32;
-constexpr int AT_CHUNK = AT_WARPS * 32;       // tokens per chunk: one 32-token strip per warp
+constexpr int AT_CHUNK = AT_WARPS * 32;       // union rows per chunk: one 32-row strip per warp
 constexpr int AT_PART = RBQ_D + 2;            // floats per partial: o[128], m, l
-constexpr int AT_MAX_ROWS = 4096;
 
 struct Row8 { float v[8]; };
 
@@ -34,175 +451,138 @@ __device__ __forceinline__ Row8 load8(const float* p) {
   return r;
 }
 
-// exclusive prefix of per-row chunk counts into s_start[0..rows]; every CTA computes the same table
-__device__ void build_chunk_table(const int32_t* __restrict__ sel_cnt, const int32_t* __restrict__ n_indexed,
-                                  const int32_t* __restrict__ n_total, int rows, int Hq, int* s_start, int* s_warp) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int per = (rows + AT_THREADS - 1) / AT_THREADS;
-  const int r0 = tid * per;
-  int local = 0;
-  for (int r = r0; r < min(rows, r0 + per); ++r) {
-    const int b = r / Hq;
-    const int na = sel_cnt[r] + max(0, n_total[b] - n_indexed[b]);
-    local += (na + AT_CHUNK - 1) / AT_CHUNK;
-  }
-  int incl = local;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int v = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += v;
-  }
-  if (lane == 31) s_warp[warp] = incl;
-  __syncthreads();
-  int woff = 0;
-  for (int w = 0; w < warp; ++w) woff += s_warp[w];
-  int run = woff + incl - local;
-  for (int r = r0; r < min(rows, r0 + per); ++r) {
-    const int b = r / Hq;
-    const int na = sel_cnt[r] + max(0, n_total[b] - n_indexed[b]);
-    s_start[r] = run;
-    run += (na + AT_CHUNK - 1) / AT_CHUNK;
-  }
-  if (tid == AT_THREADS - 1) s_start[rows] = woff + incl;     // rows beyond the last thread's block are empty
-  __syncthreads();
-  // threads whose block starts beyond `rows` wrote nothing; the last thread holds the grand total
-}
-
+// grid = (max chunks per group, B*Hq rows).  Chunk ch of row (b,h) covers union rows [ch*256, ch*256+256) of the
+// row's KV group; rows whose head-mask bit is clear are skipped.  part: [rows][max_chunks][AT_PART].
 template <typename T, typename TQ>
 __global__ void __launch_bounds__(AT_THREADS)
-attn_chunk_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __restrict__ V, long long sb, long long sh,
-                  long long st, const int32_t* __restrict__ sel_idx, const int32_t* __restrict__ sel_cnt,
-                  const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total, int rows, int Hq, int Hkv,
-                  int Lcap, float sm_scale, float* __restrict__ part, int* __restrict__ chunk_start) {
-  __shared__ int s_start[AT_MAX_ROWS + 1];
-  __shared__ int s_warp[AT_WARPS];
+attn_simt_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __restrict__ V, long long sb, long long sh,
+                 long long st, const uint32_t* __restrict__ ulist, const int32_t* __restrict__ ucount,
+                 const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total, int Hq, int Hkv, int Lcap,
+                 float sm_scale, int max_chunks, float* __restrict__ part) {
   __shared__ float s_part[AT_WARPS][AT_PART];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int half = lane >> 4, c = lane & 15;                  // half-warp per row, 8 dims per lane
   const int G = Hq / Hkv;
+  const int row = blockIdx.y, b = row / Hq, h = row % Hq, g = h / G, hl = h % G;
+  const int gi = b * Hkv + g;
+  const int usel = ucount[gi], nidx = max(0, n_indexed[b]);
+  const int na = usel + max(0, n_total[b] - nidx);
+  const int ch = blockIdx.x;
+  float* dst = part + ((size_t)row * max_chunks + ch) * AT_PART;
+  if (ch * AT_CHUNK >= na) {
+    if (tid == 0) { dst[RBQ_D] = -INFINITY; dst[RBQ_D + 1] = 0.0f; }
+    return;
+  }
+  const int i0 = ch * AT_CHUNK + warp * 32;
+  const int nw = max(0, min(32, na - i0));
+  const T* Kb = K + (long long)b * sb + (long long)g * sh;
+  const T* Vb = V + (long long)b * sb + (long long)g * sh;
+  const uint32_t* ul = ulist + (size_t)gi * Lcap;
 
-  build_chunk_table(sel_cnt, n_indexed, n_total, rows, Hq, s_start, s_warp);
-  const int total = s_start[rows];
-  if (blockIdx.x == 0)
-    for (int r = tid; r <= rows; r += AT_THREADS) chunk_start[r] = s_start[r];
+  Row8 qv;
+  {
+    const TQ* qp = q + ((size_t)row * RBQ_D + c * 8);
+#pragma unroll
+    for (int d = 0; d < 8; ++d) qv.v[d] = rbq_ld_elem(qp, d);
+  }
+  uint32_t my_ent = 0u;                                         // token | mask << 28 ; mask bit clear = not attended by this head
+  if (lane < nw) {
+    const int it = i0 + lane;
+    my_ent = (it < usel) ? ul[it] : ((uint32_t)(nidx + (it - usel)) | (0xFu << 28));
+  }
+  float m = -INFINITY, l = 0.0f, acc[8];
+#pragma unroll
+  for (int d = 0; d < 8; ++d) acc[d] = 0.0f;
 
-  for (int ch = blockIdx.x; ch < total; ch += gridDim.x) {
-    // row of this chunk: last r with s_start[r] <= ch
-    int lo = 0, hi = rows - 1;
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (s_start[mid] <= ch) lo = mid; else hi = mid - 1;
+  for (int base = 0; base < nw; base += 8) {
+    Row8 kr[4], vr[4];
+    bool ok[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int item = base + 2 * j + half;
+      const uint32_t ent = __shfl_sync(0xffffffffu, my_ent, item & 31);
+      ok[j] = (item < nw) && ((ent >> (28 + hl)) & 1u);
+      const long long off = (long long)(ent & 0x0FFFFFFFu) * st + c * 8;
+      kr[j] = load8(Kb + off);                                  // masked items read a valid row: harmless
+      vr[j] = load8(Vb + off);
     }
-    const int row = lo, b = row / Hq, h = row % Hq, g = h / G;
-    const int cnt = sel_cnt[row], nidx = n_indexed[b];
-    const int na = cnt + max(0, n_total[b] - nidx);
-    const int i0 = (ch - s_start[row]) * AT_CHUNK + warp * 32;   // first item of this warp's strip
-    const int nw = max(0, min(32, na - i0));
-    const T* Kb = K + (long long)b * sb + (long long)g * sh;
-    const T* Vb = V + (long long)b * sb + (long long)g * sh;
-
-    Row8 qv;
-    {
-      const TQ* qp = q + ((size_t)row * RBQ_D + c * 8);
+    float s[4];
 #pragma unroll
-      for (int d = 0; d < 8; ++d) qv.v[d] = rbq_ld_elem(qp, d);
+    for (int j = 0; j < 4; ++j) {
+      float d0 = 0.0f;
+#pragma unroll
+      for (int d = 0; d < 8; ++d) d0 = fmaf(qv.v[d], kr[j].v[d], d0);
+      s[j] = d0;
     }
-    // this lane's item -> token index
-    int my_tok = 0;
-    if (lane < nw) {
-      const int it = i0 + lane;
-      my_tok = (it < cnt) ? sel_idx[(size_t)row * Lcap + it] : nidx + (it - cnt);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) s[j] += __shfl_xor_sync(0xffffffffu, s[j], o);
+    float gmax = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      s[j] = ok[j] ? s[j] * sm_scale : -INFINITY;
+      gmax = fmaxf(gmax, s[j]);
     }
-    float m = -INFINITY, l = 0.0f, acc[8];
+    gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, 16));
+    const float m_new = fmaxf(m, gmax);
+    const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+    const float resc = __expf(m - m_use);                       // m = -inf -> 0
+    l *= resc;
 #pragma unroll
-    for (int d = 0; d < 8; ++d) acc[d] = 0.0f;
-
-    for (int base = 0; base < nw; base += 8) {
-      Row8 kr[4], vr[4];
-      bool ok[4];
+    for (int d = 0; d < 8; ++d) acc[d] *= resc;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int item = base + 2 * j + half;
-        const int tok = __shfl_sync(0xffffffffu, my_tok, item & 31);
-        ok[j] = item < nw;
-        const long long off = (long long)tok * st + c * 8;
-        kr[j] = load8(Kb + off);                                // masked items read token 0: harmless
-        vr[j] = load8(Vb + off);
-      }
-      float s[4];
+    for (int j = 0; j < 4; ++j) {
+      const float p = __expf(s[j] - m_use);                     // masked: exp(-inf) = 0
+      l += p;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        float d0 = 0.0f;
-#pragma unroll
-        for (int d = 0; d < 8; ++d) d0 = fmaf(qv.v[d], kr[j].v[d], d0);
-        s[j] = d0;
-      }
-#pragma unroll
-      for (int o = 8; o > 0; o >>= 1)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) s[j] += __shfl_xor_sync(0xffffffffu, s[j], o);
-      float gmax = -INFINITY;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        s[j] = ok[j] ? s[j] * sm_scale : -INFINITY;
-        gmax = fmaxf(gmax, s[j]);
-      }
-      gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, 16));
-      const float m_new = fmaxf(m, gmax);                        // finite: item `base` is always valid
-      const float resc = __expf(m - m_new);                      // m = -inf -> 0
-      l *= resc;
-#pragma unroll
-      for (int d = 0; d < 8; ++d) acc[d] *= resc;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const float p = __expf(s[j] - m_new);                    // masked: exp(-inf) = 0
-        l += p;
-#pragma unroll
-        for (int d = 0; d < 8; ++d) acc[d] = fmaf(p, vr[j].v[d], acc[d]);
-      }
-      m = m_new;
+      for (int d = 0; d < 8; ++d) acc[d] = fmaf(p, vr[j].v[d], acc[d]);
     }
-    // merge the two half-warps (same m), then the warps of the CTA
-    l += __shfl_xor_sync(0xffffffffu, l, 16);
+    m = m_new;
+  }
+  // merge the two half-warps (same m), then the warps of the CTA
+  l += __shfl_xor_sync(0xffffffffu, l, 16);
 #pragma unroll
-    for (int d = 0; d < 8; ++d) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], 16);
-    if (half == 0) {
+  for (int d = 0; d < 8; ++d) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], 16);
+  if (half == 0) {
 #pragma unroll
-      for (int d = 0; d < 8; ++d) s_part[warp][c * 8 + d] = acc[d];
-      if (c == 0) { s_part[warp][RBQ_D] = m; s_part[warp][RBQ_D + 1] = l; }
+    for (int d = 0; d < 8; ++d) s_part[warp][c * 8 + d] = acc[d];
+    if (c == 0) { s_part[warp][RBQ_D] = m; s_part[warp][RBQ_D + 1] = l; }
+  }
+  __syncthreads();
+  if (tid < RBQ_D) {
+    float mm = -INFINITY;
+#pragma unroll
+    for (int w = 0; w < AT_WARPS; ++w) mm = fmaxf(mm, s_part[w][RBQ_D]);
+    float o = 0.0f, ll = 0.0f;
+#pragma unroll
+    for (int w = 0; w < AT_WARPS; ++w) {
+      const float mw = s_part[w][RBQ_D];
+      const float f = (mw == -INFINITY) ? 0.0f : __expf(mw - mm);
+      o = fmaf(f, s_part[w][tid], o);
+      ll = fmaf(f, s_part[w][RBQ_D + 1], ll);
     }
-    __syncthreads();
-    if (tid < RBQ_D) {
-      float mm = -INFINITY;
-#pragma unroll
-      for (int w = 0; w < AT_WARPS; ++w) mm = fmaxf(mm, s_part[w][RBQ_D]);
-      float o = 0.0f, ll = 0.0f;
-#pragma unroll
-      for (int w = 0; w < AT_WARPS; ++w) {
-        const float mw = s_part[w][RBQ_D];
-        const float f = (mw == -INFINITY) ? 0.0f : __expf(mw - mm);
-        o = fmaf(f, s_part[w][tid], o);
-        ll = fmaf(f, s_part[w][RBQ_D + 1], ll);
-      }
-      float* dst = part + (size_t)ch * AT_PART;
-      dst[tid] = o;
-      if (tid == 0) { dst[RBQ_D] = mm; dst[RBQ_D + 1] = ll; }
-    }
-    __syncthreads();
+    dst[tid] = o;
+    if (tid == 0) { dst[RBQ_D] = mm; dst[RBQ_D + 1] = ll; }
   }
 }
 
+// grid = rows, 128 threads; natural-log units
 template <typename TO>
 __global__ void __launch_bounds__(RBQ_D)
-attn_merge_kernel(const float* __restrict__ part, const int* __restrict__ chunk_start, TO* __restrict__ out,
-                  float* __restrict__ lse) {
-  const int row = blockIdx.x, d = threadIdx.x;
-  const int c0 = chunk_start[row], c1 = chunk_start[row + 1];
+attn_simt_merge_kernel(const float* __restrict__ part, const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
+                       const int32_t* __restrict__ n_total, int Hq, int Hkv, int max_chunks, TO* __restrict__ out,
+                       float* __restrict__ lse) {
+  const int row = blockIdx.x, d = threadIdx.x, b = row / Hq, G = Hq / Hkv;
+  const int gi = b * Hkv + (row % Hq) / G;
+  const int na = ucount[gi] + max(0, n_total[b] - max(0, n_indexed[b]));
+  const int nch = min(max_chunks, (na + AT_CHUNK - 1) / AT_CHUNK);
+  const float* base = part + (size_t)row * max_chunks * AT_PART;
   float mm = -INFINITY;
-  for (int ch = c0; ch < c1; ++ch) mm = fmaxf(mm, part[(size_t)ch * AT_PART + RBQ_D]);
+  for (int ch = 0; ch < nch; ++ch) mm = fmaxf(mm, base[(size_t)ch * AT_PART + RBQ_D]);
   float o = 0.0f, l = 0.0f;
-  for (int ch = c0; ch < c1; ++ch) {
-    const float* p = part + (size_t)ch * AT_PART;
+  for (int ch = 0; ch < nch; ++ch) {
+    const float* p = base + (size_t)ch * AT_PART;
     const float f = (p[RBQ_D] == -INFINITY) ? 0.0f : __expf(p[RBQ_D] - mm);
     o = fmaf(f, p[d], o);
     l = fmaf(f, p[RBQ_D + 1], l);
@@ -213,38 +593,89 @@ attn_merge_kernel(const float* __restrict__ part, const int* __restrict__ chunk_
 }
 
 template <typename T, typename TQ>
-int launch_chunks(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const int32_t* sel_idx,
-                  const int32_t* sel_cnt, float* part, int* chunk_start, cudaStream_t s) {
+int launch_simt(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* ulist, const int32_t* ucount,
+                int max_chunks, float* part, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
-  const int grid = ctx->sm_count * 4;
-  attn_chunk_kernel<T, TQ><<<grid, AT_THREADS, 0, s>>>((const TQ*)q, (const T*)kv.k, (const T*)kv.v, kv.sb, kv.sh, kv.st,
-                                                       sel_idx, sel_cnt, idx->n_indexed, idx->n_total, rows,
-                                                       ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
-                                                       ctx->sm_scale, part, chunk_start);
+  dim3 grid(max_chunks, rows);
+  attn_simt_kernel<T, TQ><<<grid, AT_THREADS, 0, s>>>((const TQ*)q, (const T*)kv.k, (const T*)kv.v, kv.sb, kv.sh, kv.st, ulist,
+                                                      ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                      ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->sm_scale, max_chunks, part);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
 }  // namespace
 
-int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const int32_t* sel_idx,
-                         const int32_t* sel_cnt, void* out, float* lse, cudaStream_t s) {
+size_t rbq_attention_part_bytes(const rbq_ctx* ctx) {
+  const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads, groups = (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads;
+  const bool mma = ctx->cfg.kv_dtype == RBQ_BF16 && ctx->cfg.q_dtype == RBQ_BF16;
+  if (mma) return ((size_t)ctx->sm_count + groups) * ctx->G * GA_PART * sizeof(float);
+  const size_t max_chunks = ((size_t)ctx->cfg.max_tokens + AT_CHUNK - 1) / AT_CHUNK;
+  return rows * max_chunks * AT_PART * sizeof(float);
+}
+
+int rbq_launch_bits_from_lists(rbq_ctx* ctx, const rbq_index* idx, const int32_t* sel_idx, const int32_t* sel_cnt, uint32_t* bits,
+                               cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
-  if (rows > AT_MAX_ROWS) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch*n_q_heads %d > %d", rows, AT_MAX_ROWS);
-  float* part = reinterpret_cast<float*>(static_cast<char*>(ctx->ws) + ctx->off_part);
-  int* chunk_start = reinterpret_cast<int*>(static_cast<char*>(ctx->ws) + ctx->off_part_meta);
-  const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
-  int rc;
-  if (kbf && qbf) rc = launch_chunks<__nv_bfloat16, __nv_bfloat16>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
-  else if (kbf) rc = launch_chunks<__nv_bfloat16, float>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
-  else if (qbf) rc = launch_chunks<float, __nv_bfloat16>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
-  else rc = launch_chunks<float, float>(ctx, q, kv, idx, sel_idx, sel_cnt, part, chunk_start, s);
-  if (rc != RBQ_OK) return rc;
+  const int wpr = rbq_words_per_row(ctx);
+  RBQ_CUDA_OK(ctx, cudaMemsetAsync(bits, 0, (size_t)rows * wpr * sizeof(uint32_t), s));
+  dim3 grid(max(1, min(64, (ctx->cfg.max_tokens + 255) / 256)), rows);
+  bits_from_lists_kernel<<<grid, 256, 0, s>>>(sel_idx, sel_cnt, idx->n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, wpr, bits);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
+
+// S7 from the per-row selection bitmaps in the workspace: plan -> gather -> merge.
+int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits, void* out,
+                         float* lse, cudaStream_t s) {
+  const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads, groups = ctx->cfg.batch * ctx->cfg.n_kv_heads;
+  if (groups > AT_MAX_GROUPS) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch*n_kv_heads %d > %d", groups, AT_MAX_GROUPS);
+  const int wpr = rbq_words_per_row(ctx);
+  char* ws = static_cast<char*>(ctx->ws);
+  uint32_t* ulist = reinterpret_cast<uint32_t*>(ws + ctx->off_ulist);
+  int32_t* ucount = reinterpret_cast<int32_t*>(ws + ctx->off_ucount);
+  float* part = reinterpret_cast<float*>(ws + ctx->off_part);
+  attn_plan_kernel<<<dim3(PL_SPLIT, groups), PL_THREADS, 0, s>>>(bits, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                                 ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount);
+  RBQ_LAUNCH_OK(ctx);
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
+  const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
+  if (kbf && qbf) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(attn_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GA_SMEM));
+      attr_set = true;
+    }
+    const int nc = ctx->sm_count;
+    attn_gather_kernel<<<nc, GA_THREADS, GA_SMEM, s>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)kv.k,
+                                                       (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, ulist, ucount,
+                                                       idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
+                                                       ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
+                                                       ctx->sm_scale * 1.4426950408889634f, part);
+    RBQ_LAUNCH_OK(ctx);
+    if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[5], s));
+    if (ctx->cfg.out_dtype == RBQ_BF16)
+      attn_merge_kernel<<<rows, 256, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
+                                             ctx->cfg.n_kv_heads, nc, (__nv_bfloat16*)out, lse);
+    else
+      attn_merge_kernel<<<rows, 256, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
+                                             ctx->cfg.n_kv_heads, nc, (float*)out, lse);
+    RBQ_LAUNCH_OK(ctx);
+    return RBQ_OK;
+  }
+  const int max_chunks = (ctx->cfg.max_tokens + AT_CHUNK - 1) / AT_CHUNK;
+  int rc;
+  if (kbf) rc = launch_simt<__nv_bfloat16, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  else if (qbf) rc = launch_simt<float, __nv_bfloat16>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  else rc = launch_simt<float, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  if (rc != RBQ_OK) return rc;
+  if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[5], s));
   if (ctx->cfg.out_dtype == RBQ_BF16)
-    attn_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, chunk_start, (__nv_bfloat16*)out, lse);
+    attn_simt_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                  ctx->cfg.n_kv_heads, max_chunks, (__nv_bfloat16*)out, lse);
   else
-    attn_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, chunk_start, (float*)out, lse);
+    attn_simt_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                  ctx->cfg.n_kv_heads, max_chunks, (float*)out, lse);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

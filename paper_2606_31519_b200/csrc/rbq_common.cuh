@@ -40,9 +40,8 @@ struct rbq_ctx {
   void* ws;
   size_t ws_bytes;
   // workspace carve-up (byte offsets), filled by rbq_layout_workspace
-  size_t off_qconst, off_rowstat, off_scores, off_selidx, off_selcnt, off_part, off_part_meta,
-      off_stage_q, off_stage_out, off_centroid, off_counters, off_cand, total_bytes;
-  int max_chunks;
+  size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_part,
+      off_stage_q, off_stage_out, off_centroid, total_bytes;
   cudaEvent_t ev_copy, ev_flush;
   int pending;               // host shadow of n_total - n_indexed (uniform over the batch)
   int in_flight;             // rows encoded by an enqueued flush, not yet committed
@@ -105,7 +104,14 @@ int rbq_launch_append_copy(rbq_ctx*, const void* k_new, const void* v_new, int n
 int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, float* qparams, cudaStream_t);
 int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop,
                         cudaStream_t);
-int rbq_launch_topp(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx,
-                    int32_t* sel_cnt, cudaStream_t);
-int rbq_launch_attention(rbq_ctx*, const void* q, const RbqKV&, const rbq_index*, const int32_t* sel_idx,
-                         const int32_t* sel_cnt, void* out, float* lse, cudaStream_t);
+// S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.
+int rbq_launch_topp(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, uint32_t* sel_bits,
+                    int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
+int rbq_launch_bits_from_lists(rbq_ctx*, const rbq_index*, const int32_t* sel_idx, const int32_t* sel_cnt,
+                               uint32_t* sel_bits, cudaStream_t);
+// S7 from the selection bitmaps: union plan -> gather attention -> merge.
+int rbq_launch_attention(rbq_ctx*, const void* q, const RbqKV&, const rbq_index*, const uint32_t* sel_bits,
+                         void* out, float* lse, cudaStream_t);
+size_t rbq_attention_part_bytes(const rbq_ctx*);
+// 32-bit words per bitmap row, padded to a multiple of 4 (16-byte vector loads)
+static inline int rbq_words_per_row(const rbq_ctx* c) { return (((c->cfg.max_tokens + 31) / 32) + 3) & ~3; }

@@ -21,12 +21,15 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   const int h = g * G + min(hs, G - 1);              // slices beyond G recompute head G-1, write nothing
   const size_t row = (size_t)b * Hq + h;
 
+  extern __shared__ __align__(16) float s_rot[];  // dense: P [D][D] staged with one round of independent 128-bit loads
+  __shared__ float s_ck[RBQ_D], s_cq[RBQ_MAX_G][RBQ_D];
   __shared__ float s_x[RBQ_MAX_G][RBQ_D];      // xq, then u
   __shared__ float s_y[RBQ_MAX_G][RBQ_D];      // q'
   __shared__ float s_red[RBQ_MAX_G][8];        // per-warp min / max
   __shared__ int s_isum[RBQ_MAX_G][4];
   __shared__ float s_qn[RBQ_MAX_G];
   __shared__ double s_dot[RBQ_MAX_G][2];
+  __shared__ double s_dred[RBQ_MAX_G][2][4];
   __shared__ uint8_t s_qu[RBQ_MAX_G][RBQ_D];
 
   const float qv = rbq_ld_elem(q, row * RBQ_D + j);
@@ -35,27 +38,38 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   const float xq = c_q ? __fsub_rn(qv, cqv) : qv;
   s_x[hs][j] = xq;
   s_y[hs][j] = qv;                               // staged for the fp64 dot chains below
-  __syncthreads();
-  // three sequential chains per head, on three different threads (orders of DESIGN.md R1)
-  if (j == 0) {
-    float n2 = 0.0f;
-    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(s_x[hs][i], s_x[hs][i], n2);
-    s_qn[hs] = __fsqrt_rn(n2);
-  } else if (j == 32) {                          // <q, c_k> : fp64, i ascending
-    double a = 0.0;
-    const float* ck = c_k + (size_t)bg * RBQ_D;
-    for (int i = 0; i < RBQ_D; ++i) a = fma((double)s_y[hs][i], (double)ck[i], a);
-    s_dot[hs][0] = a;
-  } else if (j == 64) {                          // <c_q, c_k>
-    double a = 0.0;
-    if (c_q) {
-      const float* ck = c_k + (size_t)bg * RBQ_D;
-      const float* cq = c_q + row * RBQ_D;
-      for (int i = 0; i < RBQ_D; ++i) a = fma((double)cq[i], (double)ck[i], a);
-    }
-    s_dot[hs][1] = a;
+  s_cq[hs][j] = cqv;
+  if (hs == 0) s_ck[j] = ckv;
+  if (rot_kind == RBQ_ROT_DENSE) {
+    const float4* src = reinterpret_cast<const float4*>(rot);
+    float4* dst = reinterpret_cast<float4*>(s_rot);
+#pragma unroll 8
+    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x) dst[i] = src[i];
   }
   __syncthreads();
+  // ||xq||: the canonical sequential fp32 chain (R1) on one thread per head; the two fp64 dot products
+  // <q,c_k>, <c_q,c_k> (exact products, fp64 sums, rounded to fp32 at the end) as a fixed reduction tree.
+  {
+    double p0 = (double)qv * (double)ckv;
+    double p1 = c_q ? (double)cqv * (double)ckv : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      p0 += __shfl_xor_sync(0xffffffffu, p0, o);
+      p1 += __shfl_xor_sync(0xffffffffu, p1, o);
+    }
+    if ((j & 31) == 0) { s_dred[hs][0][j >> 5] = p0; s_dred[hs][1][j >> 5] = p1; }
+  }
+  if (j == 0) {
+    float n2 = 0.0f;
+#pragma unroll 16
+    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(s_x[hs][i], s_x[hs][i], n2);
+    s_qn[hs] = __fsqrt_rn(n2);
+  }
+  __syncthreads();
+  if (j == 0) {
+    s_dot[hs][0] = (s_dred[hs][0][0] + s_dred[hs][0][1]) + (s_dred[hs][0][2] + s_dred[hs][0][3]);
+    s_dot[hs][1] = (s_dred[hs][1][0] + s_dred[hs][1][1]) + (s_dred[hs][1][2] + s_dred[hs][1][3]);
+  }
   const float qn = s_qn[hs];
   const float u = (qn > 0.0f) ? __fdiv_rn(xq, qn) : 0.0f;
   s_x[hs][j] = u;
@@ -64,8 +78,8 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   float qp;
   if (rot_kind == RBQ_ROT_DENSE) {
     float acc = 0.0f;
-#pragma unroll 8
-    for (int i = 0; i < RBQ_D; ++i) acc = fmaf(s_x[hs][i], rot[i * RBQ_D + j], acc);
+#pragma unroll 32
+    for (int i = 0; i < RBQ_D; ++i) acc = fmaf(s_x[hs][i], s_rot[i * RBQ_D + j], acc);
     qp = acc;
   } else {
     // warp 0 of the slice runs the 128-point butterflies (4 elements per lane), as in S1
@@ -168,12 +182,19 @@ int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t*
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   RbqQConst* qc = reinterpret_cast<RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
   const int threads = max(256, ctx->G * RBQ_D);
+  const size_t smem = ctx->cfg.rot_kind == RBQ_ROT_DENSE ? (size_t)RBQ_D * RBQ_D * sizeof(float) : 0;
+  static bool attr_set = false;
+  if (!attr_set) {
+    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(query_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_D * RBQ_D * 4));
+    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(query_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_D * RBQ_D * 4));
+    attr_set = true;
+  }
   if (ctx->cfg.q_dtype == RBQ_BF16)
-    query_kernel<<<BG, threads, 0, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                        ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+    query_kernel<<<BG, threads, smem, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
   else
-    query_kernel<<<BG, threads, 0, s>>>((const float*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                        ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+    query_kernel<<<BG, threads, smem, s>>>((const float*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

@@ -32,7 +32,12 @@ def _chained(orc, w, rot, kind, p, with_cq=False):
     # fused call
     sel_idx2, sel_cnt2 = c.new_sel()
     c.decode_step(q, p, out2, sel_idx2, sel_cnt2)
+    # fused call without index lists: the selection stays a bitmap in the workspace
+    out3, sel_cnt3 = c.new_out(), c.new_sel()[1]
+    c.decode_step(q, p, out3, None, sel_cnt3)
     torch.cuda.synchronize()
+    assert (out3.cpu().numpy().view(np.uint32) == out2.cpu().numpy().view(np.uint32)).all(), "fused without lists != fused"
+    assert (sel_cnt3.cpu().numpy() == sel_cnt2.cpu().numpy()).all()
     s = scores.cpu().numpy()
     U.assert_logits_close(s, o["scores"], w.seq_lens, w.Hq)
     idx, cnt = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy()

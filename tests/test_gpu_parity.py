@@ -285,6 +285,34 @@ def test_topp_edge_rows(orc, rot128):
     c.close()
 
 
+@pytest.mark.parametrize("B,L", [(1, 40000), (8, 3000), (16, 2100), (3, 90)])
+def test_topp_cluster_sizes(orc, rot128, B, L):
+    """Every cluster size of the Top-p kernel (8 / 4 / 2 / 1 CTAs per row, chosen from the row count), rows
+    shorter than one bitmap word per CTA, and the fused step without index lists (sel_idx = NULL)."""
+    import torch
+    rng = np.random.default_rng(5 + B)
+    w = U.workload(3, L=L, B=B)
+    rows, Lc = w.B * w.Hq, w.Lcap
+    n_seq = w.seq_lens.copy()
+    scores = (rng.standard_normal((w.B, w.Hq, Lc)) * rng.uniform(0.5, 6.0, (w.B, w.Hq, 1))).astype(np.float32)
+    scores[:, 0, :] = np.round(scores[:, 0, :] * 2) / 2            # heavy ties
+    o = dict(codes=np.zeros((w.B, w.Hkv, Lc, 4), np.uint32), f_scale=np.zeros((w.B, w.Hkv, Lc), np.float32),
+             c_k=np.zeros((w.B, w.Hkv, 128), np.float32), n_indexed=n_seq, n_total=n_seq)
+    c = U.make_cache(w, rot128[0], upload_kv=False)
+    U.load_index(c, o)
+    for p in (0.5, 0.9):
+        ref_idx, ref_cnt = orc.topp(scores.reshape(rows, Lc), np.repeat(n_seq, w.Hq), p)
+        ref_idx, ref_cnt = ref_idx.reshape(w.B, w.Hq, Lc), ref_cnt.reshape(w.B, w.Hq)
+        idx, cnt = _run_topp(c, scores, p)
+        for b in range(w.B):
+            n = int(n_seq[b])
+            for h in range(w.Hq):
+                g = idx[b, h, :cnt[b, h]]
+                assert (np.diff(g) > 0).all() and g.min() >= 0 and g.max() < n
+                U.assert_topp_row(scores[b, h, :n], g, ref_idx[b, h, :ref_cnt[b, h]], p)
+    c.close()
+
+
 def test_topp_literal_config_tie_break(orc, rot128):
     """P9: literal BASELINE config 0 (sink keys = 2 x query): Top-p(0.9) = {0,1,2,3}, Top-p(0.7) = {0,1,2}."""
     import torch
