@@ -165,12 +165,12 @@ int64_t rbq_launch_count(const rbq_ctx* ctx);
 
 /* ---- per-stage device timing of rbq_decode_step (measurement aid) ----------------- */
 /* Stages: 0 = S3 query prep, 1 = S4/S5 estimator, 2 = S6 Top-p, 3 = S7 union plan, 4 = S7 gather
- * attention, 5 = S7 merge.  While enabled, every rbq_decode_step records RBQ_N_STAGES + 1 timing
+ * attention (including the merge of its partials).  While enabled, every rbq_decode_step records RBQ_N_STAGES + 1 timing
  * events on its stream (up to RBQ_PROFILE_MAX_STEPS steps, later steps are not recorded).
  * rbq_profile_read BLOCKS until the recorded steps have finished (the only call that waits),
  * writes the summed milliseconds per stage to ms_host[RBQ_N_STAGES] and the number of recorded
  * steps to n_steps_host, and clears the record.                                                  */
-#define RBQ_N_STAGES 6
+#define RBQ_N_STAGES 5
 #define RBQ_PROFILE_MAX_STEPS 512
 int rbq_profile_enable(rbq_ctx* ctx, int enable);
 int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host);

@@ -29,8 +29,8 @@ EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspac
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
            "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_sparse_attention",
            "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read"]
-N_STAGES = 6
-STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather", "attn_merge"]
+N_STAGES = 5
+STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather"]
 
 
 class RbqError(RuntimeError):

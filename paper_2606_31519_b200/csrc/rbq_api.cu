@@ -21,6 +21,8 @@ void layout_workspace(rbq_ctx* c) {
   c->off_selcnt = take(rows * sizeof(int32_t));
   c->off_ulist = take(B * Hkv * L * sizeof(uint32_t));
   c->off_ucount = take(B * Hkv * sizeof(int32_t));
+  c->off_gdone = take(B * Hkv * sizeof(int32_t));
+  c->off_rowmax = take(rows * sizeof(uint32_t));
   c->off_part = take(rbq_attention_part_bytes(c));
   c->off_stage_q = take(rows * RBQ_D * sizeof(float));
   c->off_stage_out = take(rows * RBQ_D * sizeof(float));
@@ -216,7 +218,7 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
   if (!scores || !sel_idx || !sel_cnt) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores/sel_idx/sel_cnt null");
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
   if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
-  return rbq_launch_topp(ctx, scores, idx->n_indexed, p, ws_ptr<uint32_t>(ctx, ctx->off_selbits), sel_idx, sel_cnt,
+  return rbq_launch_topp(ctx, scores, nullptr, idx->n_indexed, p, ws_ptr<uint32_t>(ctx, ctx->off_selbits), sel_idx, sel_cnt,
                          (cudaStream_t)stream);
 }
 
@@ -252,7 +254,7 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  RBQ_TRY(rbq_launch_topp(ctx, scores, idx->n_indexed, p, bits, sel_idx, sn, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, ws_ptr<uint32_t>(ctx, ctx->off_rowmax), idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
   const int rc = rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
   ctx->stage_ev = nullptr;

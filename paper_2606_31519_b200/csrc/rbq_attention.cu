@@ -15,7 +15,8 @@
 //                      softmax statistics stay inside a quad, as in FlashAttention-2), head masks applied
 //                      to S.  The dot products are tiny (4*D FLOP per row and head); the tensor pipe is used
 //                      because it leaves the issue slots to the address generation of the gather.
-//   attn_merge_kernel  (m, l, o) partials of the CTAs that touched a group -> out, lse.
+//                      The last CTA to finish a group (arrival counter) merges the group's (m, l, o) partials
+//                      into out / lse, so no merge launch sits on the critical path.
 // fp32 K/V or q (parity config 0) take the FP32-pipe kernel attn_simt_kernel over the same union lists.
 #include "rbq_common.cuh"
 
@@ -42,7 +43,8 @@ constexpr int PL_SPLIT = 8;
 // (lane = token bit of a word, position by popcount prefix).
 __global__ void __launch_bounds__(PL_THREADS)
 attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total,
-                 int Hq, int Hkv, int Lcap, int wpr, uint32_t* __restrict__ ulist, int32_t* __restrict__ ucount) {
+                 int Hq, int Hkv, int Lcap, int wpr, uint32_t* __restrict__ ulist, int32_t* __restrict__ ucount,
+                 int32_t* __restrict__ gdone) {
   __shared__ uint32_t s_warp[PL_THREADS / 32];
   __shared__ uint32_t s_pre[PL_THREADS], s_cntb[PL_THREADS];
   __shared__ uint32_t s_base;
@@ -106,7 +108,7 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
     if (tid == 0) s_base += tot;
     __syncthreads();
   }
-  if (blockIdx.x == 0 && tid == 0) ucount[gi] = (int32_t)s_base;
+  if (blockIdx.x == 0 && tid == 0) { ucount[gi] = (int32_t)s_base; gdone[gi] = 0; }
 }
 
 // ---- shared by the gather kernels: exclusive prefix of attended rows per group ----------------------------------
@@ -154,7 +156,7 @@ constexpr int GA_TILE = 16;                                   // rows per warp t
 constexpr int GA_TILE_BYTES = GA_TILE * RBQ_D * 2;            // 4 KB per operand
 constexpr int GA_STAGE_BYTES = 2 * GA_TILE_BYTES;             // K + V
 constexpr int GA_SMEM = GA_WARPS * GA_STAGES * GA_STAGE_BYTES;   // 192 KB
-constexpr int GA_PART = RBQ_D + 2;                            // floats per (partial, head): o[128], m (base-2 units), l
+constexpr int GA_PART = RBQ_D + 4;                            // floats per (partial, head): o[128], m (base-2 units), l, pad (16-byte rows)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
@@ -188,16 +190,29 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
                    long long sb, long long sh, long long st, const uint32_t* __restrict__ ulist,
                    const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
                    const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int Lcap, float scale_log2,
-                   float* __restrict__ part) {
+                   float* __restrict__ part, int32_t* __restrict__ gdone, void* __restrict__ out, int out_bf16,
+                   float* __restrict__ lse) {
   extern __shared__ __align__(128) unsigned char ga_smem[];
   __shared__ int s_start[AT_MAX_GROUPS + 1];
   __shared__ int s_warp[GA_WARPS];
+  __shared__ int s_last, s_clo, s_chi;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
   const int G = Hq / Hkv;
 
   build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
   const long long total = s_start[ngroups];
+  if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
+    for (int e = tid; e < ngroups * G * RBQ_D; e += GA_THREADS) {
+      const int gq = e / (G * RBQ_D), hd = e % (G * RBQ_D);
+      if (s_start[gq + 1] == s_start[gq]) {
+        const size_t orow = (size_t)(gq / Hkv) * Hq + (size_t)(gq % Hkv) * G + hd / RBQ_D;
+        if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * RBQ_D + hd % RBQ_D] = __float2bfloat16_rn(0.0f);
+        else reinterpret_cast<float*>(out)[orow * RBQ_D + hd % RBQ_D] = 0.0f;
+        if (lse && hd % RBQ_D == 0) lse[orow] = -INFINITY;
+      }
+    }
+  }
   const long long r0 = cta_begin(total, blockIdx.x, gridDim.x), r1 = cta_begin(total, blockIdx.x + 1, gridDim.x);
   if (r0 >= r1) return;
   // first group with s_start[gi + 1] > r0
@@ -364,68 +379,85 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       pdst[(size_t)h * GA_PART + d] = oo;
       if (d == 0) { pdst[(size_t)h * GA_PART + RBQ_D] = mm; pdst[(size_t)h * GA_PART + RBQ_D + 1] = ll; }
     }
+    // ---- arrival: the last CTA that finishes a group merges the group's partials into out / lse -------------------------
+    __threadfence();
+    const int nc = (int)gridDim.x;
+    const bool touches = tid < nc && max(cta_begin(total, tid, nc), ga) < min(cta_begin(total, tid + 1, nc), gb);
+    if (tid == 0) { s_clo = nc; s_chi = -1; }
+    const int expected = __syncthreads_count(touches);         // also: staging area free, partial stores fenced
+    if (touches) { atomicMin(&s_clo, tid); atomicMax(&s_chi, tid); }
+    if (tid == 0) s_last = (atomicAdd(&gdone[gi], 1) == expected - 1);
+    __syncthreads();
+    if (s_last) {
+      __threadfence();
+      float* s_f = stg;                                        // [G][GA_THREADS]: m of slot c, then its factor 2^(m - max)
+      float* s_l = stg + RBQ_MAX_G * GA_THREADS;
+      float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [128] second half's partial sums
+      const int clo = s_clo, chi = s_chi;
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        float pm = -INFINITY, pl = 0.0f;
+        if (h < G && touches) {
+          const float* pp = part + ((size_t)(tid + gi) * G + h) * GA_PART;
+          pm = __ldcg(pp + RBQ_D); pl = __ldcg(pp + RBQ_D + 1);
+        }
+        s_f[h * GA_THREADS + tid] = pm; s_l[h * GA_THREADS + tid] = pl;
+      }
+      __syncthreads();
+      const int item = tid & 127, half = tid >> 7, h = item >> 5, d4 = (item & 31) * 4;
+      float mm = -INFINITY;
+      if (h < G) for (int c = clo; c <= chi; ++c) mm = fmaxf(mm, s_f[h * GA_THREADS + c]);
+      __syncthreads();
+#pragma unroll
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) {                  // thread tid converts slot tid: needs the max of every head
+        float mh = -INFINITY;
+        if (hh < G) for (int c = clo; c <= chi; ++c) mh = fmaxf(mh, s_f[hh * GA_THREADS + c]);
+        const float mc = s_f[hh * GA_THREADS + tid];
+        __syncthreads();
+        s_f[hh * GA_THREADS + tid] = (mc == -INFINITY) ? 0.0f : exp2f(mc - mh);
+      }
+      __syncthreads();
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      float ll = 0.0f;
+      if (h < G) {
+        const float* pcol = part + ((size_t)gi * G + h) * GA_PART + d4;
+        const size_t pstride = (size_t)G * GA_PART;
+        for (int c0 = clo + half; c0 <= chi; c0 += 16) {
+          float f[8];
+          float4 v[8];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const int c = c0 + 2 * k;
+            f[k] = (c <= chi) ? s_f[h * GA_THREADS + c] : 0.0f;
+            v[k] = (f[k] != 0.0f) ? __ldcg(reinterpret_cast<const float4*>(pcol + (size_t)c * pstride)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            acc.x = fmaf(f[k], v[k].x, acc.x); acc.y = fmaf(f[k], v[k].y, acc.y);
+            acc.z = fmaf(f[k], v[k].z, acc.z); acc.w = fmaf(f[k], v[k].w, acc.w);
+          }
+        }
+        for (int c = clo; c <= chi; ++c) ll = fmaf(s_f[h * GA_THREADS + c], s_l[h * GA_THREADS + c], ll);
+      }
+      if (half == 1) s_o[item] = acc;
+      __syncthreads();
+      if (half == 0 && h < G) {
+        const float4 o2 = s_o[item];
+        acc.x += o2.x; acc.y += o2.y; acc.z += o2.z; acc.w += o2.w;
+        const bool empty = !(ll > 0.0f);
+        const float inv = empty ? 0.0f : 1.0f / ll;
+        const size_t orow = (size_t)b * Hq + (size_t)g * G + h;
+        const float r4[4] = {acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * RBQ_D + d4 + k] = __float2bfloat16_rn(r4[k]);
+          else reinterpret_cast<float*>(out)[orow * RBQ_D + d4 + k] = r4[k];
+        }
+        if (lse && d4 == 0) lse[orow] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(ll);
+      }
+      if (tid == 0) gdone[gi] = 0;                             // ready for the next step
+    }
     __syncthreads();                                           // staging area free before the next group's pipeline
-  }
-}
-
-// grid = B*Hq rows, 256 threads = 2 slices x 128 dims.  Partial slots of the row's group: every CTA c whose range
-// intersects the group, slot c + gi.  m is in base-2 units (scaled by log2 e).  (m, l) of all slots are staged
-// first so that the o loop has independent loads.
-constexpr int MG_MAX_SLOTS = 256;
-
-template <typename TO>
-__global__ void __launch_bounds__(256)
-attn_merge_kernel(const float* __restrict__ part, const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
-                  const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int nc, TO* __restrict__ out,
-                  float* __restrict__ lse) {
-  __shared__ int s_start[AT_MAX_GROUPS + 1];
-  __shared__ int s_warp[8];
-  __shared__ float s_m[MG_MAX_SLOTS], s_f[MG_MAX_SLOTS], s_l[MG_MAX_SLOTS];
-  __shared__ float s_o[RBQ_D];
-  const int row = blockIdx.x, b = row / Hq, h = row % Hq, G = Hq / Hkv;
-  const int gi = b * Hkv + h / G, hl = h % G;
-  const int tid = threadIdx.x, d = tid & 127, slice = tid >> 7;
-  build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, 256);
-  const long long total = s_start[ngroups], ga = s_start[gi], gb = s_start[gi + 1];
-  int c0 = 0, nslots = 0;
-  if (gb > ga) {
-    c0 = (int)min((long long)nc - 1, ga * nc / max(total, 1ll));
-    while (c0 > 0 && cta_begin(total, c0, nc) > ga) --c0;
-    while (c0 + 1 < nc && cta_begin(total, c0 + 1, nc) <= ga) ++c0;
-    int c1 = (int)min((long long)nc - 1, (gb - 1) * nc / max(total, 1ll));
-    while (c1 > 0 && cta_begin(total, c1, nc) > gb - 1) --c1;
-    while (c1 + 1 < nc && cta_begin(total, c1 + 1, nc) <= gb - 1) ++c1;
-    nslots = c1 - c0 + 1;
-  }
-  const float* pbase = part + ((size_t)(c0 + gi) * G + hl) * GA_PART;
-  const size_t pstride = (size_t)G * GA_PART;
-  for (int i = tid; i < nslots; i += 256) {
-    const int c = c0 + i;
-    const long long x0 = max(cta_begin(total, c, nc), ga), x1 = min(cta_begin(total, c + 1, nc), gb);
-    float pm = -INFINITY, pl = 0.0f;
-    if (x0 < x1) { pm = pbase[i * pstride + RBQ_D]; pl = pbase[i * pstride + RBQ_D + 1]; }
-    s_m[i] = pm; s_l[i] = pl;
-  }
-  __syncthreads();
-  float mm = -INFINITY;
-  for (int i = 0; i < nslots; ++i) mm = fmaxf(mm, s_m[i]);
-  for (int i = tid; i < nslots; i += 256) s_f[i] = (s_m[i] == -INFINITY) ? 0.0f : exp2f(s_m[i] - mm);
-  __syncthreads();
-  float o = 0.0f, l = 0.0f;
-#pragma unroll 8
-  for (int i = slice; i < nslots; i += 2) {
-    const float f = s_f[i];
-    const float v = (f != 0.0f) ? pbase[i * pstride + d] : 0.0f;
-    o = fmaf(f, v, o);
-  }
-  for (int i = 0; i < nslots; ++i) l = fmaf(s_f[i], s_l[i], l);
-  if (slice == 1) s_o[d] = o;
-  __syncthreads();
-  if (slice == 0) {
-    o += s_o[d];
-    const bool empty = !(l > 0.0f);
-    rbq_st_elem(out, (long long)row * RBQ_D + d, empty ? 0.0f : o / l);
-    if (lse && d == 0) lse[row] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(l);
   }
 }
 
@@ -635,8 +667,9 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   uint32_t* ulist = reinterpret_cast<uint32_t*>(ws + ctx->off_ulist);
   int32_t* ucount = reinterpret_cast<int32_t*>(ws + ctx->off_ucount);
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
+  int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
   attn_plan_kernel<<<dim3(PL_SPLIT, groups), PL_THREADS, 0, s>>>(bits, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
-                                                                 ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount);
+                                                                 ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount, gdone);
   RBQ_LAUNCH_OK(ctx);
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
@@ -646,20 +679,13 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
       RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(attn_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GA_SMEM));
       attr_set = true;
     }
-    const int nc = ctx->sm_count;
+    const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the arrival count uses one thread per CTA
     attn_gather_kernel<<<nc, GA_THREADS, GA_SMEM, s>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)kv.k,
                                                        (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, ulist, ucount,
                                                        idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
                                                        ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
-                                                       ctx->sm_scale * 1.4426950408889634f, part);
-    RBQ_LAUNCH_OK(ctx);
-    if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[5], s));
-    if (ctx->cfg.out_dtype == RBQ_BF16)
-      attn_merge_kernel<<<rows, 256, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
-                                             ctx->cfg.n_kv_heads, nc, (__nv_bfloat16*)out, lse);
-    else
-      attn_merge_kernel<<<rows, 256, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
-                                             ctx->cfg.n_kv_heads, nc, (float*)out, lse);
+                                                       ctx->sm_scale * 1.4426950408889634f, part, gdone, out,
+                                                       ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse);
     RBQ_LAUNCH_OK(ctx);
     return RBQ_OK;
   }
@@ -669,7 +695,6 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   else if (qbf) rc = launch_simt<float, __nv_bfloat16>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
   else rc = launch_simt<float, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
   if (rc != RBQ_OK) return rc;
-  if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[5], s));
   if (ctx->cfg.out_dtype == RBQ_BF16)
     attn_simt_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
                                                   ctx->cfg.n_kv_heads, max_chunks, (__nv_bfloat16*)out, lse);

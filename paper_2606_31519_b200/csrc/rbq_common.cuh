@@ -40,7 +40,7 @@ struct rbq_ctx {
   void* ws;
   size_t ws_bytes;
   // workspace carve-up (byte offsets), filled by rbq_layout_workspace
-  size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_part,
+  size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_gdone, off_rowmax, off_part,
       off_stage_q, off_stage_out, off_centroid, total_bytes;
   cudaEvent_t ev_copy, ev_flush;
   int pending;               // host shadow of n_total - n_indexed (uniform over the batch)
@@ -105,8 +105,9 @@ int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, flo
 int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop,
                         cudaStream_t);
 // S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.
-int rbq_launch_topp(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, uint32_t* sel_bits,
-                    int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
+// rowmax_key: order-preserving keys of the row maxima [B*Hq] (written by S5), or NULL to compute them here.
+int rbq_launch_topp(rbq_ctx*, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p,
+                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
 int rbq_launch_bits_from_lists(rbq_ctx*, const rbq_index*, const int32_t* sel_idx, const int32_t* sel_cnt,
                                uint32_t* sel_bits, cudaStream_t);
 // S7 from the selection bitmaps: union plan -> gather attention -> merge.

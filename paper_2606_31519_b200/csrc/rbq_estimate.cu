@@ -10,8 +10,12 @@
 // and mma.sync.m16n8k32.u8.u8.s32 (native IMMA.16832 on sm_100a) contracts 16 tokens x 128 dims
 // against 8 columns = G query heads interleaved with all-ones columns (the latter yield
 // 8*popcount(c_b) for free).  The K permutation implied by the masks is baked into the B fragments
-// by S3.  Codes and factors are staged HBM -> shared memory by TMA bulk copies (cp.async.bulk +
-// mbarrier), all stages of a CTA in flight at once; warps consume 32-token groups.
+// by S3.
+//
+// Streaming: no shared memory.  The 32-token groups of all (sequence, KV head) pairs form one flat
+// list that is cut into equal contiguous ranges, one per WARP (grid = a multiple of the SM count);
+// a warp keeps two groups of loads in flight.  MMA rows are mapped to tokens so that lane (g, t)
+// ends up with head t's logits of tokens 4g..4g+3: one 16-byte coalesced store per lane and group.
 //
 // Integer results are exact.  Epilogue in fp32 without cancellation:
 //   acc_d = 4*(2*dot - sum(qu)), acc_p = 4*(2*pop - D)   (exact ints: accumulators start at
@@ -22,32 +26,8 @@
 namespace {
 
 constexpr int EST_THREADS = 256;
-constexpr int EST_STAGES = 4;
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "LAB_WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra LAB_DONE_%=;\n"
-      "bra LAB_WAIT_%=;\n"
-      "LAB_DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
+constexpr int EST_WARPS = EST_THREADS / 32;
+constexpr int EST_MAX_B = 1024;               // sequences whose group prefix fits the shared table
 
 __device__ __forceinline__ void imma_16832(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                            uint32_t b0, uint32_t b1) {
@@ -65,108 +45,148 @@ __device__ __forceinline__ void tile_mma(int (&c)[4], uint32_t wa, uint32_t wb, 
   imma_16832(c, ha & 0x04040404u, hb & 0x04040404u, ha & 0x08080808u, hb & 0x08080808u, bf[3][0], bf[3][1]);
 }
 
-// grid = (ceil(Lcap / SPAN), B*Hkv); SPAN = EST_STAGES * TS tokens per CTA.
-template <int TS, bool INT_OUT, bool HAS_BIAS>
-__global__ void __launch_bounds__(EST_THREADS)
+struct GroupLoad {            // what lane (g, t) needs of one 32-token group
+  uint32_t w[4];              // word t of tokens 4g .. 4g+3
+  float4 fs;                  // f_scale of tokens 4g .. 4g+3
+};
+
+__device__ __forceinline__ GroupLoad load_group(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
+                                                size_t tok0, int g, int t, int tmax) {
+  // tok0: flat index of the group's first token in [B*Hkv][Lcap]; tmax: tokens of this group that exist in the
+  // allocation (>= 1, multiple of 4 because Lcap is); lanes beyond it load nothing.
+  GroupLoad r;
+  const bool ok = 4 * g < tmax;
+  const uint32_t* p = codes + (tok0 + 4 * g) * RBQ_WORDS + t;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) r.w[k] = ok ? __ldg(p + k * RBQ_WORDS) : 0u;
+  r.fs = ok ? __ldg(reinterpret_cast<const float4*>(f_scale + tok0 + 4 * g)) : make_float4(0.f, 0.f, 0.f, 0.f);
+  return r;
+}
+
+// grid = k * SMs CTAs of EST_WARPS warps.  Flat group index -> (sequence b, KV head, 32-token group).
+template <bool INT_OUT, bool HAS_BIAS>
+__global__ void __launch_bounds__(EST_THREADS, 4)
 estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
                 const float* __restrict__ f_bias, const int32_t* __restrict__ n_indexed,
-                const RbqQConst* __restrict__ qconst, int Hq, int Hkv, int Lcap, float sm_scale,
-                float* __restrict__ scores, int32_t* __restrict__ dot_out, int32_t* __restrict__ pop_out) {
-  constexpr int SPAN = EST_STAGES * TS;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  uint4* s_codes = reinterpret_cast<uint4*>(smem_raw);                           // [SPAN]
-  float* s_fs = reinterpret_cast<float*>(smem_raw + (size_t)SPAN * 16);           // [SPAN]
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)SPAN * 20);    // [EST_STAGES]
-
-  const int bg = blockIdx.y, b = bg / Hkv, gk = bg % Hkv, G = Hq / Hkv;
-  const int n = n_indexed[b];
-  const int t0 = blockIdx.x * SPAN;
-  if (t0 >= n) return;
-  const int cnt = min(SPAN, n - t0);
+                const RbqQConst* __restrict__ qconst, int B, int Hq, int Hkv, int Lcap, float sm_scale,
+                float* __restrict__ scores, int32_t* __restrict__ dot_out, int32_t* __restrict__ pop_out,
+                uint32_t* __restrict__ rowmax_key) {
+  __shared__ int s_gstart[EST_MAX_B + 1];     // exclusive prefix over sequences of Hkv * ceil(n_b / 32)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-
+  const int g = lane >> 2, t = lane & 3, G = Hq / Hkv;
   if (tid == 0) {
-    for (int s = 0; s < EST_STAGES; ++s) mbar_init(&s_bar[s], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    const size_t tok0 = (size_t)bg * Lcap + t0;
-    for (int s = 0; s < EST_STAGES; ++s) {
-      const int c = min(TS, cnt - s * TS);
-      if (c <= 0) break;
-      const int c4 = (c + 3) & ~3;                         // f_scale bytes must be a multiple of 16
-      mbar_expect_tx(&s_bar[s], (uint32_t)(c * 16 + c4 * 4));
-      bulk_g2s(s_codes + s * TS, codes + (tok0 + (size_t)s * TS) * RBQ_WORDS, (uint32_t)(c * 16), &s_bar[s]);
-      bulk_g2s(s_fs + s * TS, f_scale + tok0 + (size_t)s * TS, (uint32_t)(c4 * 4), &s_bar[s]);
-    }
+    int run = 0;
+    for (int b = 0; b < B; ++b) { s_gstart[b] = run; run += Hkv * ((max(0, n_indexed[b]) + 31) >> 5); }
+    s_gstart[B] = run;
   }
-  // per-warp constants: B fragments (8 regs) and this lane's head constants
-  const RbqQConst* qc = qconst + bg;
-  const int g = lane >> 2, t = lane & 3;
-  uint32_t bf[4][2];
-#pragma unroll
-  for (int s = 0; s < 4; ++s) {
-    const uint2 v = *reinterpret_cast<const uint2*>(&qc->bfrag[s][lane][0]);
-    bf[s][0] = v.x; bf[s][1] = v.y;
+  __syncthreads();
+  const long long total = s_gstart[B];
+  const long long nwarps = (long long)gridDim.x * EST_WARPS, wid = (long long)blockIdx.x * EST_WARPS + warp;
+  long long gcur = total * wid / nwarps;
+  const long long gend = total * (wid + 1) / nwarps;
+  if (gcur >= gend) return;
+  int b = 0;
+  {
+    int lo = 0, hi = B - 1;                    // last b with s_gstart[b] <= gcur
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if ((long long)s_gstart[mid] <= gcur) lo = mid; else hi = mid - 1; }
+    b = lo;
   }
   const bool head_ok = t < G;
   const int hsel = head_ok ? t : 0;
-  const float cA = qc->cA[hsel], cB = qc->cB[hsel], cD = qc->cD[hsel];
-  const int init_d = qc->init_d[hsel], init_p = qc->init_p;
-  const size_t row = ((size_t)b * Hq + gk * G + hsel) * Lcap;
-  const size_t prow = (size_t)bg * Lcap;
-  __syncthreads();                                         // barrier inits visible to all waiters
 
-  const uint32_t* s_words = reinterpret_cast<const uint32_t*>(s_codes);
-  const int ngroups = (cnt + 31) >> 5;
-  for (int gi = warp; gi < ngroups; gi += EST_THREADS / 32) {
-    const int base = gi << 5;                              // token offset inside the span
-    mbar_wait(&s_bar[base / TS], 0);
-    // lane (g,t) holds word t of tokens base+g, +8, +16, +24 (conflict-free: 4*(base+g)+t)
-    const uint32_t w0 = s_words[(base + g) * 4 + t];
-    const uint32_t w1 = s_words[(base + g + 8) * 4 + t];
-    const uint32_t w2 = s_words[(base + g + 16) * 4 + t];
-    const uint32_t w3 = s_words[(base + g + 24) * 4 + t];
-    int c0[4] = {init_d, init_p, init_d, init_p};
-    int c1[4] = {init_d, init_p, init_d, init_p};
-    tile_mma(c0, w0, w1, bf);
-    tile_mma(c1, w2, w3, bf);
-    const int acc_d[4] = {c0[0], c0[2], c1[0], c1[2]};
-    const int acc_p[4] = {c0[1], c0[3], c1[1], c1[3]};
+  while (gcur < gend) {
+    // segment: groups of one (b, KV head) handled by this warp
+    while ((long long)s_gstart[b + 1] <= gcur) ++b;
+    const int n = n_indexed[b];
+    const int gpb = (n + 31) >> 5;                              // groups per (b, KV head)
+    const int rel = (int)(gcur - s_gstart[b]);
+    const int gk = rel / gpb, g0 = rel % gpb;
+    const int g1 = (int)min((long long)gpb, (long long)g0 + (gend - gcur));
+    const int bg = b * Hkv + gk;
+    const RbqQConst* qc = qconst + bg;
+    uint32_t bf[4][2];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int tl = base + g + 8 * r;
-      if (tl < cnt && head_ok) {
-        const int tok = t0 + tl;
+    for (int s = 0; s < 4; ++s) {
+      const uint2 v = *reinterpret_cast<const uint2*>(&qc->bfrag[s][lane][0]);
+      bf[s][0] = v.x; bf[s][1] = v.y;
+    }
+    const float cA = qc->cA[hsel], cB = qc->cB[hsel], cD = qc->cD[hsel];
+    const int init_d = qc->init_d[hsel], init_p = qc->init_p;
+    const size_t row = ((size_t)b * Hq + gk * G + hsel) * Lcap;
+    const size_t prow = (size_t)bg * Lcap;
+
+    float smax = -INFINITY;                                     // running max of this lane's head over the segment
+    GroupLoad cur = load_group(codes, f_scale, prow + (size_t)g0 * 32, g, t, Lcap - g0 * 32);
+    for (int gi = g0; gi < g1; ++gi) {
+      GroupLoad nxt = cur;
+      if (gi + 1 < g1) nxt = load_group(codes, f_scale, prow + (size_t)(gi + 1) * 32, g, t, Lcap - (gi + 1) * 32);
+      // tile 0: rows g / g+8 = tokens 4g / 4g+1 ; tile 1: tokens 4g+2 / 4g+3
+      int c0[4] = {init_d, init_p, init_d, init_p};
+      int c1[4] = {init_d, init_p, init_d, init_p};
+      tile_mma(c0, cur.w[0], cur.w[1], bf);
+      tile_mma(c1, cur.w[2], cur.w[3], bf);
+      const int acc_d[4] = {c0[0], c0[2], c1[0], c1[2]};
+      const int acc_p[4] = {c0[1], c0[3], c1[1], c1[3]};
+      const int tok = gi * 32 + 4 * g;                          // first of this lane's 4 tokens
+      if (head_ok && tok < n) {
         if (INT_OUT) {
-          dot_out[row + tok] = (acc_d[r] - init_d) >> 3;
-          if (t == 0) pop_out[prow + tok] = (acc_p[r] - init_p) >> 3;
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            if (tok + r < n) {
+              dot_out[row + tok + r] = (acc_d[r] - init_d) >> 3;
+              if (t == 0) pop_out[prow + tok + r] = (acc_p[r] - init_p) >> 3;
+            }
+          }
         } else {
-          const float fd = __fsub_rn(__int_as_float(acc_d[r]), 12582912.0f);
-          const float fp = __fsub_rn(__int_as_float(acc_p[r]), 12582912.0f);
-          const float ip = fmaf(cA, fd, __fmul_rn(cB, fp));
-          float sc = fmaf(s_fs[tl], ip, cD);
-          if (HAS_BIAS) sc = fmaf(sm_scale, f_bias[row + tok], sc);
-          scores[row + tok] = sc;
+          const float fsv[4] = {cur.fs.x, cur.fs.y, cur.fs.z, cur.fs.w};
+          float sc[4];
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float fd = __fsub_rn(__int_as_float(acc_d[r]), 12582912.0f);
+            const float fp = __fsub_rn(__int_as_float(acc_p[r]), 12582912.0f);
+            const float ip = fmaf(cA, fd, __fmul_rn(cB, fp));
+            sc[r] = fmaf(fsv[r], ip, cD);
+          }
+          if (HAS_BIAS) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) if (tok + r < n) sc[r] = fmaf(sm_scale, f_bias[row + tok + r], sc[r]);
+          }
+          if (tok + 3 < n) {
+            *reinterpret_cast<float4*>(scores + row + tok) = make_float4(sc[0], sc[1], sc[2], sc[3]);
+            smax = fmaxf(fmaxf(smax, fmaxf(sc[0], sc[1])), fmaxf(sc[2], sc[3]));
+          } else {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) if (tok + r < n) { scores[row + tok + r] = sc[r]; smax = fmaxf(smax, sc[r]); }
+          }
         }
       }
+      cur = nxt;
     }
+    if (!INT_OUT) {                                             // row maximum for S6 (keys pre-zeroed by S3)
+      smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 4));
+      smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 8));
+      smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 16));
+      if (g == 0 && head_ok && smax > -INFINITY)
+        atomicMax(&rowmax_key[(size_t)b * Hq + gk * G + t], rbq_fkey(__fadd_rn(smax, 0.0f)));
+    }
+    gcur += g1 - g0;
   }
 }
 
-template <int TS, bool INT_OUT, bool HAS_BIAS>
+template <bool INT_OUT, bool HAS_BIAS>
 int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, cudaStream_t s) {
-  constexpr int SPAN = EST_STAGES * TS;
-  const size_t smem = (size_t)SPAN * 20 + EST_STAGES * 8;
-  auto kern = estimate_kernel<TS, INT_OUT, HAS_BIAS>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
-  dim3 grid((ctx->cfg.max_tokens + SPAN - 1) / SPAN, ctx->cfg.batch * ctx->cfg.n_kv_heads);
+  if (ctx->cfg.batch > EST_MAX_B) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch %d > %d", ctx->cfg.batch, EST_MAX_B);
+  // upper bound of the work: every sequence full; 4 CTAs (32 warps) per SM, fewer when there is little work
+  const long long max_groups = (long long)ctx->cfg.batch * ctx->cfg.n_kv_heads * ((ctx->cfg.max_tokens + 31) / 32);
+  long long ctas = (max_groups + 2 * EST_WARPS - 1) / (2 * EST_WARPS);          // >= 2 groups per warp
+  const long long cap = (long long)ctx->sm_count * 4;
+  if (ctas > cap) ctas = cap;
+  if (ctas < 1) ctas = 1;
   const RbqQConst* qc = reinterpret_cast<const RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
-  kern<<<grid, EST_THREADS, smem, s>>>(idx->codes, idx->f_scale, idx->f_bias, idx->n_indexed, qc, ctx->cfg.n_q_heads,
-                                       ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop);
+  estimate_kernel<INT_OUT, HAS_BIAS><<<(int)ctas, EST_THREADS, 0, s>>>(idx->codes, idx->f_scale, idx->f_bias, idx->n_indexed, qc,
+                                                                      ctx->cfg.batch, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
+                                                                      ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop,
+                                                                      reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
@@ -174,8 +194,7 @@ int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, in
 }  // namespace
 
 int rbq_launch_estimate(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, cudaStream_t s) {
-  constexpr int TS = 512;
-  if (dot) return launch_t<TS, true, false>(ctx, idx, scores, dot, pop, s);
-  if (idx->f_bias && idx->c_q) return launch_t<TS, false, true>(ctx, idx, scores, dot, pop, s);
-  return launch_t<TS, false, false>(ctx, idx, scores, dot, pop, s);
+  if (dot) return launch_t<true, false>(ctx, idx, scores, dot, pop, s);
+  if (idx->f_bias && idx->c_q) return launch_t<false, true>(ctx, idx, scores, dot, pop, s);
+  return launch_t<false, false>(ctx, idx, scores, dot, pop, s);
 }

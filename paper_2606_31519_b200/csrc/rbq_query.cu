@@ -14,7 +14,8 @@ template <typename TQ>
 __global__ void __launch_bounds__(RBQ_MAX_G * RBQ_D)
 query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const float* __restrict__ c_k,
              const float* __restrict__ rot, int rot_kind, int Hq, int Hkv, float sm_scale,
-             uint8_t* __restrict__ qu_out, float* __restrict__ qparams, RbqQConst* __restrict__ qc_out) {
+             uint8_t* __restrict__ qu_out, float* __restrict__ qparams, RbqQConst* __restrict__ qc_out,
+             uint32_t* __restrict__ rowmax_key) {
   const int G = Hq / Hkv;
   const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv;
   const int hs = threadIdx.x >> 7, j = threadIdx.x & 127;      // head slice, dim
@@ -141,6 +142,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   __syncthreads();
   const int sumq = s_isum[hs][0] + s_isum[hs][1] + s_isum[hs][2] + s_isum[hs][3];
 
+  if (hs < G && j == 0) rowmax_key[row] = 0u;                  // S5 accumulates the row maximum with atomicMax
   if (hs < G) {
     if (qu_out) qu_out[row * RBQ_D + j] = (uint8_t)v;
     if (j == 0) {
@@ -181,6 +183,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
 int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, cudaStream_t s) {
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   RbqQConst* qc = reinterpret_cast<RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
+  uint32_t* rk = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax);
   const int threads = max(256, ctx->G * RBQ_D);
   const size_t smem = ctx->cfg.rot_kind == RBQ_ROT_DENSE ? (size_t)RBQ_D * RBQ_D * sizeof(float) : 0;
   static bool attr_set = false;
@@ -191,10 +194,10 @@ int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t*
   }
   if (ctx->cfg.q_dtype == RBQ_BF16)
     query_kernel<<<BG, threads, smem, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk);
   else
     query_kernel<<<BG, threads, smem, s>>>((const float*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc);
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

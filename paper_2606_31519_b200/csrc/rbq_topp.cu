@@ -6,17 +6,18 @@
 // row 10-25 times with one CTA per row.  Here one THREAD-BLOCK CLUSTER of CS CTAs owns a row: every
 // CTA keeps its slice of the row resident in shared memory, so the row is read from L2/HBM exactly
 // once.  The selection is an exact cut in the total order (score descending, index ascending), i.e.
-// on the composite key  C(t) = (orderkey(score_t) << 32) | ~t  whose values are all distinct:
-//   level 0 : 2048 bins of width 1/64 in u = max - score (monotone in C).  Per bin a packed
-//             (count, sum of r) pair, r = exp(-(u - j/64)) in 2^-28 fixed point, so that the bin
-//             mass is exp(-j/64) * sum(r): integer sums => order-independent and deterministic.
-//             Histograms are combined across the cluster through distributed shared memory; a block
-//             scan (fp64) finds the bin where the cumulative mass crosses T = p * Z.
-//   candidates (tokens of the crossing bin, a few hundred at 128 K context) are gathered from all CTAs
-//             and ranked exactly with integer prefix masses; the cut C* is the first candidate whose
-//             inclusive prefix reaches the remaining mass.  If the crossing bin holds more than
-//             TP_CAND tokens (heavy ties), it is first narrowed by 11-bit radix levels on C itself.
-//   output  : token t is selected  <=>  C(t) >= C*.  Written as a per-row BITMAP (the representation
+// on the composite key  C(t) = (orderkey(score_t) << 32) | ~t  whose values are all distinct.
+// The row maximum m comes with the scores (S5 epilogue, or rowmax_kernel for caller-provided scores):
+//   pass 1  : while the slice is loaded, 2048 bins of width 1/64 in u = m - score (monotone in C).
+//             Per bin a (count, sum of r) pair, r = 2^(-(u - j/64) log2 e) in 2^-28 fixed point, so the
+//             bin mass is exp(-j/64) * sum(r): integer sums => order-independent and deterministic.
+//             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin
+//             travel through distributed shared memory (DSMEM is ~20 B/clk per SM).
+//   pass 2  : the tokens of the crossing bin (a few hundred at 128 K context) are gathered from all
+//             CTAs and cut exactly with integer prefix masses: local 11-bit radix levels on C until
+//             <= 64 remain, then exact ranking.  If the crossing bin holds more than TP_CAND tokens
+//             (heavy ties), it is first narrowed by cluster-wide radix levels on C.
+//   pass 3  : token t is selected  <=>  C(t) >= C*.  Written as a per-row BITMAP (the representation
 //             the gather attention consumes), the count, and -- only when the caller asks for it --
 //             the ascending index list.
 #include <cooperative_groups.h>
@@ -30,24 +31,27 @@ namespace {
 constexpr int TP_THREADS = 512;
 constexpr int TP_WARPS = TP_THREADS / 32;
 constexpr int TP_NB = 4 * TP_THREADS;          // 2048 bins, 4 per thread in the scans
-constexpr int TP_CAND = 1024;                  // candidates ranked exactly
+constexpr int TP_NC = 64;                      // coarse bins (32 fine bins each)
+constexpr int TP_CAND = 1024;                  // candidates gathered per row
+constexpr int TP_RANK = 64;                    // candidates ranked by direct comparison
 constexpr unsigned FULL = 0xffffffffu;
 typedef unsigned long long u64;
 
 struct TpSmall {
-  double wt_d[TP_WARPS];
   u64 wt_u[TP_WARPS];
   uint32_t wt_c[TP_WARPS];
-  float red_f[TP_WARPS];
   u64 red_lo[TP_WARPS], red_hi[TP_WARPS];
+  double tabA[TP_NC], tabB[32];                // exp(-k/2), exp(-i/64)
+  double tot_mass[TP_NC];
+  uint32_t tot_cnt[TP_NC];
   // results broadcast inside the CTA
   double trem;            // mass still needed inside the candidate range, in units of 2^-28 * exp(-bx/64)
-  u64 rx;                 // total r of the candidate range
-  u64 lo64, hi64;         // candidate range on C (refinement only)
+  u64 lo64, hi64;         // candidate range on C
   u64 cstar;
-  uint32_t bx, cntx, cnt_above, found;
+  uint32_t bx, cntx, cnt_above, found, kx, nlist;
   // read by cluster peers
-  float x_max;
+  double xc_mass[TP_NC];
+  uint32_t xc_cnt[TP_NC];
   u64 x_lo, x_hi;
   uint32_t x_tot;
   uint32_t lcount;
@@ -58,14 +62,17 @@ constexpr size_t TP_OFF_A = TP_OFF_HIST + TP_NB * sizeof(uint2);                
 constexpr size_t TP_A_HALF = TP_CAND * 12;                                       // comp u64 + rfix u32
 constexpr size_t TP_OFF_SC = TP_OFF_A + 2 * TP_A_HALF;
 
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^28
 __device__ __forceinline__ void bin0(float m, float s, int& j, uint32_t& rfix) {
   const float u = __fsub_rn(m, s);
   j = min(TP_NB - 1, __float2int_rz(__fmul_rn(u, 64.0f)));
   const float frac = __fsub_rn(u, __fmul_rn((float)j, 0.015625f));
-  rfix = __float2uint_rn(__fmul_rn(expf(-frac), 268435456.0f));
-}
-__device__ __forceinline__ int bin0_only(float m, float s) {
-  return min(TP_NB - 1, __float2int_rz(__fmul_rn(__fsub_rn(m, s), 64.0f)));
+  rfix = __float2uint_rn(__fmul_rn(ex2_approx(__fmul_rn(frac, -1.4426950408889634f)), 268435456.0f));
 }
 __device__ __forceinline__ u64 composite(float s, int t) {
   return ((u64)rbq_fkey(s) << 32) | (u64)(~(uint32_t)t);
@@ -77,8 +84,12 @@ __device__ __forceinline__ void hist_add(uint2* hist, int j, u64 v, uint32_t c) 
   const uint32_t carry = (old + lo < old) ? 1u : 0u;
   atomicAdd(&hist[j].y, (c << 12) + (uint32_t)(v >> 32) + carry);
 }
+__device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
+  cnt = v.y >> 12;
+  R = ((u64)(v.y & 0xFFFu) << 32) | v.x;
+}
 
-// totals of this thread's 4 bins over the CS histograms of the cluster
+// totals of this thread's 4 bins over the CS histograms of the cluster (cluster-wide radix levels only)
 template <int CS>
 __device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint2* hist, int tid, uint32_t (&cnt)[4], u64 (&R)[4]) {
 #pragma unroll
@@ -87,23 +98,74 @@ __device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint2* h
   for (int r = 0; r < CS; ++r) {
     const uint4* rh = reinterpret_cast<const uint4*>(CS == 1 ? hist : cluster.map_shared_rank(hist, r)) + tid * 2;
     const uint4 a = rh[0], b = rh[1];
-    cnt[0] += a.y >> 12; R[0] += ((u64)(a.y & 0xFFFu) << 32) | a.x;
-    cnt[1] += a.w >> 12; R[1] += ((u64)(a.w & 0xFFFu) << 32) | a.z;
-    cnt[2] += b.y >> 12; R[2] += ((u64)(b.y & 0xFFFu) << 32) | b.x;
-    cnt[3] += b.w >> 12; R[3] += ((u64)(b.w & 0xFFFu) << 32) | b.z;
+    uint32_t c; u64 v;
+    unpack_bin(make_uint2(a.x, a.y), c, v); cnt[0] += c; R[0] += v;
+    unpack_bin(make_uint2(a.z, a.w), c, v); cnt[1] += c; R[1] += v;
+    unpack_bin(make_uint2(b.x, b.y), c, v); cnt[2] += c; R[2] += v;
+    unpack_bin(make_uint2(b.z, b.w), c, v); cnt[3] += c; R[3] += v;
   }
+}
+
+// Integer block scan over TP_NB bins (4 per thread, ascending bin = descending C): finds the bin where the inclusive
+// prefix of R first reaches sh.trem (clamped to the total), and updates sh.{trem, cnt_above, cntx, lo64, hi64}.
+// `lo64`, `hi64`, `shift` describe the binning  bin = TP_NB-1 - ((C - lo64) >> shift).  Ends with a block barrier.
+__device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4], const u64 (&R)[4], u64 lo64, u64 hi64, int shift) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const u64 tsum = R[0] + R[1] + R[2] + R[3];
+  const uint32_t csum = cnt[0] + cnt[1] + cnt[2] + cnt[3];
+  u64 si = tsum;
+  uint32_t ci = csum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const u64 v = __shfl_up_sync(FULL, si, o);
+    const uint32_t c = __shfl_up_sync(FULL, ci, o);
+    if (lane >= o) { si += v; ci += c; }
+  }
+  const double trem_in = sh.trem;                               // read before the barrier: the claiming thread rewrites it
+  if (lane == 31) { sh.wt_u[warp] = si; sh.wt_c[warp] = ci; }
+  __syncthreads();
+  u64 wp = 0, tot = 0;
+  uint32_t wc = 0;
+  for (int w = 0; w < TP_WARPS; ++w) { if (w < warp) { wp += sh.wt_u[w]; wc += sh.wt_c[w]; } tot += sh.wt_u[w]; }
+  const double trem = fmin(trem_in, (double)tot);
+  const u64 excl = wp + si - tsum, incl = wp + si;
+  // exact integers: exactly one thread claims.  tot == 0 (every candidate weight underflows): first non-empty bin.
+  const bool claim = tot > 0 ? ((double)excl < trem && (double)incl >= trem) : (wc + ci - csum == 0 && csum > 0);
+  if (claim) {
+    u64 c = excl;
+    uint32_t cc = wc + ci - csum;
+    int kx = -1;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (kx < 0) {
+        if (tot > 0 ? ((double)(c + R[k]) >= trem) : (cnt[k] > 0)) kx = k;
+        else { c += R[k]; cc += cnt[k]; }
+      }
+    }
+    if (kx < 0) kx = 3;
+    const int bsel = 4 * tid + kx;
+    const u64 nmin = lo64 + ((u64)(TP_NB - 1 - bsel) << shift);
+    const u64 nmax = nmin + (((u64)1 << shift) - 1ull);
+    sh.lo64 = max(nmin, lo64);
+    sh.hi64 = min(nmax, hi64);
+    sh.cntx = cnt[kx];
+    sh.cnt_above += cc;
+    sh.trem = fmin(trem - (double)c, (double)R[kx]);
+  }
+  __syncthreads();
 }
 
 // grid = (CS, rows); cluster = CS CTAs along x.
 // smem: TpSmall | hist uint2[TP_NB] (later: selection words) | cand_all | cand_loc | scores slice [s_cap]
 template <int CS>
 __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
-topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_indexed, int Hq, int Lcap, int wpr, float p_f,
-            uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx, int32_t* __restrict__ sel_cnt) {
+topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
+            int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
+            int32_t* __restrict__ sel_cnt) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
   uint2* hist = reinterpret_cast<uint2*>(smem_raw + TP_OFF_HIST);
-  uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);          // aliases hist after the candidate sync
+  uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);          // aliases hist once the cut is known
   u64* all_comp = reinterpret_cast<u64*>(smem_raw + TP_OFF_A);
   uint32_t* all_rfix = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A + TP_CAND * 8);
   uint32_t* woff = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A);             // aliases cand_all after the cut is known
@@ -137,144 +199,146 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
   }
   auto csync = [&]() { if (CS == 1) __syncthreads(); else cluster.sync(); };
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
+  const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
 
-  // ---- load the slice (read once), zero the histogram, row maximum -----------------------------------
+  // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
   for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
-  float lmax = -INFINITY;
-  {
-    const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
-    const int n4 = len >> 2;
-    for (int i = tid; i < n4; i += TP_THREADS) {
-      float4 v = src[i];
-      v.x = __fadd_rn(v.x, 0.0f); v.y = __fadd_rn(v.y, 0.0f); v.z = __fadd_rn(v.z, 0.0f); v.w = __fadd_rn(v.w, 0.0f);   // -0 -> +0
-      reinterpret_cast<float4*>(sc)[i] = v;
-      lmax = fmaxf(fmaxf(lmax, fmaxf(v.x, v.y)), fmaxf(v.z, v.w));
-    }
-    for (int i = (n4 << 2) + tid; i < len; i += TP_THREADS) {
-      const float v = __fadd_rn(scores[rbase + lo + i], 0.0f);
-      sc[i] = v;
-      lmax = fmaxf(lmax, v);
-    }
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(FULL, lmax, o));
-  if (lane == 0) sh.red_f[warp] = lmax;
+  if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
+  else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
+  if (tid == 0) { sh.lcount = 0; sh.found = 0; sh.nlist = 0; }
   __syncthreads();
-  if (tid == 0) {
-    float r = sh.red_f[0];
-    for (int w = 1; w < TP_WARPS; ++w) r = fmaxf(r, sh.red_f[w]);
-    sh.x_max = r;
-  }
-  csync();                                                    // S1: x_max of every CTA visible (and hist zeroed)
-  float m = -INFINITY;
-#pragma unroll
-  for (int r = 0; r < CS; ++r) m = fmaxf(m, peer(r)->x_max);
-
-  // ---- level 0: (count, mass) histogram over u = m - s -------------------------------------------------
   {
     uint32_t of_c = 0;                                        // overflow bin kept in registers (can be half the row)
     u64 of_r = 0;
-    for (int base = warp * 32; base < len; base += TP_THREADS) {
-      const int i = base + lane;
-      int j = -1;
-      uint32_t rfix = 0;
-      if (i < len) bin0(m, sc[i], j, rfix);
-      const int j0 = __shfl_sync(FULL, j, 0);
-      if (__all_sync(FULL, j == j0)) {                        // whole warp in one bin (ties): one update
-        u64 v = rfix;
+    const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
+    const int n4 = (len + 3) >> 2;                            // whole float4 groups (Lcap % 4 == 0: in bounds)
+    for (int base = warp * 32; base < n4; base += TP_THREADS) {
+      const int i4 = base + lane;
+      float v[4] = {0.f, 0.f, 0.f, 0.f};
+      if (i4 < n4) {
+        const float4 t4 = __ldcs(src + i4);
+        v[0] = __fadd_rn(t4.x, 0.0f); v[1] = __fadd_rn(t4.y, 0.0f); v[2] = __fadd_rn(t4.z, 0.0f); v[3] = __fadd_rn(t4.w, 0.0f);   // -0 -> +0
+        reinterpret_cast<float4*>(sc)[i4] = make_float4(v[0], v[1], v[2], v[3]);
+      }
+      int j[4];
+      uint32_t rf[4];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+      for (int k = 0; k < 4; ++k) {
+        j[k] = -1; rf[k] = 0;
+        if (4 * i4 + k < len) bin0(m, v[k], j[k], rf[k]);
+      }
+      const int j0 = __shfl_sync(FULL, j[0], 0);
+      if (__all_sync(FULL, j[0] == j0 && j[1] == j0 && j[2] == j0 && j[3] == j0)) {   // 128 tokens in one bin (ties)
+        u64 t = (u64)rf[0] + rf[1] + rf[2] + rf[3];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
         if (lane == 0) {
-          if (j0 == TP_NB - 1) { of_c += 32; of_r += v; } else hist_add(hist, j0, v, 32u);
+          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add(hist, j0, t, 128u);
         }
-      } else if (j >= 0) {
-        if (j == TP_NB - 1) { of_c += 1; of_r += rfix; } else hist_add(hist, j, (u64)rfix, 1u);
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (j[k] == TP_NB - 1) { of_c += 1; of_r += rf[k]; }
+          else if (j[k] >= 0) hist_add(hist, j[k], (u64)rf[k], 1u);
+        }
       }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { of_c += __shfl_xor_sync(FULL, of_c, o); of_r += __shfl_xor_sync(FULL, of_r, o); }
     if (lane == 0 && of_c) hist_add(hist, TP_NB - 1, of_r, of_c);
   }
-  csync();                                                    // S2: histograms complete
-
-  uint32_t cnt[4];
-  u64 R[4];
-  gather_bins<CS>(cluster, hist, tid, cnt, R);
+  __syncthreads();
+  // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins 4t..4t+3, 8 threads per coarse bin
   {
-    double ms[4], tsum = 0.0;
-    uint32_t csum = 0;
+    double ms = 0.0;
+    uint32_t cs = 0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      ms[k] = (double)R[k] * exp(-(double)(4 * tid + k) * 0.015625);
-      tsum += ms[k];
-      csum += cnt[k];
+      uint32_t c; u64 R;
+      unpack_bin(hist[4 * tid + k], c, R);
+      ms += (double)R * sh.tabB[(4 * tid + k) & 31];
+      cs += c;
     }
-    double si = tsum;
-    uint32_t ci = csum;
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) { ms += __shfl_xor_sync(FULL, ms, o); cs += __shfl_xor_sync(FULL, cs, o); }
+    if ((tid & 7) == 0) { sh.xc_mass[tid >> 3] = ms * sh.tabA[tid >> 3]; sh.xc_cnt[tid >> 3] = cs; }
+  }
+  csync();                                                    // S1: histograms and coarse summaries complete
+  if (tid < TP_NC) {
+    double a = 0.0;
+    uint32_t c = 0;
+#pragma unroll
+    for (int r = 0; r < CS; ++r) { const TpSmall* ps = peer(r); a += ps->xc_mass[tid]; c += ps->xc_cnt[tid]; }
+    sh.tot_mass[tid] = a; sh.tot_cnt[tid] = c;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    // coarse crossing (lane 0, serial over 64 bins), then the 32 fine bins of that coarse bin (one per lane)
+    double T = 0.0, above = 0.0;
+    uint32_t cab = 0;
+    int kx = 0;
+    if (lane == 0) {
+      double Z = 0.0;
+      for (int k = 0; k < TP_NC; ++k) Z += sh.tot_mass[k];
+      T = (double)p_f * Z;
+      double cum = 0.0;
+      int last = 0;
+      kx = -1;
+      for (int k = 0; k < TP_NC; ++k) {
+        if (sh.tot_cnt[k] == 0) continue;
+        last = k;
+        if (cum + sh.tot_mass[k] >= T) { kx = k; break; }
+        cum += sh.tot_mass[k]; cab += sh.tot_cnt[k];
+      }
+      if (kx < 0) { kx = last; cum -= sh.tot_mass[last]; cab -= sh.tot_cnt[last]; }
+      above = cum;
+    }
+    kx = __shfl_sync(FULL, kx, 0); T = __shfl_sync(FULL, T, 0); above = __shfl_sync(FULL, above, 0); cab = __shfl_sync(FULL, cab, 0);
+    uint32_t c = 0;
+    u64 R = 0;
+#pragma unroll
+    for (int r = 0; r < CS; ++r) {
+      const uint2* rh = CS == 1 ? hist : cluster.map_shared_rank(hist, r);
+      uint32_t cc; u64 rr;
+      unpack_bin(rh[32 * kx + lane], cc, rr);
+      c += cc; R += rr;
+    }
+    const double e = sh.tabA[kx] * sh.tabB[lane];
+    const double ms = (double)R * e;
+    double si = ms;
+    uint32_t ci = c;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const double v = __shfl_up_sync(FULL, si, o);
-      const uint32_t c = __shfl_up_sync(FULL, ci, o);
-      if (lane >= o) { si += v; ci += c; }
+      const uint32_t cv = __shfl_up_sync(FULL, ci, o);
+      if (lane >= o) { si += v; ci += cv; }
     }
-    if (lane == 31) { sh.wt_d[warp] = si; sh.wt_c[warp] = ci; }
-    if (tid == 0) { sh.bx = 0xFFFFFFFFu; sh.found = 0; sh.lcount = 0; }
-    __syncthreads();
-    double wp = 0.0, Z = 0.0;
-    uint32_t wc = 0;
-    for (int w = 0; w < TP_WARPS; ++w) {
-      if (w == warp) { wp = Z; }
-      Z += sh.wt_d[w];
-      if (w < warp) wc += sh.wt_c[w];
+    const bool cross = c > 0 && above + si >= T;
+    unsigned bal = __ballot_sync(FULL, cross);
+    const unsigned nonempty = __ballot_sync(FULL, c > 0);
+    if (bal == 0u) bal = nonempty ? (1u << (31 - __clz(nonempty))) : 1u;      // rounding at the last ulp: last non-empty bin
+    const int lx = __ffs(bal) - 1;
+    if (lane == lx) {
+      const double ab = above + (si - ms);
+      sh.bx = (uint32_t)(32 * kx + lane);
+      sh.cntx = c;
+      sh.cnt_above = cab + (ci - c);
+      sh.trem = fmin(fmax((T - ab) / e, 0.5), (double)R);
     }
-    const double T = (double)p_f * Z;
-    double se = __shfl_up_sync(FULL, si, 1);
-    uint32_t ce = __shfl_up_sync(FULL, ci, 1);
-    if (lane == 0) { se = 0.0; ce = 0; }
-    const double excl = wp + se, incl = wp + si;              // excl of thread t+1 is bit-identical to incl of thread t
-    const bool claim = (excl < T) && (incl >= T);
-    if (claim) atomicMin(&sh.bx, (uint32_t)(4 * tid));
-    __syncthreads();
-    if (claim && sh.bx == (uint32_t)(4 * tid)) {
-      double c = excl;
-      uint32_t cc = wc + ce;
-      int kx = -1;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        if (kx < 0) {
-          if (cnt[k] > 0 && c + ms[k] >= T) kx = k;
-          else { c += ms[k]; cc += cnt[k]; }
-        }
-      }
-      if (kx < 0) {                                           // rounding: take the last non-empty bin of this thread
-        c = excl; cc = wc + ce;
-        int last = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) if (cnt[k] > 0) last = k;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) if (k < last) { c += ms[k]; cc += cnt[k]; }
-        kx = last;
-      }
-      const int bxx = 4 * tid + kx;
-      sh.bx = (uint32_t)bxx;
-      sh.cntx = cnt[kx];
-      sh.cnt_above = cc;
-      sh.rx = R[kx];
-      const double rem = (T - c) / exp(-(double)bxx * 0.015625);
-      sh.trem = fmin(fmax(rem, 0.5), (double)R[kx]);
-    }
-    __syncthreads();
   }
+  __syncthreads();
   const int bx = (int)sh.bx;
   uint32_t cntx = sh.cntx;
+  const float u_lo = (float)bx * 0.015625f, u_hi = (bx == TP_NB - 1) ? INFINITY : (float)(bx + 1) * 0.015625f;
   bool use_range = false;
 
-  // ---- heavy ties only: narrow the candidate range by 11-bit radix levels on C --------------------------
+  // ---- heavy ties only: narrow the candidate range by cluster-wide 11-bit radix levels on C --------------
   if (cntx > TP_CAND) {
     u64 mn = ~0ull, mx = 0ull;
     for (int i = tid; i < len; i += TP_THREADS) {
       const float s = sc[i];
-      if (bin0_only(m, s) == bx) { const u64 c = composite(s, lo + i); mn = min(mn, c); mx = max(mx, c); }
+      const float u = __fsub_rn(m, s);
+      if (u >= u_lo && u < u_hi) { const u64 c = composite(s, lo + i); mn = min(mn, c); mx = max(mx, c); }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { mn = min(mn, __shfl_xor_sync(FULL, mn, o)); mx = max(mx, __shfl_xor_sync(FULL, mx, o)); }
@@ -284,15 +348,14 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
       for (int w = 1; w < TP_WARPS; ++w) { mn = min(mn, sh.red_lo[w]); mx = max(mx, sh.red_hi[w]); }
       sh.x_lo = mn; sh.x_hi = mx;
     }
-    csync();                                                  // also: every CTA is done reading the level-0 histograms
+    csync();                                                  // also: every CTA is done reading the pass-1 histograms
     u64 lo64 = ~0ull, hi64 = 0ull;
 #pragma unroll
     for (int r = 0; r < CS; ++r) { lo64 = min(lo64, peer(r)->x_lo); hi64 = max(hi64, peer(r)->x_hi); }
     use_range = true;
     while (cntx > TP_CAND) {
       const u64 range = hi64 - lo64;
-      const int bits = 64 - __clzll((long long)range);
-      const int shift = max(0, bits - 11);
+      const int shift = max(0, (64 - __clzll((long long)range)) - 11);
       for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
       __syncthreads();
       for (int base = warp * 32; base < len; base += TP_THREADS) {
@@ -319,77 +382,39 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
         }
       }
       csync();
+      uint32_t cnt[4];
+      u64 R[4];
       gather_bins<CS>(cluster, hist, tid, cnt, R);
-      u64 tsum = R[0] + R[1] + R[2] + R[3];
-      uint32_t csum = cnt[0] + cnt[1] + cnt[2] + cnt[3];
-      u64 si = tsum;
-      uint32_t ci = csum;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const u64 v = __shfl_up_sync(FULL, si, o);
-        const uint32_t c = __shfl_up_sync(FULL, ci, o);
-        if (lane >= o) { si += v; ci += c; }
-      }
-      const double trem = sh.trem;                            // read before the barrier: the claiming thread rewrites it below
-      if (lane == 31) { sh.wt_u[warp] = si; sh.wt_c[warp] = ci; }
-      __syncthreads();
-      u64 wp = 0;
-      uint32_t wc = 0;
-      for (int w = 0; w < warp; ++w) { wp += sh.wt_u[w]; wc += sh.wt_c[w]; }
-      const u64 excl = wp + si - tsum, incl = wp + si;
-      if ((double)excl < trem && (double)incl >= trem) {       // exact integers: exactly one thread
-        u64 c = excl;
-        uint32_t cc = wc + ci - csum;
-        int kx = -1;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          if (kx < 0) {
-            if ((double)(c + R[k]) >= trem) kx = k;
-            else { c += R[k]; cc += cnt[k]; }
-          }
-        }
-        if (kx < 0) kx = 3;
-        const int bsel = 4 * tid + kx;
-        const u64 nmin = lo64 + ((u64)(TP_NB - 1 - bsel) << shift);
-        const u64 nmax = (shift >= 64) ? hi64 : nmin + (((u64)1 << shift) - 1ull);
-        sh.lo64 = max(nmin, lo64);
-        sh.hi64 = min(nmax, hi64);
-        sh.cntx = cnt[kx];
-        sh.cnt_above += cc;
-        sh.rx = R[kx];
-        sh.trem = fmin(trem - (double)c, (double)R[kx]);
-      }
-      csync();                                                // result visible; peers done reading this level's histogram
+      radix_scan(sh, cnt, R, lo64, hi64, shift);
+      csync();                                                // peers done reading this level's histogram
       lo64 = sh.lo64; hi64 = sh.hi64; cntx = sh.cntx;
       if (shift == 0) break;                                  // one C per bin: a single candidate is left
     }
   }
 
-  // ---- candidates of this CTA -> local list; gather all; exact ranking ------------------------------------
+  // ---- pass 2: candidates of this CTA -> local list; gather all ---------------------------------------------
   {
     u64 lo64 = 0, hi64 = 0;
     if (use_range) { lo64 = sh.lo64; hi64 = sh.hi64; }
     for (int i = tid; i < len; i += TP_THREADS) {
       const float s = sc[i];
-      bool is;
-      u64 c = composite(s, lo + i);
-      if (use_range) is = (c >= lo64 && c <= hi64);
-      else is = (bin0_only(m, s) == bx);
+      const float u = __fsub_rn(m, s);
+      bool is = (u >= u_lo && u < u_hi);
+      if (is && use_range) { const u64 c = composite(s, lo + i); is = (c >= lo64 && c <= hi64); }
       if (is) {
         int j_unused;
         uint32_t rfix;
         bin0(m, s, j_unused, rfix);
         const uint32_t slot = atomicAdd(&sh.lcount, 1u);
-        if (slot < TP_CAND) { loc_comp[slot] = c; loc_rfix[slot] = rfix; }
+        if (slot < TP_CAND) { loc_comp[slot] = composite(s, lo + i); loc_rfix[slot] = rfix; }
       }
     }
   }
-  csync();                                                    // S3: candidate lists complete; histograms free
+  csync();                                                    // S2: candidate lists complete; histograms free
   int ncand = 0;
 #pragma unroll
   for (int r = 0; r < CS; ++r) {
-    const TpSmall* ps = peer(r);
-    const int lc = min((int)ps->lcount, TP_CAND);
+    const int lc = min((int)peer(r)->lcount, TP_CAND);
     const u64* rc = CS == 1 ? loc_comp : cluster.map_shared_rank(loc_comp, r);
     const uint32_t* rr = CS == 1 ? loc_rfix : cluster.map_shared_rank(loc_rfix, r);
     for (int k = tid; k < lc; k += TP_THREADS) {
@@ -398,13 +423,65 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
     ncand = min(TP_CAND, ncand + lc);
   }
   __syncthreads();
+
+  // ---- exact cut among the candidates: local radix levels until <= TP_RANK remain, then direct ranking ------
   {
+    // each thread keeps up to 2 candidates in registers
+    u64 cc[2];
+    uint32_t cr[2];
+    bool cv[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int i = tid + k * TP_THREADS;
+      cv[k] = i < ncand;
+      cc[k] = cv[k] ? all_comp[i] : 0ull;
+      cr[k] = cv[k] ? all_rfix[i] : 0u;
+    }
+    int live = ncand;
+    while (live > TP_RANK) {
+      u64 mn = ~0ull, mx = 0ull;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) if (cv[k]) { mn = min(mn, cc[k]); mx = max(mx, cc[k]); }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { mn = min(mn, __shfl_xor_sync(FULL, mn, o)); mx = max(mx, __shfl_xor_sync(FULL, mx, o)); }
+      if (lane == 0) { sh.red_lo[warp] = mn; sh.red_hi[warp] = mx; }
+      for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
+      __syncthreads();
+      u64 lo64 = ~0ull, hi64 = 0ull;
+      for (int w = 0; w < TP_WARPS; ++w) { lo64 = min(lo64, sh.red_lo[w]); hi64 = max(hi64, sh.red_hi[w]); }
+      const int shift = max(0, (64 - __clzll((long long)(hi64 - lo64))) - 11);
+#pragma unroll
+      for (int k = 0; k < 2; ++k)
+        if (cv[k]) hist_add(hist, TP_NB - 1 - (int)((cc[k] - lo64) >> shift), (u64)cr[k], 1u);
+      __syncthreads();
+      uint32_t cnt[4];
+      u64 R[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) unpack_bin(hist[4 * tid + k], cnt[k], R[k]);
+      radix_scan(sh, cnt, R, lo64, hi64, shift);
+      const u64 nlo = sh.lo64, nhi = sh.hi64;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) cv[k] = cv[k] && cc[k] >= nlo && cc[k] <= nhi;
+      live = (int)sh.cntx;
+      __syncthreads();                                        // sh.* and hist reused by the next level
+      if (shift == 0) break;
+    }
+    // survivors -> compact list (aliases the gathered arrays: all threads hold their candidates in registers)
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      if (cv[k]) {
+        const uint32_t slot = atomicAdd(&sh.nlist, 1u);
+        if (slot < TP_CAND) { all_comp[slot] = cc[k]; all_rfix[slot] = cr[k]; }
+      }
+    }
+    __syncthreads();
+    const int nl = min((int)sh.nlist, TP_CAND);
     const double trem = sh.trem;
-    for (int i = tid; i < ncand; i += TP_THREADS) {
+    for (int i = tid; i < nl; i += TP_THREADS) {
       const u64 ci = all_comp[i];
       u64 P = 0;
       uint32_t rk = 0;
-      for (int j = 0; j < ncand; ++j) {
+      for (int j = 0; j < nl; ++j) {
         const bool ge = all_comp[j] >= ci;
         P += ge ? (u64)all_rfix[j] : 0ull;
         rk += ge ? 1u : 0u;
@@ -412,22 +489,27 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
       if ((double)P >= trem && (double)(P - all_rfix[i]) < trem) { sh.cstar = ci; sh.cnt_above += rk; sh.found = 1; }
     }
     __syncthreads();
-    if (!sh.found && tid == 0) {                              // rounding at the last ulp: take every candidate
+    if (!sh.found && tid == 0) {                              // rounding at the last ulp / zero weights: take every survivor
       u64 mn = ~0ull;
-      for (int j = 0; j < ncand; ++j) mn = min(mn, all_comp[j]);
-      sh.cstar = mn; sh.cnt_above += (uint32_t)ncand;
+      for (int j = 0; j < nl; ++j) mn = min(mn, all_comp[j]);
+      sh.cstar = mn; sh.cnt_above += (uint32_t)nl;
     }
     __syncthreads();
   }
   const u64 cstar = sh.cstar;
   const uint32_t total_sel = sh.cnt_above;
 
-  // ---- output: bitmap words (always), ascending index list (on request) -----------------------------------
-  for (int w = warp; w < nwords; w += TP_WARPS) {
-    const int i = w * 32 + lane;
-    const bool sel = (i < len) && composite(sc[i], lo + i) >= cstar;
-    const unsigned bal = __ballot_sync(FULL, sel);
-    if (lane == 0) { bits_row[(lo >> 5) + w] = bal; selw[w] = bal; }
+  // ---- pass 3: bitmap words (always), ascending index list (on request) ---------------------------------------
+  {
+    const float sstar = rbq_fkey_inv((uint32_t)(cstar >> 32));
+    const int tstar = (int)(~(uint32_t)cstar);                // equal scores: indices <= tstar are selected
+    for (int w = warp; w < nwords; w += TP_WARPS) {
+      const int i = w * 32 + lane;
+      bool sel = false;
+      if (i < len) { const float s = sc[i]; sel = (s > sstar) || (s == sstar && lo + i <= tstar); }
+      const unsigned bal = __ballot_sync(FULL, sel);
+      if (lane == 0) { bits_row[(lo >> 5) + w] = bal; selw[w] = bal; }
+    }
   }
   if (rank == 0 && tid == 0) sel_cnt[row] = (int32_t)total_sel;
   if (sel_idx) {
@@ -458,7 +540,7 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
       run += pc[k];
     }
     if (tid == 0) sh.x_tot = tot;
-    csync();                                                  // S4: per-CTA totals visible
+    csync();                                                  // per-CTA totals visible
     uint32_t obase = 0;
 #pragma unroll
     for (int r = 0; r < CS; ++r) if (r < rank) obase += peer(r)->x_tot;
@@ -471,9 +553,20 @@ topp_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_inde
   csync();                                                    // keep shared memory alive until every peer has read it
 }
 
+// order-preserving key of the row maximum, for caller-provided scores (rbq_topp_select); rowmax_key pre-zeroed
+__global__ void rowmax_kernel(const float* __restrict__ scores, const int32_t* __restrict__ n_indexed, int Hq, int Lcap,
+                              uint32_t* __restrict__ rowmax_key) {
+  const int row = blockIdx.y, n = n_indexed[row / Hq];
+  float mx = -INFINITY;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) mx = fmaxf(mx, scores[(size_t)row * Lcap + i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, o));
+  if ((threadIdx.x & 31) == 0 && mx > -INFINITY) atomicMax(&rowmax_key[row], rbq_fkey(__fadd_rn(mx, 0.0f)));
+}
+
 template <int CS>
-int launch_cs(rbq_ctx* ctx, const float* scores, const int32_t* n_indexed, float p, uint32_t* bits, int wpr, int32_t* sel_idx,
-              int32_t* sel_cnt, cudaStream_t s) {
+int launch_cs(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p, uint32_t* bits,
+              int wpr, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
   const int s_cap = ((((ctx->cfg.max_tokens + CS - 1) / CS) + 31) & ~31) + 32;
   const size_t smem = TP_OFF_SC + (size_t)s_cap * 4;
@@ -484,7 +577,8 @@ int launch_cs(rbq_ctx* ctx, const float* scores, const int32_t* n_indexed, float
     attr_smem = smem;
   }
   dim3 grid(CS, rows);
-  kern<<<grid, TP_THREADS, smem, s>>>(scores, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, wpr, p, bits, sel_idx, sel_cnt);
+  kern<<<grid, TP_THREADS, smem, s>>>(scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, wpr, p, bits, sel_idx,
+                                      sel_cnt);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
@@ -500,17 +594,27 @@ int rbq_topp_cluster_size(const rbq_ctx* ctx) {
   return cs;
 }
 
-int rbq_launch_topp(rbq_ctx* ctx, const float* scores, const int32_t* n_indexed, float p, uint32_t* sel_bits, int32_t* sel_idx,
-                    int32_t* sel_cnt, cudaStream_t s) {
+// rowmax_key == NULL: the maxima are computed here (rbq_topp_select on caller-provided scores).
+int rbq_launch_topp(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p,
+                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int cs = rbq_topp_cluster_size(ctx);
   const int wpr = rbq_words_per_row(ctx);
+  const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
   const int s_cap = ((((ctx->cfg.max_tokens + cs - 1) / cs) + 31) & ~31) + 32;
   if (TP_OFF_SC + (size_t)s_cap * 4 > 227 * 1024 || s_cap > 32 * TP_NB)
     RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "rbq_topp_select: max_tokens %d exceeds the cluster-resident limit", ctx->cfg.max_tokens);
+  if (!rowmax_key) {
+    uint32_t* rk = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax);
+    RBQ_CUDA_OK(ctx, cudaMemsetAsync(rk, 0, (size_t)rows * sizeof(uint32_t), s));
+    dim3 grid(max(1, min(32, (ctx->cfg.max_tokens + 4095) / 4096)), rows);
+    rowmax_kernel<<<grid, 256, 0, s>>>(scores, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, rk);
+    RBQ_LAUNCH_OK(ctx);
+    rowmax_key = rk;
+  }
   switch (cs) {
-    case 8: return launch_cs<8>(ctx, scores, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
-    case 4: return launch_cs<4>(ctx, scores, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
-    case 2: return launch_cs<2>(ctx, scores, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
-    default: return launch_cs<1>(ctx, scores, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    case 8: return launch_cs<8>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    case 4: return launch_cs<4>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    case 2: return launch_cs<2>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    default: return launch_cs<1>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
   }
 }
