@@ -286,8 +286,6 @@ def run_b200(args):
     # ---- device-timed region: W warm-ups, then exactly K steps ---------------------------------------------
     for i in range(args.warmup):
         step(i)
-    for c in caches:
-        c.profile_enable(True)
     launches0 = sum(c.launch_count() for c in caches)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -302,6 +300,13 @@ def run_b200(args):
     rdist.barrier()
     ms_total = e0.elapsed_time(e1)
     gpu_launches = sum(c.launch_count() for c in caches) - launches0
+    # per-stage breakdown: a second, separate pass with the library's stage events between the kernels (the events
+    # serialise the launches, so the stage times add up to a little more than the step timed above)
+    for c in caches:
+        c.profile_enable(True)
+    for i in range(min(args.steps, 256)):
+        step(args.warmup + i)
+    torch.cuda.synchronize()
     stage_ms = {k: 0.0 for k in rb.STAGE_NAMES}
     n_prof = 0
     for c in caches:

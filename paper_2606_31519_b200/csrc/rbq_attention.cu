@@ -48,12 +48,14 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
   __shared__ uint32_t s_warp[PL_THREADS / 32];
   __shared__ uint32_t s_pre[PL_THREADS], s_cntb[PL_THREADS];
   __shared__ uint32_t s_base;
+  rbq_pdl_trigger();
+  rbq_pdl_wait();                                             // selection bitmaps of S6
   const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nidx = max(0, n_indexed[b]);
   const int nw = (nidx + 31) >> 5, nblk = (nw + 3) >> 2;
   const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
-  uint32_t* out = ulist + (size_t)gi * Lcap;
+  uint32_t* __restrict__ out = ulist + (size_t)gi * Lcap;
   if (tid == 0) s_base = 0;
   __syncthreads();
   for (int blk0 = 0; blk0 < nblk; blk0 += PL_THREADS) {
@@ -81,27 +83,34 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
     s_pre[tid] = s_base + wp + si - c;
     s_cntb[tid] = c;
     __syncthreads();
+    // this warp's blocks: lb = blockIdx.x + PL_SPLIT * (warp + 32 i), i < 4.  Lane l < 16 prefetches word (l & 3) of head
+    // (l >> 2) of each block first (one round of independent loads), then the words are broadcast by shuffles.
     const unsigned lt = (1u << lane) - 1u;
-    for (int lb = (int)blockIdx.x + PL_SPLIT * warp; lb < PL_THREADS; lb += PL_SPLIT * (PL_THREADS / 32)) {
+    constexpr int PL_BPW = PL_THREADS / (PL_SPLIT * (PL_THREADS / 32));          // blocks per warp and iteration (4)
+    uint32_t pre[PL_BPW];
+#pragma unroll
+    for (int i = 0; i < PL_BPW; ++i) {
+      const int lb = (int)blockIdx.x + PL_SPLIT * (warp + (PL_THREADS / 32) * i);
+      const int wi = 4 * (blk0 + lb) + (lane & 3), h = lane >> 2;
+      pre[i] = (lane < 16 && h < G && blk0 + lb < nblk && wi < nw && s_cntb[lb] != 0) ? rows0[(size_t)h * wpr + wi] : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < PL_BPW; ++i) {
+      const int lb = (int)blockIdx.x + PL_SPLIT * (warp + (PL_THREADS / 32) * i);
       const int bk = blk0 + lb;
-      if (bk >= nblk || s_cntb[lb] == 0) continue;
+      if (bk >= nblk || s_cntb[lb] == 0) continue;              // warp-uniform
       uint32_t pos = s_pre[lb];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const int wi = 4 * bk + k;
-        if (wi < nw) {
-          uint32_t u = 0, mask = 0;
+        uint32_t u = 0, mask = 0;
 #pragma unroll
-          for (int h = 0; h < RBQ_MAX_G; ++h) {
-            if (h < G) {
-              const uint32_t hwv = rows0[(size_t)h * wpr + wi];
-              u |= hwv;
-              mask |= ((hwv >> lane) & 1u) << h;
-            }
-          }
-          if ((u >> lane) & 1u) out[pos + __popc(u & lt)] = (uint32_t)(wi * 32 + lane) | (mask << 28);
-          pos += __popc(u);
+        for (int h = 0; h < RBQ_MAX_G; ++h) {
+          const uint32_t hwv = __shfl_sync(0xffffffffu, pre[i], 4 * h + k);
+          u |= hwv;
+          mask |= ((hwv >> lane) & 1u) << h;
         }
+        if ((u >> lane) & 1u) out[pos + __popc(u & lt)] = (uint32_t)((4 * bk + k) * 32 + lane) | (mask << 28);
+        pos += __popc(u);
       }
     }
     __syncthreads();
@@ -199,6 +208,8 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
   const int G = Hq / Hkv;
+  rbq_pdl_trigger();
+  rbq_pdl_wait();                                             // union lists of the plan kernel
 
   build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
   const long long total = s_start[ngroups];
@@ -668,8 +679,9 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   int32_t* ucount = reinterpret_cast<int32_t*>(ws + ctx->off_ucount);
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
   int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
-  attn_plan_kernel<<<dim3(PL_SPLIT, groups), PL_THREADS, 0, s>>>(bits, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
-                                                                 ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount, gdone);
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_plan_kernel, dim3(PL_SPLIT, groups), dim3(PL_THREADS), 0, s, bits,
+                                  (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, ctx->cfg.n_q_heads,
+                                  ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount, gdone));
   RBQ_LAUNCH_OK(ctx);
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
@@ -680,12 +692,12 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
       attr_set = true;
     }
     const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the arrival count uses one thread per CTA
-    attn_gather_kernel<<<nc, GA_THREADS, GA_SMEM, s>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)kv.k,
-                                                       (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, ulist, ucount,
-                                                       idx->n_indexed, idx->n_total, groups, ctx->cfg.n_q_heads,
-                                                       ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
-                                                       ctx->sm_scale * 1.4426950408889634f, part, gdone, out,
-                                                       ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse);
+    RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_gather_kernel, dim3(nc), dim3(GA_THREADS), (size_t)GA_SMEM, s, (const __nv_bfloat16*)q,
+                                    (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st,
+                                    (const uint32_t*)ulist, (const int32_t*)ucount, (const int32_t*)idx->n_indexed,
+                                    (const int32_t*)idx->n_total, groups, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
+                                    ctx->cfg.max_tokens, ctx->sm_scale * 1.4426950408889634f, part, gdone, out,
+                                    ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse));
     RBQ_LAUNCH_OK(ctx);
     return RBQ_OK;
   }

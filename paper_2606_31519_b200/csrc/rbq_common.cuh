@@ -93,6 +93,25 @@ __device__ __forceinline__ float rbq_fkey_inv(uint32_t k) {
   return __uint_as_float(u);
 }
 
+// ---- programmatic dependent launch (PDL) -----------------------------------------------------------
+// The kernels of a decode step are launched with programmatic stream serialisation: a kernel's CTAs may become
+// resident while its predecessor drains, which hides the launch latency between the short kernels of the step.
+// Every kernel calls rbq_pdl_trigger() first and rbq_pdl_wait() before it touches anything the predecessor
+// wrote (and before any early exit, so that completion stays transitive along the chain).
+__device__ __forceinline__ void rbq_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void rbq_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t rbq_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // ---- kernel launchers (defined in the .cu files, called from rbq_api.cu) ------------------------
 int rbq_launch_centroid(rbq_ctx*, const RbqKV&, const int32_t* seq_lens, float* c_k, cudaStream_t);
 int rbq_launch_encode(rbq_ctx*, const RbqKV&, const int32_t* t_begin, const int32_t* t_count_or_null,

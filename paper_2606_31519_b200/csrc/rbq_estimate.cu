@@ -36,10 +36,18 @@ __device__ __forceinline__ void imma_16832(int (&c)[4], uint32_t a0, uint32_t a1
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
+// first k-step of a tile: D = A*B + C with C = the (biased) start values, so no accumulator initialisation moves
+__device__ __forceinline__ void imma_16832_first(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                                 uint32_t b0, uint32_t b1, int cd, int cp) {
+  asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%11,%10,%11};"
+               : "=r"(d[0]), "=r"(d[1]), "=r"(d[2]), "=r"(d[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "r"(cd), "r"(cp));
+}
+
 // One 16-token tile: rows g (code word wa) and g+8 (code word wb) of this lane's quad column.
-__device__ __forceinline__ void tile_mma(int (&c)[4], uint32_t wa, uint32_t wb, const uint32_t (&bf)[4][2]) {
+__device__ __forceinline__ void tile_mma(int (&c)[4], uint32_t wa, uint32_t wb, const uint32_t (&bf)[4][2], int cd, int cp) {
   const uint32_t ha = wa >> 4, hb = wb >> 4;
-  imma_16832(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x02020202u, wb & 0x02020202u, bf[0][0], bf[0][1]);
+  imma_16832_first(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x02020202u, wb & 0x02020202u, bf[0][0], bf[0][1], cd, cp);
   imma_16832(c, wa & 0x04040404u, wb & 0x04040404u, wa & 0x08080808u, wb & 0x08080808u, bf[1][0], bf[1][1]);
   imma_16832(c, ha & 0x01010101u, hb & 0x01010101u, ha & 0x02020202u, hb & 0x02020202u, bf[2][0], bf[2][1]);
   imma_16832(c, ha & 0x04040404u, hb & 0x04040404u, ha & 0x08080808u, hb & 0x08080808u, bf[3][0], bf[3][1]);
@@ -65,13 +73,15 @@ __device__ __forceinline__ GroupLoad load_group(const uint32_t* __restrict__ cod
 
 // grid = k * SMs CTAs of EST_WARPS warps.  Flat group index -> (sequence b, KV head, 32-token group).
 template <bool INT_OUT, bool HAS_BIAS>
-__global__ void __launch_bounds__(EST_THREADS, 4)
+__global__ void __launch_bounds__(EST_THREADS, 3)
 estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
                 const float* __restrict__ f_bias, const int32_t* __restrict__ n_indexed,
                 const RbqQConst* __restrict__ qconst, int B, int Hq, int Hkv, int Lcap, float sm_scale,
                 float* __restrict__ scores, int32_t* __restrict__ dot_out, int32_t* __restrict__ pop_out,
                 uint32_t* __restrict__ rowmax_key) {
   __shared__ int s_gstart[EST_MAX_B + 1];     // exclusive prefix over sequences of Hkv * ceil(n_b / 32)
+  rbq_pdl_trigger();
+  rbq_pdl_wait();                               // S3's query constants and zeroed row maxima
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3, G = Hq / Hkv;
   if (tid == 0) {
@@ -116,15 +126,17 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const size_t prow = (size_t)bg * Lcap;
 
     float smax = -INFINITY;                                     // running max of this lane's head over the segment
-    GroupLoad cur = load_group(codes, f_scale, prow + (size_t)g0 * 32, g, t, Lcap - g0 * 32);
-    for (int gi = g0; gi < g1; ++gi) {
-      GroupLoad nxt = cur;
-      if (gi + 1 < g1) nxt = load_group(codes, f_scale, prow + (size_t)(gi + 1) * 32, g, t, Lcap - (gi + 1) * 32);
+    auto load_at = [&](int gi) -> GroupLoad {
+      GroupLoad r;
+      r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0u; r.fs = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (gi < g1) r = load_group(codes, f_scale, prow + (size_t)gi * 32, g, t, Lcap - gi * 32);
+      return r;
+    };
+    auto process = [&](const GroupLoad& cur, int gi) {
       // tile 0: rows g / g+8 = tokens 4g / 4g+1 ; tile 1: tokens 4g+2 / 4g+3
-      int c0[4] = {init_d, init_p, init_d, init_p};
-      int c1[4] = {init_d, init_p, init_d, init_p};
-      tile_mma(c0, cur.w[0], cur.w[1], bf);
-      tile_mma(c1, cur.w[2], cur.w[3], bf);
+      int c0[4], c1[4];
+      tile_mma(c0, cur.w[0], cur.w[1], bf, init_d, init_p);
+      tile_mma(c1, cur.w[2], cur.w[3], bf, init_d, init_p);
       const int acc_d[4] = {c0[0], c0[2], c1[0], c1[2]};
       const int acc_p[4] = {c0[1], c0[3], c1[1], c1[3]};
       const int tok = gi * 32 + 4 * g;                          // first of this lane's 4 tokens
@@ -160,7 +172,16 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
           }
         }
       }
-      cur = nxt;
+    };
+    // three groups of loads in flight per warp
+    GroupLoad l0 = load_at(g0), l1 = load_at(g0 + 1), l2 = load_at(g0 + 2);
+    for (int gi = g0; gi < g1; gi += 3) {
+      process(l0, gi);
+      l0 = load_at(gi + 3);
+      if (gi + 1 < g1) process(l1, gi + 1);
+      l1 = load_at(gi + 4);
+      if (gi + 2 < g1) process(l2, gi + 2);
+      l2 = load_at(gi + 5);
     }
     if (!INT_OUT) {                                             // row maximum for S6 (keys pre-zeroed by S3)
       smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 4));
@@ -176,17 +197,18 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
 template <bool INT_OUT, bool HAS_BIAS>
 int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, cudaStream_t s) {
   if (ctx->cfg.batch > EST_MAX_B) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch %d > %d", ctx->cfg.batch, EST_MAX_B);
-  // upper bound of the work: every sequence full; 4 CTAs (32 warps) per SM, fewer when there is little work
+  // upper bound of the work: every sequence full; 3 CTAs (24 warps) per SM, fewer when there is little work
   const long long max_groups = (long long)ctx->cfg.batch * ctx->cfg.n_kv_heads * ((ctx->cfg.max_tokens + 31) / 32);
   long long ctas = (max_groups + 2 * EST_WARPS - 1) / (2 * EST_WARPS);          // >= 2 groups per warp
-  const long long cap = (long long)ctx->sm_count * 4;
+  const long long cap = (long long)ctx->sm_count * 3;
   if (ctas > cap) ctas = cap;
   if (ctas < 1) ctas = 1;
   const RbqQConst* qc = reinterpret_cast<const RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
-  estimate_kernel<INT_OUT, HAS_BIAS><<<(int)ctas, EST_THREADS, 0, s>>>(idx->codes, idx->f_scale, idx->f_bias, idx->n_indexed, qc,
-                                                                      ctx->cfg.batch, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
-                                                                      ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop,
-                                                                      reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax));
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(estimate_kernel<INT_OUT, HAS_BIAS>, dim3((unsigned)ctas), dim3(EST_THREADS), 0, s,
+                                  (const uint32_t*)idx->codes, (const float*)idx->f_scale, (const float*)idx->f_bias,
+                                  (const int32_t*)idx->n_indexed, qc, ctx->cfg.batch, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
+                                  ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop,
+                                  reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax)));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

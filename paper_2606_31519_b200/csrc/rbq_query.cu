@@ -16,6 +16,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
              const float* __restrict__ rot, int rot_kind, int Hq, int Hkv, float sm_scale,
              uint8_t* __restrict__ qu_out, float* __restrict__ qparams, RbqQConst* __restrict__ qc_out,
              uint32_t* __restrict__ rowmax_key) {
+  rbq_pdl_trigger();                               // S4/S5 may become resident while this kernel runs
   const int G = Hq / Hkv;
   const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv;
   const int hs = threadIdx.x >> 7, j = threadIdx.x & 127;      // head slice, dim

@@ -162,6 +162,8 @@ __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
 topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
+  rbq_pdl_trigger();
+  rbq_pdl_wait();                                             // scores and row maxima of S5
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
   uint2* hist = reinterpret_cast<uint2*>(smem_raw + TP_OFF_HIST);
@@ -577,8 +579,8 @@ int launch_cs(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, con
     attr_smem = smem;
   }
   dim3 grid(CS, rows);
-  kern<<<grid, TP_THREADS, smem, s>>>(scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, wpr, p, bits, sel_idx,
-                                      sel_cnt);
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, grid, dim3(TP_THREADS), smem, s, scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads,
+                                  ctx->cfg.max_tokens, wpr, p, bits, sel_idx, sel_cnt));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
