@@ -121,7 +121,7 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
 }
 
 // ---- shared by the gather kernels: exclusive prefix of attended rows per group ----------------------------------
-constexpr int AT_MAX_GROUPS = 2048;
+constexpr int AT_MAX_GROUPS = 1024;
 
 // s_start[gi] = sum over groups < gi of (ucount + pending); s_start[ngroups] = total.  Every CTA computes the same table.
 __device__ void build_group_table(const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
@@ -158,9 +158,15 @@ __device__ void build_group_table(const int32_t* __restrict__ ucount, const int3
 __device__ __forceinline__ long long cta_begin(long long total, int c, int nc) { return total * c / nc; }
 
 // ---- tensor-pipe gather attention (bf16 K/V and q) ----------------------------------------------------------------------
-constexpr int GA_WARPS = 8;
+#ifndef RBQ_GA_WARPS
+#define RBQ_GA_WARPS 8
+#endif
+#ifndef RBQ_GA_STAGES
+#define RBQ_GA_STAGES 3
+#endif
+constexpr int GA_WARPS = RBQ_GA_WARPS;
 constexpr int GA_THREADS = GA_WARPS * 32;
-constexpr int GA_STAGES = 3;
+constexpr int GA_STAGES = RBQ_GA_STAGES;
 constexpr int GA_TILE = 16;                                   // rows per warp tile
 constexpr int GA_TILE_BYTES = GA_TILE * RBQ_D * 2;            // 4 KB per operand
 constexpr int GA_STAGE_BYTES = 2 * GA_TILE_BYTES;             // K + V
@@ -286,20 +292,25 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         cp_async16(d + GA_TILE_BYTES, Vb + off);
       }
     };
-    uint32_t ent_next[GA_STAGES - 1];
+    // entries of the tiles in flight (ring) and of the next tile to issue, loaded one iteration ahead so that the
+    // index load never sits between a freed stage and its refill
+    uint32_t ent_ring[GA_STAGES - 1], ent_pend;
+#pragma unroll
+    for (int s = 0; s < GA_STAGES - 1; ++s) ent_ring[s] = (s < my_tiles) ? tile_entry(s) : 0u;
+    ent_pend = (GA_STAGES - 1 < my_tiles) ? tile_entry(GA_STAGES - 1) : 0u;
 #pragma unroll
     for (int s = 0; s < GA_STAGES - 1; ++s) {
-      ent_next[s] = 0u;
-      if (s < my_tiles) { ent_next[s] = tile_entry(s); issue(s, ent_next[s]); }
+      if (s < my_tiles) issue(s, ent_ring[s]);
       cp_async_commit();
     }
     for (int i = 0; i < my_tiles; ++i) {
-      const uint32_t ent = ent_next[0];
-#pragma unroll
-      for (int s = 0; s + 1 < GA_STAGES - 1; ++s) ent_next[s] = ent_next[s + 1];
+      const uint32_t ent = ent_ring[0];
       const int nx = i + GA_STAGES - 1;
-      ent_next[GA_STAGES - 2] = 0u;
-      if (nx < my_tiles) { ent_next[GA_STAGES - 2] = tile_entry(nx); issue(nx, ent_next[GA_STAGES - 2]); }
+      if (nx < my_tiles) issue(nx, ent_pend);
+#pragma unroll
+      for (int s = 0; s + 1 < GA_STAGES - 1; ++s) ent_ring[s] = ent_ring[s + 1];
+      ent_ring[GA_STAGES - 2] = ent_pend;
+      ent_pend = (nx + 1 < my_tiles) ? tile_entry(nx + 1) : 0u;
       cp_async_commit();
       cp_async_wait<GA_STAGES - 1>();
       __syncwarp();
@@ -415,7 +426,9 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         s_f[h * GA_THREADS + tid] = pm; s_l[h * GA_THREADS + tid] = pl;
       }
       __syncthreads();
-      const int item = tid & 127, half = tid >> 7, h = item >> 5, d4 = (item & 31) * 4;
+      constexpr int NH = GA_THREADS >= 256 ? 2 : 1;             // slot halves worked on in parallel
+      const int item = tid & 127, half = tid >> 7, d4 = (item & 31) * 4;
+      const int h = (half < NH) ? (item >> 5) : RBQ_MAX_G;      // threads beyond NH * 128 only take part in the barriers
       float mm = -INFINITY;
       if (h < G) for (int c = clo; c <= chi; ++c) mm = fmaxf(mm, s_f[h * GA_THREADS + c]);
       __syncthreads();
@@ -433,12 +446,12 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       if (h < G) {
         const float* pcol = part + ((size_t)gi * G + h) * GA_PART + d4;
         const size_t pstride = (size_t)G * GA_PART;
-        for (int c0 = clo + half; c0 <= chi; c0 += 16) {
+        for (int c0 = clo + half; c0 <= chi; c0 += 8 * NH) {
           float f[8];
           float4 v[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
-            const int c = c0 + 2 * k;
+            const int c = c0 + NH * k;
             f[k] = (c <= chi) ? s_f[h * GA_THREADS + c] : 0.0f;
             v[k] = (f[k] != 0.0f) ? __ldcg(reinterpret_cast<const float4*>(pcol + (size_t)c * pstride)) : make_float4(0.f, 0.f, 0.f, 0.f);
           }
@@ -450,11 +463,13 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         }
         for (int c = clo; c <= chi; ++c) ll = fmaf(s_f[h * GA_THREADS + c], s_l[h * GA_THREADS + c], ll);
       }
-      if (half == 1) s_o[item] = acc;
+      if (half == 1 && NH == 2) s_o[item] = acc;
       __syncthreads();
       if (half == 0 && h < G) {
-        const float4 o2 = s_o[item];
-        acc.x += o2.x; acc.y += o2.y; acc.z += o2.z; acc.w += o2.w;
+        if (NH == 2) {
+          const float4 o2 = s_o[item];
+          acc.x += o2.x; acc.y += o2.y; acc.z += o2.z; acc.w += o2.w;
+        }
         const bool empty = !(ll > 0.0f);
         const float inv = empty ? 0.0f : 1.0f / ll;
         const size_t orow = (size_t)b * Hq + (size_t)g * G + h;
