@@ -48,7 +48,7 @@ struct TpSmall {
   double trem;            // mass still needed inside the candidate range, in units of 2^-28 * exp(-bx/64)
   u64 lo64, hi64;         // candidate range on C
   u64 cstar;
-  uint32_t bx, cntx, cnt_above, found, kx, nlist;
+  uint32_t bx, cntx, cnt_above, found, ksel;
   // read by cluster peers
   double xc_mass[TP_NC];
   uint32_t xc_cnt[TP_NC];
@@ -207,7 +207,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
   if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
   else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
-  if (tid == 0) { sh.lcount = 0; sh.found = 0; sh.nlist = 0; }
+  if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   __syncthreads();
   {
     uint32_t of_c = 0;                                        // overflow bin kept in registers (can be half the row)
@@ -266,36 +266,45 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     if ((tid & 7) == 0) { sh.xc_mass[tid >> 3] = ms * sh.tabA[tid >> 3]; sh.xc_cnt[tid >> 3] = cs; }
   }
   csync();                                                    // S1: histograms and coarse summaries complete
-  if (tid < TP_NC) {
-    double a = 0.0;
-    uint32_t c = 0;
-#pragma unroll
-    for (int r = 0; r < CS; ++r) { const TpSmall* ps = peer(r); a += ps->xc_mass[tid]; c += ps->xc_cnt[tid]; }
-    sh.tot_mass[tid] = a; sh.tot_cnt[tid] = c;
-  }
-  __syncthreads();
   if (warp == 0) {
-    // coarse crossing (lane 0, serial over 64 bins), then the 32 fine bins of that coarse bin (one per lane)
-    double T = 0.0, above = 0.0;
-    uint32_t cab = 0;
-    int kx = 0;
-    if (lane == 0) {
-      double Z = 0.0;
-      for (int k = 0; k < TP_NC; ++k) Z += sh.tot_mass[k];
-      T = (double)p_f * Z;
-      double cum = 0.0;
-      int last = 0;
-      kx = -1;
-      for (int k = 0; k < TP_NC; ++k) {
-        if (sh.tot_cnt[k] == 0) continue;
-        last = k;
-        if (cum + sh.tot_mass[k] >= T) { kx = k; break; }
-        cum += sh.tot_mass[k]; cab += sh.tot_cnt[k];
-      }
-      if (kx < 0) { kx = last; cum -= sh.tot_mass[last]; cab -= sh.tot_cnt[last]; }
-      above = cum;
+    // coarse crossing: lane l owns coarse bins 2l, 2l+1 (totals over the cluster in rank order), warp scan in fp64;
+    // then the 32 fine bins of the crossing coarse bin, one per lane
+    double m0 = 0.0, m1 = 0.0;
+    uint32_t c0 = 0, c1 = 0;
+#pragma unroll
+    for (int r = 0; r < CS; ++r) {
+      const TpSmall* ps = peer(r);
+      m0 += ps->xc_mass[2 * lane]; m1 += ps->xc_mass[2 * lane + 1];
+      c0 += ps->xc_cnt[2 * lane]; c1 += ps->xc_cnt[2 * lane + 1];
     }
-    kx = __shfl_sync(FULL, kx, 0); T = __shfl_sync(FULL, T, 0); above = __shfl_sync(FULL, above, 0); cab = __shfl_sync(FULL, cab, 0);
+    double si2 = m0 + m1;
+    uint32_t ci2 = c0 + c1;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const double v = __shfl_up_sync(FULL, si2, o);
+      const uint32_t cv = __shfl_up_sync(FULL, ci2, o);
+      if (lane >= o) { si2 += v; ci2 += cv; }
+    }
+    const double Z = __shfl_sync(FULL, si2, 31);
+    double T = (double)p_f * Z;
+    const double ex2 = si2 - (m0 + m1);
+    const uint32_t cex = ci2 - (c0 + c1);
+    const bool x0 = c0 > 0 && ex2 + m0 >= T, x1 = c1 > 0 && (ex2 + m0) + m1 >= T;
+    unsigned cb = __ballot_sync(FULL, x0 || x1);
+    const unsigned ne = __ballot_sync(FULL, (c0 | c1) != 0);
+    bool forced = false;
+    if (cb == 0u) { cb = ne ? (1u << (31 - __clz(ne))) : 1u; forced = true; }   // rounding at the last ulp: last non-empty bin
+    const int lsel = __ffs(cb) - 1;
+    int kx = 0;
+    double above = 0.0;
+    uint32_t cab = 0;
+    if (lane == lsel) {
+      const bool second = forced ? (c1 > 0) : !x0;
+      kx = 2 * lane + (second ? 1 : 0);
+      above = second ? ex2 + m0 : ex2;
+      cab = second ? cex + c0 : cex;
+    }
+    kx = __shfl_sync(FULL, kx, lsel); above = __shfl_sync(FULL, above, lsel); cab = __shfl_sync(FULL, cab, lsel);
     uint32_t c = 0;
     u64 R = 0;
 #pragma unroll
@@ -398,17 +407,23 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   {
     u64 lo64 = 0, hi64 = 0;
     if (use_range) { lo64 = sh.lo64; hi64 = sh.hi64; }
-    for (int i = tid; i < len; i += TP_THREADS) {
-      const float s = sc[i];
-      const float u = __fsub_rn(m, s);
-      bool is = (u >= u_lo && u < u_hi);
-      if (is && use_range) { const u64 c = composite(s, lo + i); is = (c >= lo64 && c <= hi64); }
-      if (is) {
-        int j_unused;
-        uint32_t rfix;
-        bin0(m, s, j_unused, rfix);
-        const uint32_t slot = atomicAdd(&sh.lcount, 1u);
-        if (slot < TP_CAND) { loc_comp[slot] = composite(s, lo + i); loc_rfix[slot] = rfix; }
+    const int n4 = (len + 3) >> 2;
+    for (int i4 = tid; i4 < n4; i4 += TP_THREADS) {
+      const float4 v4 = reinterpret_cast<const float4*>(sc)[i4];
+      const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float u = __fsub_rn(m, v[k]);
+        if (u >= u_lo && u < u_hi && 4 * i4 + k < len) {
+          const u64 c = composite(v[k], lo + 4 * i4 + k);
+          if (!use_range || (c >= lo64 && c <= hi64)) {
+            int j_unused;
+            uint32_t rfix;
+            bin0(m, v[k], j_unused, rfix);
+            const uint32_t slot = atomicAdd(&sh.lcount, 1u);
+            if (slot < TP_CAND) { loc_comp[slot] = c; loc_rfix[slot] = rfix; }
+          }
+        }
       }
     }
   }
@@ -426,91 +441,70 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   }
   __syncthreads();
 
-  // ---- exact cut among the candidates: local radix levels until <= TP_RANK remain, then direct ranking ------
+  // ---- exact cut: every CTA ranks its share of the candidates against all of them (4 threads per candidate, integer
+  //      prefix masses); the one thread that finds the cut publishes it to every CTA of the cluster -----------------
   {
-    // each thread keeps up to 2 candidates in registers
-    u64 cc[2];
-    uint32_t cr[2];
-    bool cv[2];
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int i = tid + k * TP_THREADS;
-      cv[k] = i < ncand;
-      cc[k] = cv[k] ? all_comp[i] : 0ull;
-      cr[k] = cv[k] ? all_rfix[i] : 0u;
-    }
-    int live = ncand;
-    while (live > TP_RANK) {
-      u64 mn = ~0ull, mx = 0ull;
-#pragma unroll
-      for (int k = 0; k < 2; ++k) if (cv[k]) { mn = min(mn, cc[k]); mx = max(mx, cc[k]); }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) { mn = min(mn, __shfl_xor_sync(FULL, mn, o)); mx = max(mx, __shfl_xor_sync(FULL, mx, o)); }
-      if (lane == 0) { sh.red_lo[warp] = mn; sh.red_hi[warp] = mx; }
-      for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
-      __syncthreads();
-      u64 lo64 = ~0ull, hi64 = 0ull;
-      for (int w = 0; w < TP_WARPS; ++w) { lo64 = min(lo64, sh.red_lo[w]); hi64 = max(hi64, sh.red_hi[w]); }
-      const int shift = max(0, (64 - __clzll((long long)(hi64 - lo64))) - 11);
-#pragma unroll
-      for (int k = 0; k < 2; ++k)
-        if (cv[k]) hist_add(hist, TP_NB - 1 - (int)((cc[k] - lo64) >> shift), (u64)cr[k], 1u);
-      __syncthreads();
-      uint32_t cnt[4];
-      u64 R[4];
-#pragma unroll
-      for (int k = 0; k < 4; ++k) unpack_bin(hist[4 * tid + k], cnt[k], R[k]);
-      radix_scan(sh, cnt, R, lo64, hi64, shift);
-      const u64 nlo = sh.lo64, nhi = sh.hi64;
-#pragma unroll
-      for (int k = 0; k < 2; ++k) cv[k] = cv[k] && cc[k] >= nlo && cc[k] <= nhi;
-      live = (int)sh.cntx;
-      __syncthreads();                                        // sh.* and hist reused by the next level
-      if (shift == 0) break;
-    }
-    // survivors -> compact list (aliases the gathered arrays: all threads hold their candidates in registers)
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      if (cv[k]) {
-        const uint32_t slot = atomicAdd(&sh.nlist, 1u);
-        if (slot < TP_CAND) { all_comp[slot] = cc[k]; all_rfix[slot] = cr[k]; }
-      }
-    }
-    __syncthreads();
-    const int nl = min((int)sh.nlist, TP_CAND);
     const double trem = sh.trem;
-    for (int i = tid; i < nl; i += TP_THREADS) {
-      const u64 ci = all_comp[i];
+    const int per = (ncand + CS - 1) / CS;
+    const int i0 = rank * per, i1 = min(ncand, i0 + per);
+    const int sub = tid & 3;
+    const int jq = (ncand + 3) >> 2, j0 = sub * jq, j1 = min(ncand, j0 + jq);
+    for (int ib = i0; ib < i1; ib += TP_THREADS / 4) {
+      const int i = ib + (tid >> 2);
+      const bool valid = i < i1;
+      const u64 ci = valid ? all_comp[i] : ~0ull;
       u64 P = 0;
       uint32_t rk = 0;
-      for (int j = 0; j < nl; ++j) {
+      for (int j = j0; j < j1; ++j) {
         const bool ge = all_comp[j] >= ci;
         P += ge ? (u64)all_rfix[j] : 0ull;
         rk += ge ? 1u : 0u;
       }
-      if ((double)P >= trem && (double)(P - all_rfix[i]) < trem) { sh.cstar = ci; sh.cnt_above += rk; sh.found = 1; }
+      P += __shfl_xor_sync(FULL, P, 1); rk += __shfl_xor_sync(FULL, rk, 1);
+      P += __shfl_xor_sync(FULL, P, 2); rk += __shfl_xor_sync(FULL, rk, 2);
+      if (valid && sub == 0 && (double)P >= trem && (double)(P - all_rfix[i]) < trem) {
+#pragma unroll
+        for (int r = 0; r < CS; ++r) {
+          TpSmall* ps = CS == 1 ? &sh : cluster.map_shared_rank(&sh, r);
+          ps->cstar = ci; ps->ksel = sh.cnt_above + rk; ps->found = 1;
+        }
+      }
     }
-    __syncthreads();
-    if (!sh.found && tid == 0) {                              // rounding at the last ulp / zero weights: take every survivor
+  }
+  csync();                                                    // S3: the cut is visible in every CTA
+  if (!sh.found) {                                            // zero-weight candidates / rounding at the last ulp: take all of them
+    if (tid == 0) {
       u64 mn = ~0ull;
-      for (int j = 0; j < nl; ++j) mn = min(mn, all_comp[j]);
-      sh.cstar = mn; sh.cnt_above += (uint32_t)nl;
+      for (int j = 0; j < ncand; ++j) mn = min(mn, all_comp[j]);
+      sh.cstar = mn; sh.ksel = sh.cnt_above + (uint32_t)ncand;
     }
     __syncthreads();
   }
   const u64 cstar = sh.cstar;
-  const uint32_t total_sel = sh.cnt_above;
+  const uint32_t total_sel = sh.ksel;
 
-  // ---- pass 3: bitmap words (always), ascending index list (on request) ---------------------------------------
+  // ---- pass 3: bitmap words (always), ascending index list (on request).  A lane classifies 4 consecutive tokens,
+  //      8 lanes assemble one 32-token word ---------------------------------------------------------------------
   {
     const float sstar = rbq_fkey_inv((uint32_t)(cstar >> 32));
     const int tstar = (int)(~(uint32_t)cstar);                // equal scores: indices <= tstar are selected
-    for (int w = warp; w < nwords; w += TP_WARPS) {
-      const int i = w * 32 + lane;
-      bool sel = false;
-      if (i < len) { const float s = sc[i]; sel = (s > sstar) || (s == sstar && lo + i <= tstar); }
-      const unsigned bal = __ballot_sync(FULL, sel);
-      if (lane == 0) { bits_row[(lo >> 5) + w] = bal; selw[w] = bal; }
+    const int n4r = nwords * 8;                               // float4 groups, rounded up to whole words
+    for (int base = warp * 32; base < n4r; base += TP_THREADS) {
+      const int i4 = base + lane;
+      const float4 v4 = (i4 < n4r) ? reinterpret_cast<const float4*>(sc)[i4] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+      uint32_t nib = 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int i = 4 * i4 + k;
+        const bool sel = (i < len) && ((v[k] > sstar) || (v[k] == sstar && lo + i <= tstar));
+        nib |= sel ? (1u << k) : 0u;
+      }
+      uint32_t word = nib << (4 * (lane & 7));
+      word |= __shfl_xor_sync(FULL, word, 1);
+      word |= __shfl_xor_sync(FULL, word, 2);
+      word |= __shfl_xor_sync(FULL, word, 4);
+      if ((lane & 7) == 0 && i4 < n4r) { const int w = i4 >> 3; bits_row[(lo >> 5) + w] = word; selw[w] = word; }
     }
   }
   if (rank == 0 && tid == 0) sel_cnt[row] = (int32_t)total_sel;
