@@ -213,7 +213,7 @@ class RaBitQCache:
 
     def __init__(self, batch, n_q_heads, n_kv_heads, max_tokens, rot: torch.Tensor, *, head_dim=128, flush_tokens=0,
                  kv_dtype=torch.bfloat16, q_dtype=None, out_dtype=None, sm_scale=0.0, rot_kind=RBQ_ROT_DENSE,
-                 enc_mode=RBQ_ENC_EXACT, with_cq=False, device="cuda"):
+                 enc_mode=RBQ_ENC_EXACT, with_cq=False, device="cuda", interleave_kv=True):
         self.dev = torch.device(device)
         self.B, self.Hq, self.Hkv, self.D, self.Lcap = batch, n_q_heads, n_kv_heads, head_dim, max_tokens
         self.kv_dtype = kv_dtype
@@ -227,8 +227,14 @@ class RaBitQCache:
         self.ws = torch.empty(rbq_workspace_bytes(self.ctx), dtype=torch.uint8, device=self.dev)
         rbq_set_workspace(self.ctx, self.ws)
         z = dict(device=self.dev)
-        self.K = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
-        self.V = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
+        if interleave_kv:
+            # one allocation [B][Hkv][Lcap][2][D]: the K row and the V row of a token are adjacent in HBM, so the gather
+            # attention fetches 4*D contiguous bytes per attended token (rbq_kv carries the strides: stride_t = 2*D)
+            self.KV = torch.zeros(batch, n_kv_heads, max_tokens, 2, head_dim, dtype=kv_dtype, **z)
+            self.K, self.V = self.KV[:, :, :, 0, :], self.KV[:, :, :, 1, :]
+        else:
+            self.K = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
+            self.V = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
         self.codes = torch.zeros(batch, n_kv_heads, max_tokens, head_dim // 32, dtype=torch.int32, **z)
         self.f_scale = torch.zeros(batch, n_kv_heads, max_tokens, dtype=torch.float32, **z)
         self.c_k = torch.zeros(batch, n_kv_heads, head_dim, dtype=torch.float32, **z)

@@ -25,7 +25,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
 
   extern __shared__ __align__(16) float s_rot[];  // dense: P [D][D] staged with one round of independent 128-bit loads
   __shared__ float s_ck[RBQ_D], s_cq[RBQ_MAX_G][RBQ_D];
-  __shared__ float s_x[RBQ_MAX_G][RBQ_D];      // xq, then u
+  __shared__ __align__(16) float s_x[RBQ_MAX_G][RBQ_D];      // xq, then u
   __shared__ float s_y[RBQ_MAX_G][RBQ_D];      // q'
   __shared__ float s_red[RBQ_MAX_G][8];        // per-warp min / max
   __shared__ int s_isum[RBQ_MAX_G][4];
@@ -42,11 +42,11 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   s_y[hs][j] = qv;                               // staged for the fp64 dot chains below
   s_cq[hs][j] = cqv;
   if (hs == 0) s_ck[j] = ckv;
-  if (rot_kind == RBQ_ROT_DENSE) {
-    const float4* src = reinterpret_cast<const float4*>(rot);
-    float4* dst = reinterpret_cast<float4*>(s_rot);
-#pragma unroll 8
-    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x) dst[i] = src[i];
+  if (rot_kind == RBQ_ROT_DENSE) {                 // P -> shared memory, asynchronously; awaited just before the rotation
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_rot);
+    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (uint32_t)i), "l"(rot + 4 * i) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
   }
   __syncthreads();
   // ||xq||: the canonical sequential fp32 chain (R1) on one thread per head; the two fp64 dot products
@@ -62,9 +62,19 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
     if ((j & 31) == 0) { s_dred[hs][0][j >> 5] = p0; s_dred[hs][1][j >> 5] = p1; }
   }
   if (j == 0) {
+    // compact loops on purpose: this code runs once per launch, so straight-line code is instruction-fetch bound
     float n2 = 0.0f;
-#pragma unroll 16
-    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(s_x[hs][i], s_x[hs][i], n2);
+#pragma unroll 1
+    for (int i0 = 0; i0 < RBQ_D; i0 += 16) {
+      float4 xv[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) xv[k] = *reinterpret_cast<const float4*>(&s_x[hs][i0 + 4 * k]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        n2 = fmaf(xv[k].x, xv[k].x, n2); n2 = fmaf(xv[k].y, xv[k].y, n2);
+        n2 = fmaf(xv[k].z, xv[k].z, n2); n2 = fmaf(xv[k].w, xv[k].w, n2);
+      }
+    }
     s_qn[hs] = __fsqrt_rn(n2);
   }
   __syncthreads();
@@ -75,14 +85,37 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   const float qn = s_qn[hs];
   const float u = (qn > 0.0f) ? __fdiv_rn(xq, qn) : 0.0f;
   s_x[hs][j] = u;
+  asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
 
   float qp;
   if (rot_kind == RBQ_ROT_DENSE) {
-    float acc = 0.0f;
-#pragma unroll 32
-    for (int i = 0; i < RBQ_D; ++i) acc = fmaf(s_x[hs][i], s_rot[i * RBQ_D + j], acc);
-    qp = acc;
+    // Threads 0..127 own one output column each for ALL heads of the group: one shared-memory read of P[i][j] feeds G
+    // independent canonical chains (reading P once per head instead would be bound by shared-memory bandwidth).
+    if (threadIdx.x < RBQ_D) {
+      const int jj = threadIdx.x;
+      float acc[RBQ_MAX_G];
+#pragma unroll
+      for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) acc[h2] = 0.0f;
+#pragma unroll 1
+      for (int i0 = 0; i0 < RBQ_D; i0 += 8) {
+        float rv[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) rv[k] = s_rot[(i0 + k) * RBQ_D + jj];
+#pragma unroll
+        for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) {
+          const float4 xa = *reinterpret_cast<const float4*>(&s_x[h2][i0]), xb = *reinterpret_cast<const float4*>(&s_x[h2][i0 + 4]);
+          float a = acc[h2];
+          a = fmaf(xa.x, rv[0], a); a = fmaf(xa.y, rv[1], a); a = fmaf(xa.z, rv[2], a); a = fmaf(xa.w, rv[3], a);
+          a = fmaf(xb.x, rv[4], a); a = fmaf(xb.y, rv[5], a); a = fmaf(xb.z, rv[6], a); a = fmaf(xb.w, rv[7], a);
+          acc[h2] = a;
+        }
+      }
+#pragma unroll
+      for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) s_y[h2][jj] = acc[h2];
+    }
+    __syncthreads();
+    qp = s_y[hs][j];
   } else {
     // warp 0 of the slice runs the 128-point butterflies (4 elements per lane), as in S1
     if (j < 32) {

@@ -67,12 +67,12 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^28
+// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^28 = 2^(28 - (64u - j) log2(e)/64)
 __device__ __forceinline__ void bin0(float m, float s, int& j, uint32_t& rfix) {
-  const float u = __fsub_rn(m, s);
-  j = min(TP_NB - 1, __float2int_rz(__fmul_rn(u, 64.0f)));
-  const float frac = __fsub_rn(u, __fmul_rn((float)j, 0.015625f));
-  rfix = __float2uint_rn(__fmul_rn(ex2_approx(__fmul_rn(frac, -1.4426950408889634f)), 268435456.0f));
+  const float t = __fmul_rn(__fsub_rn(m, s), 64.0f);
+  j = min(TP_NB - 1, __float2int_rz(t));
+  const float f = __fsub_rn(t, (float)j);                     // exact for j < TP_NB - 1; large in the overflow bin
+  rfix = __float2uint_rn(ex2_approx(fmaf(f, -0.022542110013890053f, 28.0f)));
 }
 __device__ __forceinline__ u64 composite(float s, int t) {
   return ((u64)rbq_fkey(s) << 32) | (u64)(~(uint32_t)t);
@@ -240,8 +240,10 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
       } else {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          if (j[k] == TP_NB - 1) { of_c += 1; of_r += rf[k]; }
-          else if (j[k] >= 0) hist_add(hist, j[k], (u64)rf[k], 1u);
+          const bool of = j[k] == TP_NB - 1;
+          of_c += of ? 1u : 0u;
+          of_r += of ? (u64)rf[k] : 0ull;
+          if (j[k] >= 0 && !of) hist_add(hist, j[k], (u64)rf[k], 1u);
         }
       }
     }
