@@ -45,11 +45,12 @@ def _chained(orc, w, rot, kind, p, with_cq=False):
     n_rows = np.repeat(w.seq_lens, w.Hq)
     ref_idx, ref_cnt = orc.topp(s.reshape(w.B * w.Hq, w.Lcap), n_rows, p)     # exact rule on the GPU's logits
     ref_idx, ref_cnt = ref_idx.reshape(w.B, w.Hq, w.Lcap), ref_cnt.reshape(w.B, w.Hq)
+    idx2 = sel_idx2.cpu().numpy()
     for b in range(w.B):
         n = int(w.seq_lens[b])
         for h in range(w.Hq):
             g = idx[b, h, :cnt[b, h]]
-            assert (g == sel_idx2.cpu().numpy()[b, h, :cnt[b, h]]).all(), "fused and staged selections differ"
+            assert (g == idx2[b, h, :cnt[b, h]]).all(), "fused and staged selections differ"
             U.assert_topp_row(s[b, h, :n], g, ref_idx[b, h, :ref_cnt[b, h]], p)
     # budgets of the oracle chain and the GPU chain agree closely (boundary tokens only)
     assert np.abs(cnt.astype(np.int64) - o["sel_cnt"]).max() <= max(2, int(0.002 * o["sel_cnt"].max()))
@@ -221,3 +222,24 @@ def test_error_codes(rot128):
     with pytest.raises(rb.RbqError):
         rb.rbq_topp_select(h, q, idx, 0.0, q, q)                                              # p must be > 0
     assert lib.rbq_destroy(h) == 0
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_configs(orc, rot128, cfg):
+    """BASELINE.json configs 2 and 3 at FULL size (131 072-token context; 16 ragged sequences of 16 K - 64 K tokens), in the
+    launch configuration bench.py times: the whole chain against the oracle (codes bit-exact inside _chained's encode
+    check below, logits 1e-5, Top-p sets by the exact rule on the GPU's logits, outputs within tolerance)."""
+    import torch
+    w = U.workload(cfg)
+    o = _chained(orc, w, rot128[0], ROT_DENSE, w.p)
+    # codes and factors at full size, bit for bit
+    c = U.make_cache(w, rot128[0])
+    c.encode_keys(U.to_dev(w.seq_lens))
+    torch.cuda.synchronize()
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        assert (codes[b, :, :n] == o["codes"][b, :, :n]).all()
+        assert (fs[b, :, :n].view(np.uint32) == o["f_scale"][b, :, :n].view(np.uint32)).all()
+    c.close()
