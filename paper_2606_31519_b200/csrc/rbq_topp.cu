@@ -214,11 +214,19 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     u64 of_r = 0;
     const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
     const int n4 = (len + 3) >> 2;                            // whole float4 groups (Lcap % 4 == 0: in bounds)
+    // the whole slice in flight at once (16-byte cp.async, one latency round), then histogrammed from shared memory
+    {
+      const uint32_t sdst = (uint32_t)__cvta_generic_to_shared(sc);
+      for (int i4 = tid; i4 < n4; i4 += TP_THREADS)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst + 16u * (uint32_t)i4), "l"(src + i4) : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
     for (int base = warp * 32; base < n4; base += TP_THREADS) {
       const int i4 = base + lane;
       float v[4] = {0.f, 0.f, 0.f, 0.f};
-      if (i4 < n4) {
-        const float4 t4 = __ldcs(src + i4);
+      if (i4 < n4) {                                            // each thread reads back exactly the groups it copied
+        const float4 t4 = reinterpret_cast<const float4*>(sc)[i4];
         v[0] = __fadd_rn(t4.x, 0.0f); v[1] = __fadd_rn(t4.y, 0.0f); v[2] = __fadd_rn(t4.z, 0.0f); v[3] = __fadd_rn(t4.w, 0.0f);   // -0 -> +0
         reinterpret_cast<float4*>(sc)[i4] = make_float4(v[0], v[1], v[2], v[3]);
       }
@@ -431,39 +439,47 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   }
   csync();                                                    // S2: candidate lists complete; histograms free
   int ncand = 0;
+  {
+    int off[CS + 1];                                          // all peer counts first, then one round of independent remote loads
+    off[0] = 0;
 #pragma unroll
-  for (int r = 0; r < CS; ++r) {
-    const int lc = min((int)peer(r)->lcount, TP_CAND);
-    const u64* rc = CS == 1 ? loc_comp : cluster.map_shared_rank(loc_comp, r);
-    const uint32_t* rr = CS == 1 ? loc_rfix : cluster.map_shared_rank(loc_rfix, r);
-    for (int k = tid; k < lc; k += TP_THREADS) {
-      if (ncand + k < TP_CAND) { all_comp[ncand + k] = rc[k]; all_rfix[ncand + k] = rr[k]; }
+    for (int r = 0; r < CS; ++r) off[r + 1] = min(TP_CAND, off[r] + min((int)peer(r)->lcount, TP_CAND));
+    ncand = off[CS];
+    for (int k = tid; k < ncand; k += TP_THREADS) {
+      int r = 0;
+#pragma unroll
+      for (int q = 1; q < CS; ++q) r += (k >= off[q]) ? 1 : 0;
+      int base = 0;
+#pragma unroll
+      for (int q = 0; q < CS; ++q) base = (q == r) ? off[q] : base;
+      const u64* rc = CS == 1 ? loc_comp : cluster.map_shared_rank(loc_comp, r);
+      const uint32_t* rr = CS == 1 ? loc_rfix : cluster.map_shared_rank(loc_rfix, r);
+      all_comp[k] = rc[k - base]; all_rfix[k] = rr[k - base];
     }
-    ncand = min(TP_CAND, ncand + lc);
   }
   __syncthreads();
 
-  // ---- exact cut: every CTA ranks its share of the candidates against all of them (4 threads per candidate, integer
+  // ---- exact cut: every CTA ranks its share of the candidates against all of them (8 threads per candidate, integer
   //      prefix masses); the one thread that finds the cut publishes it to every CTA of the cluster -----------------
   {
     const double trem = sh.trem;
     const int per = (ncand + CS - 1) / CS;
     const int i0 = rank * per, i1 = min(ncand, i0 + per);
-    const int sub = tid & 3;
-    const int jq = (ncand + 3) >> 2, j0 = sub * jq, j1 = min(ncand, j0 + jq);
-    for (int ib = i0; ib < i1; ib += TP_THREADS / 4) {
-      const int i = ib + (tid >> 2);
+    const int sub = tid & 7;
+    for (int ib = i0; ib < i1; ib += TP_THREADS / 8) {
+      const int i = ib + (tid >> 3);
       const bool valid = i < i1;
       const u64 ci = valid ? all_comp[i] : ~0ull;
       u64 P = 0;
       uint32_t rk = 0;
-      for (int j = j0; j < j1; ++j) {
+#pragma unroll 4
+      for (int j = sub; j < ncand; j += 8) {                    // 8 consecutive candidates per warp load: conflict-free
         const bool ge = all_comp[j] >= ci;
         P += ge ? (u64)all_rfix[j] : 0ull;
         rk += ge ? 1u : 0u;
       }
-      P += __shfl_xor_sync(FULL, P, 1); rk += __shfl_xor_sync(FULL, rk, 1);
-      P += __shfl_xor_sync(FULL, P, 2); rk += __shfl_xor_sync(FULL, rk, 2);
+#pragma unroll
+      for (int o = 1; o < 8; o <<= 1) { P += __shfl_xor_sync(FULL, P, o); rk += __shfl_xor_sync(FULL, rk, o); }
       if (valid && sub == 0 && (double)P >= trem && (double)(P - all_rfix[i]) < trem) {
 #pragma unroll
         for (int r = 0; r < CS; ++r) {
