@@ -416,52 +416,69 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       float* s_l = stg + RBQ_MAX_G * GA_THREADS;
       float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [128] second half's partial sums
       const int clo = s_clo, chi = s_chi;
+      // thread tid owns slot tid: per-head maximum and normaliser by block reductions (warp shuffles + one shared round)
+      float* s_red = stg + 2 * RBQ_MAX_G * GA_THREADS + 4 * RBQ_D;   // [2][RBQ_MAX_G][GA_WARPS]
+      float pm[RBQ_MAX_G], pl[RBQ_MAX_G];
 #pragma unroll
       for (int h = 0; h < RBQ_MAX_G; ++h) {
-        float pm = -INFINITY, pl = 0.0f;
+        pm[h] = -INFINITY; pl[h] = 0.0f;
         if (h < G && touches) {
           const float* pp = part + ((size_t)(tid + gi) * G + h) * GA_PART;
-          pm = __ldcg(pp + RBQ_D); pl = __ldcg(pp + RBQ_D + 1);
+          pm[h] = __ldcg(pp + RBQ_D); pl[h] = __ldcg(pp + RBQ_D + 1);
         }
-        s_f[h * GA_THREADS + tid] = pm; s_l[h * GA_THREADS + tid] = pl;
+      }
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        float v = pm[h];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if (lane == 0) s_red[h * GA_WARPS + warp] = v;
+      }
+      __syncthreads();
+      float mall[RBQ_MAX_G];
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        float v = -INFINITY;
+#pragma unroll
+        for (int w = 0; w < GA_WARPS; ++w) v = fmaxf(v, s_red[h * GA_WARPS + w]);
+        mall[h] = v;
+        const float f = (pm[h] == -INFINITY) ? 0.0f : exp2f(pm[h] - v);
+        s_f[h * GA_THREADS + tid] = f;
+        float fl = f * pl[h];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) fl += __shfl_xor_sync(0xffffffffu, fl, o);
+        if (lane == 0) s_red[(RBQ_MAX_G + h) * GA_WARPS + warp] = fl;
       }
       __syncthreads();
       constexpr int NH = GA_THREADS >= 256 ? 2 : 1;             // slot halves worked on in parallel
       const int item = tid & 127, half = tid >> 7, d4 = (item & 31) * 4;
       const int h = (half < NH) ? (item >> 5) : RBQ_MAX_G;      // threads beyond NH * 128 only take part in the barriers
       float mm = -INFINITY;
-      if (h < G) for (int c = clo; c <= chi; ++c) mm = fmaxf(mm, s_f[h * GA_THREADS + c]);
-      __syncthreads();
 #pragma unroll
-      for (int hh = 0; hh < RBQ_MAX_G; ++hh) {                  // thread tid converts slot tid: needs the max of every head
-        float mh = -INFINITY;
-        if (hh < G) for (int c = clo; c <= chi; ++c) mh = fmaxf(mh, s_f[hh * GA_THREADS + c]);
-        const float mc = s_f[hh * GA_THREADS + tid];
-        __syncthreads();
-        s_f[hh * GA_THREADS + tid] = (mc == -INFINITY) ? 0.0f : exp2f(mc - mh);
-      }
-      __syncthreads();
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) mm = (hh == h) ? mall[hh] : mm;
       float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
       float ll = 0.0f;
       if (h < G) {
         const float* pcol = part + ((size_t)gi * G + h) * GA_PART + d4;
         const size_t pstride = (size_t)G * GA_PART;
-        for (int c0 = clo + half; c0 <= chi; c0 += 8 * NH) {
-          float f[8];
-          float4 v[8];
+        constexpr int MU = 24;                                  // slot partials in flight per thread: one round for <= 48 slots
+        for (int c0 = clo + half; c0 <= chi; c0 += MU * NH) {
+          float f[MU];
+          float4 v[MU];
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
+          for (int k = 0; k < MU; ++k) {
             const int c = c0 + NH * k;
             f[k] = (c <= chi) ? s_f[h * GA_THREADS + c] : 0.0f;
             v[k] = (f[k] != 0.0f) ? __ldcg(reinterpret_cast<const float4*>(pcol + (size_t)c * pstride)) : make_float4(0.f, 0.f, 0.f, 0.f);
           }
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
+          for (int k = 0; k < MU; ++k) {
             acc.x = fmaf(f[k], v[k].x, acc.x); acc.y = fmaf(f[k], v[k].y, acc.y);
             acc.z = fmaf(f[k], v[k].z, acc.z); acc.w = fmaf(f[k], v[k].w, acc.w);
           }
         }
-        for (int c = clo; c <= chi; ++c) ll = fmaf(s_f[h * GA_THREADS + c], s_l[h * GA_THREADS + c], ll);
+#pragma unroll
+        for (int w = 0; w < GA_WARPS; ++w) ll += s_red[(RBQ_MAX_G + h) * GA_WARPS + w];
       }
       if (half == 1 && NH == 2) s_o[item] = acc;
       __syncthreads();
