@@ -80,8 +80,7 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
                 float* __restrict__ scores, int32_t* __restrict__ dot_out, int32_t* __restrict__ pop_out,
                 uint32_t* __restrict__ rowmax_key) {
   __shared__ int s_gstart[EST_MAX_B + 1];     // exclusive prefix over sequences of Hkv * ceil(n_b / 32)
-  rbq_pdl_trigger();
-  rbq_pdl_wait();                               // S3's query constants and zeroed row maxima
+  rbq_pdl_trigger();                            // the wait for S3 comes after the first code loads are in flight
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3, G = Hq / Hkv;
   if (tid == 0) {
@@ -94,7 +93,8 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
   const long long nwarps = (long long)gridDim.x * EST_WARPS, wid = (long long)blockIdx.x * EST_WARPS + warp;
   long long gcur = total * wid / nwarps;
   const long long gend = total * (wid + 1) / nwarps;
-  if (gcur >= gend) return;
+  if (gcur >= gend) { rbq_pdl_wait(); return; }
+  bool first_segment = true;
   int b = 0;
   {
     int lo = 0, hi = B - 1;                    // last b with s_gstart[b] <= gcur
@@ -113,6 +113,16 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const int gk = rel / gpb, g0 = rel % gpb;
     const int g1 = (int)min((long long)gpb, (long long)g0 + (gend - gcur));
     const int bg = b * Hkv + gk;
+    const size_t prow = (size_t)bg * Lcap;
+    auto load_at = [&](int gi) -> GroupLoad {
+      GroupLoad r;
+      r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0u; r.fs = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (gi < g1) r = load_group(codes, f_scale, prow + (size_t)gi * 32, g, t, Lcap - gi * 32);
+      return r;
+    };
+    // three groups of loads in flight per warp; codes and factors do not depend on S3, its constants do
+    GroupLoad l0 = load_at(g0), l1 = load_at(g0 + 1), l2 = load_at(g0 + 2);
+    if (first_segment) { rbq_pdl_wait(); first_segment = false; }   // S3's query constants and zeroed row maxima
     const RbqQConst* qc = qconst + bg;
     uint32_t bf[4][2];
 #pragma unroll
@@ -123,15 +133,8 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const float cA = qc->cA[hsel], cB = qc->cB[hsel], cD = qc->cD[hsel];
     const int init_d = qc->init_d[hsel], init_p = qc->init_p;
     const size_t row = ((size_t)b * Hq + gk * G + hsel) * Lcap;
-    const size_t prow = (size_t)bg * Lcap;
 
     float smax = -INFINITY;                                     // running max of this lane's head over the segment
-    auto load_at = [&](int gi) -> GroupLoad {
-      GroupLoad r;
-      r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0u; r.fs = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (gi < g1) r = load_group(codes, f_scale, prow + (size_t)gi * 32, g, t, Lcap - gi * 32);
-      return r;
-    };
     auto process = [&](const GroupLoad& cur, int gi) {
       // tile 0: rows g / g+8 = tokens 4g / 4g+1 ; tile 1: tokens 4g+2 / 4g+3
       int c0[4], c1[4];
@@ -173,8 +176,6 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
         }
       }
     };
-    // three groups of loads in flight per warp
-    GroupLoad l0 = load_at(g0), l1 = load_at(g0 + 1), l2 = load_at(g0 + 2);
     for (int gi = g0; gi < g1; gi += 3) {
       process(l0, gi);
       l0 = load_at(gi + 3);

@@ -8,15 +8,16 @@
 // once.  The selection is an exact cut in the total order (score descending, index ascending), i.e.
 // on the composite key  C(t) = (orderkey(score_t) << 32) | ~t  whose values are all distinct.
 // The row maximum m comes with the scores (S5 epilogue, or rowmax_kernel for caller-provided scores):
-//   pass 1  : while the slice is loaded, 2048 bins of width 1/64 in u = m - score (monotone in C).
-//             Per bin a (count, sum of r) pair, r = 2^(-(u - j/64) log2 e) in 2^-28 fixed point, so the
-//             bin mass is exp(-j/64) * sum(r): integer sums => order-independent and deterministic.
-//             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin
-//             travel through distributed shared memory (DSMEM is ~20 B/clk per SM).
-//   pass 2  : the tokens of the crossing bin (a few hundred at 128 K context) are gathered from all
-//             CTAs and cut exactly with integer prefix masses: local 11-bit radix levels on C until
-//             <= 64 remain, then exact ranking.  If the crossing bin holds more than TP_CAND tokens
-//             (heavy ties), it is first narrowed by cluster-wide radix levels on C.
+//   pass 1  : the slice is loaded by cp.async (whole slice in flight) and histogrammed: 2048 bins of width 1/64 in
+//             u = m - score (monotone in C).  Per bin a (count, sum of r) pair, r = 2^(28 - (64u - j) log2(e)/64) in
+//             fixed point, so the bin mass is exp(-j/64) * sum(r): integer sums => order-independent, deterministic.
+//             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin travel
+//             through distributed shared memory (DSMEM is ~20 B/clk per SM).
+//   pass 2  : the tokens of the crossing bin (a few hundred at 128 K context) are gathered from all CTAs in one
+//             DSMEM round; every CTA ranks its share of them against all of them with integer prefix masses
+//             (8 threads per candidate) and the one thread that finds the cut C* writes it into every CTA of the
+//             cluster.  If the crossing bin holds more than TP_CAND tokens (heavy ties), it is first narrowed by
+//             cluster-wide 11-bit radix levels on C.
 //   pass 3  : token t is selected  <=>  C(t) >= C*.  Written as a per-row BITMAP (the representation
 //             the gather attention consumes), the count, and -- only when the caller asks for it --
 //             the ascending index list.
@@ -33,7 +34,6 @@ constexpr int TP_WARPS = TP_THREADS / 32;
 constexpr int TP_NB = 4 * TP_THREADS;          // 2048 bins, 4 per thread in the scans
 constexpr int TP_NC = 64;                      // coarse bins (32 fine bins each)
 constexpr int TP_CAND = 1024;                  // candidates gathered per row
-constexpr int TP_RANK = 64;                    // candidates ranked by direct comparison
 constexpr unsigned FULL = 0xffffffffu;
 typedef unsigned long long u64;
 
@@ -162,8 +162,7 @@ __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
 topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
-  rbq_pdl_trigger();
-  rbq_pdl_wait();                                             // scores and row maxima of S5
+  rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
   uint2* hist = reinterpret_cast<uint2*>(smem_raw + TP_OFF_HIST);
@@ -183,6 +182,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   const size_t rbase = (size_t)row * Lcap;
   uint32_t* bits_row = sel_bits + (size_t)row * wpr;
   if (n <= 0) {                                               // uniform over the cluster: nobody syncs
+    rbq_pdl_wait();
     if (rank == 0 && tid == 0) sel_cnt[row] = 0;
     return;
   }
@@ -191,6 +191,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   const int len = max(0, min(n, lo + S) - lo);
   const int nwords = (len + 31) >> 5;
   if (p_f >= 1.0f) {                                          // R9: everything
+    rbq_pdl_wait();
     for (int w = tid; w < nwords; w += TP_THREADS) {
       const int rem = len - w * 32;
       bits_row[(lo >> 5) + w] = rem >= 32 ? 0xFFFFFFFFu : ((1u << rem) - 1u);
@@ -201,13 +202,14 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   }
   auto csync = [&]() { if (CS == 1) __syncthreads(); else cluster.sync(); };
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
-  const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
 
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
   for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
   if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
   else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
+  rbq_pdl_wait();                                             // scores and row maxima of S5
+  const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
   __syncthreads();
   {
     uint32_t of_c = 0;                                        // overflow bin kept in registers (can be half the row)
