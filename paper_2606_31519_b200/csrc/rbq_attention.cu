@@ -36,7 +36,7 @@ __global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, cons
 
 // ---- plan: union list per KV group ---------------------------------------------------------------------------------
 constexpr int PL_THREADS = 1024;
-constexpr int PL_SPLIT = 8;
+constexpr int PL_SPLIT = 16;
 
 // grid = (PL_SPLIT, B*Hkv).  Every CTA of a group recomputes the prefix over the 128-token blocks (one block per
 // thread: 4 words x G heads), then its warps expand the blocks with blk % PL_SPLIT == blockIdx.x cooperatively
@@ -83,7 +83,7 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
     s_pre[tid] = s_base + wp + si - c;
     s_cntb[tid] = c;
     __syncthreads();
-    // this warp's blocks: lb = blockIdx.x + PL_SPLIT * (warp + 32 i), i < 4.  Lane l < 16 prefetches word (l & 3) of head
+    // this warp's blocks: lb = blockIdx.x + PL_SPLIT * (warp + 32 i), i < PL_BPW.  Lane l < 16 prefetches word (l & 3) of head
     // (l >> 2) of each block first (one round of independent loads), then the words are broadcast by shuffles.
     const unsigned lt = (1u << lane) - 1u;
     constexpr int PL_BPW = PL_THREADS / (PL_SPLIT * (PL_THREADS / 32));          // blocks per warp and iteration (4)
