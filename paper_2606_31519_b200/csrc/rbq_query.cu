@@ -34,6 +34,12 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   __shared__ double s_dred[RBQ_MAX_G][2][4];
   __shared__ uint8_t s_qu[RBQ_MAX_G][RBQ_D];
 
+  if (rot_kind == RBQ_ROT_DENSE) {                 // P -> shared memory, asynchronously; awaited just before the rotation
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_rot);
+    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (uint32_t)i), "l"(rot + 4 * i) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
   const float qv = rbq_ld_elem(q, row * RBQ_D + j);
   const float cqv = c_q ? c_q[row * RBQ_D + j] : 0.0f;
   const float ckv = c_k[(size_t)bg * RBQ_D + j];
@@ -42,12 +48,6 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   s_y[hs][j] = qv;                               // staged for the fp64 dot chains below
   s_cq[hs][j] = cqv;
   if (hs == 0) s_ck[j] = ckv;
-  if (rot_kind == RBQ_ROT_DENSE) {                 // P -> shared memory, asynchronously; awaited just before the rotation
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_rot);
-    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x)
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (uint32_t)i), "l"(rot + 4 * i) : "memory");
-    asm volatile("cp.async.commit_group;" ::: "memory");
-  }
   __syncthreads();
   // ||xq||: the canonical sequential fp32 chain (R1) on one thread per head; the two fp64 dot products
   // <q,c_k>, <c_q,c_k> (exact products, fp64 sums, rounded to fp32 at the end) as a fixed reduction tree.
