@@ -220,9 +220,9 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
   const long long total = s_start[ngroups];
   if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
-    for (int e = tid; e < ngroups * G * RBQ_D; e += GA_THREADS) {
-      const int gq = e / (G * RBQ_D), hd = e % (G * RBQ_D);
-      if (s_start[gq + 1] == s_start[gq]) {
+    for (int gq = 0; gq < ngroups; ++gq) {
+      if (s_start[gq + 1] != s_start[gq]) continue;
+      for (int hd = tid; hd < G * RBQ_D; hd += GA_THREADS) {
         const size_t orow = (size_t)(gq / Hkv) * Hq + (size_t)(gq % Hkv) * G + hd / RBQ_D;
         if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * RBQ_D + hd % RBQ_D] = __float2bfloat16_rn(0.0f);
         else reinterpret_cast<float*>(out)[orow * RBQ_D + hd % RBQ_D] = 0.0f;

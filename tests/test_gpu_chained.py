@@ -243,3 +243,41 @@ def test_full_size_configs(orc, rot128, cfg):
         assert (codes[b, :, :n] == o["codes"][b, :, :n]).all()
         assert (fs[b, :, :n].view(np.uint32) == o["f_scale"][b, :, :n].view(np.uint32)).all()
     c.close()
+
+
+def test_config4_decode_loop_side_stream(orc, rot128):
+    """BASELINE config 4 shape at a reduced context: batch 4, W = 64, 130 decode steps, each appending one token per
+    sequence, the batched encode of every full window running on a side stream while the following decode step runs on
+    the main stream (no host synchronisation between steps except at the checked ones)."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    W, steps = 64, 130
+    w = U.workload(4, L=6000, B=4, extra_cap=192)
+    rot = rot128[0]
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, ROT_DENSE, rot, W)
+    c = U.make_cache(w, rot, flush_tokens=W)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream()
+    pool = synth.query_pool(w, 4)
+    q_dev = [U.to_dev(pool[i], torch.bfloat16) for i in range(4)]
+    out = c.new_out()
+    sel_cnt = c.new_sel()[1]
+    check = {0, W - 2, W - 1, W, W + 1, 2 * W - 1, 2 * W, steps - 1}
+    for s in range(steps):
+        k_new, v_new = synth.append_rows(4, s, w.B, w.Hkv, 1)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16), stream=main, side_stream=side)
+        c.decode_step(q_dev[s % 4], w.p, out, None, sel_cnt)
+        if s in check:
+            torch.cuda.synchronize()
+            assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all() and (c.n_total.cpu().numpy() == lazy.n_total).all()
+            ref = orc.decode_step(pool[s % 4], lazy.K, lazy.V, lazy.codes, lazy.f_scale, None, lazy.c_k, None, lazy.n_indexed,
+                                  lazy.n_total, ROT_DENSE, rot, w.p, U.SM_SCALE)
+            U.assert_attention_close(out.cpu().numpy(), ref["out"], "bf16")
+            assert np.abs(sel_cnt.cpu().numpy().astype(np.int64) - ref["sel_cnt"]).max() <= max(2, int(0.002 * ref["sel_cnt"].max()))
+    torch.cuda.synchronize()
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    for b in range(w.B):
+        n = int(lazy.n_indexed[b]) + lazy.in_flight
+        assert (codes[b, :, :n] == lazy.codes[b, :, :n]).all()
+    c.close()
