@@ -58,19 +58,6 @@ struct GroupLoad {            // what lane (g, t) needs of one 32-token group
   float4 fs;                  // f_scale of tokens 4g .. 4g+3
 };
 
-__device__ __forceinline__ GroupLoad load_group(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
-                                                size_t tok0, int g, int t, int tmax) {
-  // tok0: flat index of the group's first token in [B*Hkv][Lcap]; tmax: tokens of this group that exist in the
-  // allocation (>= 1, multiple of 4 because Lcap is); lanes beyond it load nothing.
-  GroupLoad r;
-  const bool ok = 4 * g < tmax;
-  const uint32_t* p = codes + (tok0 + 4 * g) * RBQ_WORDS + t;
-#pragma unroll
-  for (int k = 0; k < 4; ++k) r.w[k] = ok ? __ldg(p + k * RBQ_WORDS) : 0u;
-  r.fs = ok ? __ldg(reinterpret_cast<const float4*>(f_scale + tok0 + 4 * g)) : make_float4(0.f, 0.f, 0.f, 0.f);
-  return r;
-}
-
 // grid = k * SMs CTAs of EST_WARPS warps.  Flat group index -> (sequence b, KV head, 32-token group).
 template <bool INT_OUT, bool HAS_BIAS>
 __global__ void __launch_bounds__(EST_THREADS, 3)
@@ -114,14 +101,24 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const int g1 = (int)min((long long)gpb, (long long)g0 + (gend - gcur));
     const int bg = b * Hkv + gk;
     const size_t prow = (size_t)bg * Lcap;
+    // lane (g, t): word t of tokens 4g..4g+3 of a group and their factors.  A token run beyond the allocation
+    // (Lcap % 32 != 0) is clamped to its last 4 tokens (never stored); groups beyond the segment are not loaded.
+    const uint32_t* cbase = codes + prow * RBQ_WORDS + t;
+    const float* fbase = f_scale + prow;
+    const int tok_clamp = Lcap - 4;
     auto load_at = [&](int gi) -> GroupLoad {
+      const int tk = min(gi * 32 + 4 * g, tok_clamp);
+      const uint32_t* p = cbase + (size_t)tk * RBQ_WORDS;
       GroupLoad r;
-      r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0u; r.fs = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (gi < g1) r = load_group(codes, f_scale, prow + (size_t)gi * 32, g, t, Lcap - gi * 32);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) r.w[k] = __ldg(p + k * RBQ_WORDS);
+      r.fs = __ldg(reinterpret_cast<const float4*>(fbase + tk));
       return r;
     };
     // three groups of loads in flight per warp; codes and factors do not depend on S3, its constants do
-    GroupLoad l0 = load_at(g0), l1 = load_at(g0 + 1), l2 = load_at(g0 + 2);
+    GroupLoad l0 = load_at(g0), l1 = l0, l2 = l0;
+    if (g0 + 1 < g1) l1 = load_at(g0 + 1);
+    if (g0 + 2 < g1) l2 = load_at(g0 + 2);
     if (first_segment) { rbq_pdl_wait(); first_segment = false; }   // S3's query constants and zeroed row maxima
     const RbqQConst* qc = qconst + bg;
     uint32_t bf[4][2];
@@ -178,11 +175,11 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     };
     for (int gi = g0; gi < g1; gi += 3) {
       process(l0, gi);
-      l0 = load_at(gi + 3);
+      if (gi + 3 < g1) l0 = load_at(gi + 3);
       if (gi + 1 < g1) process(l1, gi + 1);
-      l1 = load_at(gi + 4);
+      if (gi + 4 < g1) l1 = load_at(gi + 4);
       if (gi + 2 < g1) process(l2, gi + 2);
-      l2 = load_at(gi + 5);
+      if (gi + 5 < g1) l2 = load_at(gi + 5);
     }
     if (!INT_OUT) {                                             // row maximum for S6 (keys pre-zeroed by S3)
       smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 4));
