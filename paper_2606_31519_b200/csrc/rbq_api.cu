@@ -108,6 +108,7 @@ int rbq_destroy(rbq_ctx* ctx) {
   if (!ctx) return RBQ_ERR_INVALID_ARG;
   cudaEventDestroy(ctx->ev_copy);
   cudaEventDestroy(ctx->ev_flush);
+  if (ctx->host_graph_state == 1) cudaGraphExecDestroy(ctx->host_graph);
   if (ctx->prof_ev) {
     for (int i = 0; i < RBQ_PROFILE_MAX_STEPS * (RBQ_N_STAGES + 1); ++i) cudaEventDestroy(ctx->prof_ev[i]);
     delete[] ctx->prof_ev;
@@ -298,16 +299,50 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
                          void* out_host, void* stream) {
   RBQ_CTX(ctx);
   RBQ_TRY(need_ws(ctx));
-  if (!q_host || !out_host) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q_host/out_host null");
+  if (!q_host || !out_host || !cache || !idx) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q_host/out_host/cache/idx null");
   cudaStream_t s = (cudaStream_t)stream;
   const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads;
   const size_t qb = rows * RBQ_D * (ctx->cfg.q_dtype == RBQ_BF16 ? 2 : 4);
   const size_t ob = rows * RBQ_D * (ctx->cfg.out_dtype == RBQ_BF16 ? 2 : 4);
   void* dq = ws_ptr<char>(ctx, ctx->off_stage_q);
   void* dout = ws_ptr<char>(ctx, ctx->off_stage_out);
-  RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
-  RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, dout, nullptr, nullptr, stream));
-  RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
+  auto direct = [&]() -> int {
+    RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
+    RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, dout, nullptr, nullptr, stream));
+    RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
+    return RBQ_OK;
+  };
+  // One CPU-side launch per step instead of seven: the sequence is captured once per argument set and replayed.
+  // Not on the legacy default stream (capture is illegal there), not while stage profiling is on (events between kernels).
+  if (ctx->prof_on || ctx->host_graph_state < 0 || s == nullptr || s == cudaStreamLegacy || s == cudaStreamPerThread) return direct();
+  decltype(ctx->host_key) key = {q_host, out_host, cache->k, cache->v, idx->codes, idx->f_scale, idx->f_bias, idx->c_k, idx->c_q,
+                                 idx->n_indexed, idx->n_total, stream, (long long)cache->stride_b, (long long)cache->stride_h,
+                                 (long long)cache->stride_t, p};
+  if (ctx->host_graph_state == 1 && memcmp(&key, &ctx->host_key, sizeof(key)) == 0) {
+    RBQ_CUDA_OK(ctx, cudaGraphLaunch(ctx->host_graph, s));
+    ctx->launches += ctx->host_graph_launches;
+    return RBQ_OK;
+  }
+  if (ctx->host_graph_state == 1) { cudaGraphExecDestroy(ctx->host_graph); ctx->host_graph_state = 0; }
+  RBQ_TRY(direct());                                          // this call runs directly (also sets every function attribute)
+  const long long l0 = ctx->launches;
+  cudaGraph_t g = nullptr;
+  if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); ctx->host_graph_state = -1; return RBQ_OK; }
+  const int rc = direct();
+  const cudaError_t e = cudaStreamEndCapture(s, &g);
+  const int nl = (int)(ctx->launches - l0);
+  ctx->launches = l0;                                         // captured, not launched
+  if (rc != RBQ_OK || e != cudaSuccess || !g || cudaGraphInstantiate(&ctx->host_graph, g, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (g) cudaGraphDestroy(g);
+    ctx->host_graph_state = -1;
+    ctx->err[0] = 0;
+    return RBQ_OK;                                            // the direct launch above already did this step
+  }
+  cudaGraphDestroy(g);
+  ctx->host_key = key;
+  ctx->host_graph_launches = nl;
+  ctx->host_graph_state = 1;
   return RBQ_OK;
 }
 

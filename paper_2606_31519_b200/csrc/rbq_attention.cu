@@ -412,8 +412,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     __syncthreads();
     if (s_last) {
       __threadfence();
-      float* s_f = stg;                                        // [G][GA_THREADS]: m of slot c, then its factor 2^(m - max)
-      float* s_l = stg + RBQ_MAX_G * GA_THREADS;
+      float* s_f = stg;                                        // [G][GA_THREADS]: factor 2^(m - max) of slot c
       float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [128] second half's partial sums
       const int clo = s_clo, chi = s_chi;
       // thread tid owns slot tid: per-head maximum and normaliser by block reductions (warp shuffles + one shared round)

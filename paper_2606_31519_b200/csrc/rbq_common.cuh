@@ -49,6 +49,12 @@ struct rbq_ctx {
   int prof_on, prof_steps;                                   // stage timing (rbq_profile_*)
   cudaEvent_t* stage_ev;                                     // events of the step being enqueued, or NULL
   cudaEvent_t* prof_ev;                                      // [RBQ_PROFILE_MAX_STEPS][RBQ_N_STAGES + 1], lazily created
+  // rbq_decode_step_host: the copies and the five launches replayed as one CUDA graph while the arguments stay the same
+  cudaGraphExec_t host_graph;
+  int host_graph_state;      // 0 = none yet, 1 = valid, -1 = capture not possible on this stream / driver: direct launches
+  int host_graph_launches;   // kernel launches one replay stands for
+  struct { const void *q, *out, *k, *v, *codes, *f_scale, *f_bias, *c_k, *c_q, *n_indexed, *n_total, *stream;
+           long long sb, sh, st; float p; } host_key;
   char err[256];
 };
 

@@ -42,8 +42,6 @@ struct TpSmall {
   uint32_t wt_c[TP_WARPS];
   u64 red_lo[TP_WARPS], red_hi[TP_WARPS];
   double tabA[TP_NC], tabB[32];                // exp(-k/2), exp(-i/64)
-  double tot_mass[TP_NC];
-  uint32_t tot_cnt[TP_NC];
   // results broadcast inside the CTA
   double trem;            // mass still needed inside the candidate range, in units of 2^-28 * exp(-bx/64)
   u64 lo64, hi64;         // candidate range on C

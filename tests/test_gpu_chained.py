@@ -178,6 +178,17 @@ def test_decode_step_host_buffers(orc, rot128):
     q_host = torch.from_numpy(w.q).to(torch.bfloat16).pin_memory()
     out_host = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32).pin_memory()
     c.decode_step_host(q_host, 0.9, out_host)
+    torch.cuda.synchronize()
+    # on a non-default stream the host step is captured once and replayed as a CUDA graph: same bits every time
+    side = torch.cuda.Stream()
+    outs = []
+    for _ in range(4):
+        o2 = torch.zeros_like(out_host).pin_memory()
+        c.decode_step_host(q_host, 0.9, out_host if _ else o2, stream=side)
+        side.synchronize()
+        outs.append((out_host if _ else o2).clone())
+    for o2 in outs[1:]:
+        assert (o2.numpy().view(np.uint32) == outs[0].numpy().view(np.uint32)).all(), "graph replay differs from the direct host step"
     out = c.new_out()
     c.decode_step(q_host.cuda(), 0.9, out)
     torch.cuda.synchronize()
