@@ -22,17 +22,59 @@ constexpr int XS = RBQ_D + 1;      // padded row stride of the x / y tile (bank-
 // correctly rounded mean irrespective of the order.
 constexpr int CEN_SPLIT = 64;
 
+// 8 consecutive elements of a row as floats (16-byte loads for bf16, 2 x 16 bytes for fp32)
+__device__ __forceinline__ void rbq_ld8(const __nv_bfloat16* p, float (&v)[8]) {
+  const uint4 u = __ldg(reinterpret_cast<const uint4*>(p));
+  v[0] = rbq_bf16lo(u.x); v[1] = rbq_bf16hi(u.x); v[2] = rbq_bf16lo(u.y); v[3] = rbq_bf16hi(u.y);
+  v[4] = rbq_bf16lo(u.z); v[5] = rbq_bf16hi(u.z); v[6] = rbq_bf16lo(u.w); v[7] = rbq_bf16hi(u.w);
+}
+__device__ __forceinline__ void rbq_ld8(const float* p, float (&v)[8]) {
+  const float4 a = __ldg(reinterpret_cast<const float4*>(p)), b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+  v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+
+// grid = (B*Hkv, CEN_SPLIT), 256 threads: 16 threads per row (8 dims each), 16 rows per round, 4 rounds in flight.
+constexpr int CEN_THREADS = 256;
+
 template <typename T>
-__global__ void centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
-                                        const int32_t* __restrict__ seq_lens, int Hkv, double* __restrict__ part) {
-  const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv, s = blockIdx.y, d = threadIdx.x;
+__global__ void __launch_bounds__(CEN_THREADS)
+centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
+                        const int32_t* __restrict__ seq_lens, int Hkv, double* __restrict__ part) {
+  __shared__ double s_acc[CEN_THREADS / 16][RBQ_D];
+  const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv, s = blockIdx.y;
+  const int c8 = (threadIdx.x & 15) * 8, r = threadIdx.x >> 4;
   const int n = seq_lens[b];
   const int per = (n + CEN_SPLIT - 1) / CEN_SPLIT;
   const int t0 = s * per, t1 = min(n, t0 + per);
-  const T* base = K + (long long)b * sb + (long long)g * sh;
-  double acc = 0.0;
-  for (int t = t0; t < t1; ++t) acc += (double)rbq_ld_elem(base, (long long)t * st + d);
-  part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + d] = acc;
+  const T* base = K + (long long)b * sb + (long long)g * sh + c8;
+  double acc[8];
+#pragma unroll
+  for (int d = 0; d < 8; ++d) acc[d] = 0.0;
+  for (int t = t0 + r; t < t1; t += 4 * (CEN_THREADS / 16)) {
+    float v[4][8];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int tt = t + u * (CEN_THREADS / 16);
+      if (tt < t1) rbq_ld8(base + (long long)tt * st, v[u]);
+      else {
+#pragma unroll
+        for (int d = 0; d < 8; ++d) v[u][d] = 0.0f;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int d = 0; d < 8; ++d) acc[d] += (double)v[u][d];
+  }
+#pragma unroll
+  for (int d = 0; d < 8; ++d) s_acc[r][c8 + d] = acc[d];
+  __syncthreads();
+  if (threadIdx.x < RBQ_D) {
+    double a = 0.0;
+#pragma unroll
+    for (int k = 0; k < CEN_THREADS / 16; ++k) a += s_acc[k][threadIdx.x];
+    part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + threadIdx.x] = a;
+  }
 }
 
 __global__ void centroid_final_kernel(const double* __restrict__ part, const int32_t* __restrict__ seq_lens,
@@ -69,11 +111,15 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
   const float* ck = c_k + (size_t)bg * RBQ_D;
 
   // x = fl32(k) - c_k
-  for (int e = tid; e < ENC_TOK * RBQ_D; e += ENC_THREADS) {
-    const int r = e >> 7, d = e & 127;
-    float x = 0.0f;
-    if (r < ntok) x = __fsub_rn(rbq_ld_elem(base, (long long)r * st + d), ck[d]);
-    xs[r * XS + d] = x;
+  // 16-byte loads; a warp covers 8 rows x 4 chunks of 8 elements so that its shared-memory stores are conflict-free
+  // with the padded row stride (bank = row + 8 * chunk + k)
+  for (int e = tid; e < ENC_TOK * RBQ_D / 8; e += ENC_THREADS) {
+    const int wv = e >> 5, ln = e & 31;
+    const int r = (wv >> 2) * 8 + (ln >> 2), d = ((wv & 3) * 4 + (ln & 3)) * 8;
+    float v[8];
+    if (r < ntok) rbq_ld8(base + (long long)r * st + d, v);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) xs[r * XS + d + k] = (r < ntok) ? __fsub_rn(v[k], ck[d + k]) : 0.0f;
   }
   if (ROT == RBQ_ROT_DENSE) {
     for (int e = tid; e < RBQ_D * RBQ_D / 4; e += ENC_THREADS)
@@ -134,13 +180,15 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
       a = __fadd_rn(u1, u3); c = __fsub_rn(u1, u3); u1 = a; u3 = c;
 #pragma unroll
       for (int m = 1; m < 32; m <<= 1) {                                      // h = 4*m
-        const bool up = (lane & m) != 0;
+        // (a, b) -> (a + b, a - b): the upper lane computes p - u, the lower one u + p; both are fmaf(u, +-1, p),
+        // bit-identical to the add / subtract (the product with +-1 is exact, one rounding)
+        const float sg = (lane & m) ? -1.0f : 1.0f;
         float p0 = __shfl_xor_sync(0xffffffffu, u0, m), p1 = __shfl_xor_sync(0xffffffffu, u1, m);
         float p2 = __shfl_xor_sync(0xffffffffu, u2, m), p3 = __shfl_xor_sync(0xffffffffu, u3, m);
-        u0 = up ? __fsub_rn(p0, u0) : __fadd_rn(u0, p0);
-        u1 = up ? __fsub_rn(p1, u1) : __fadd_rn(u1, p1);
-        u2 = up ? __fsub_rn(p2, u2) : __fadd_rn(u2, p2);
-        u3 = up ? __fsub_rn(p3, u3) : __fadd_rn(u3, p3);
+        u0 = fmaf(u0, sg, p0);
+        u1 = fmaf(u1, sg, p1);
+        u2 = fmaf(u2, sg, p2);
+        u3 = fmaf(u3, sg, p3);
       }
       __syncwarp();
       xr[0] = u0; xr[1] = u1; xr[2] = u2; xr[3] = u3;                         // unscaled u
@@ -225,10 +273,10 @@ int rbq_launch_centroid(rbq_ctx* ctx, const RbqKV& kv, const int32_t* seq_lens, 
   double* part = reinterpret_cast<double*>(static_cast<char*>(ctx->ws) + ctx->off_centroid);
   dim3 grid(BG, CEN_SPLIT);
   if (ctx->cfg.kv_dtype == RBQ_BF16)
-    centroid_partial_kernel<<<grid, RBQ_D, 0, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
+    centroid_partial_kernel<<<grid, CEN_THREADS, 0, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
                                                     ctx->cfg.n_kv_heads, part);
   else
-    centroid_partial_kernel<<<grid, RBQ_D, 0, s>>>((const float*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
+    centroid_partial_kernel<<<grid, CEN_THREADS, 0, s>>>((const float*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
                                                     ctx->cfg.n_kv_heads, part);
   RBQ_LAUNCH_OK(ctx);
   centroid_final_kernel<<<BG, RBQ_D, 0, s>>>(part, seq_lens, ctx->cfg.n_kv_heads, c_k);
