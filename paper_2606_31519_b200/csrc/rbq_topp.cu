@@ -9,8 +9,8 @@
 // on the composite key  C(t) = (orderkey(score_t) << 32) | ~t  whose values are all distinct.
 // The row maximum m comes with the scores (S5 epilogue, or rowmax_kernel for caller-provided scores):
 //   pass 1  : the slice is loaded by cp.async (whole slice in flight) and histogrammed: 2048 bins of width 1/64 in
-//             u = m - score (monotone in C).  Per bin a (count, sum of r) pair, r = 2^(28 - (64u - j) log2(e)/64) in
-//             fixed point, so the bin mass is exp(-j/64) * sum(r): integer sums => order-independent, deterministic.
+//             u = m - score (monotone in C).  Per bin a (count, sum of r) pair, r = 2^(22 - (64u - j) log2(e)/64) in
+//             2^-22 fixed point, so the bin mass is exp(-j/64) * sum(r): integer sums => order-independent, deterministic.
 //             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin travel
 //             through distributed shared memory (DSMEM is ~20 B/clk per SM).
 //   pass 2  : the tokens of the crossing bin (a few hundred at 128 K context) are gathered from all CTAs in one
@@ -43,7 +43,7 @@ struct TpSmall {
   u64 red_lo[TP_WARPS], red_hi[TP_WARPS];
   double tabA[TP_NC], tabB[32];                // exp(-k/2), exp(-i/64)
   // results broadcast inside the CTA
-  double trem;            // mass still needed inside the candidate range, in units of 2^-28 * exp(-bx/64)
+  double trem;            // mass still needed inside the candidate range, in units of 2^-22 * exp(-bx/64)
   u64 lo64, hi64;         // candidate range on C
   u64 cstar;
   uint32_t bx, cntx, cnt_above, found, ksel;
@@ -65,22 +65,27 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^28 = 2^(28 - (64u - j) log2(e)/64)
+// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^22 = 2^(22 - (64u - j) log2(e)/64).
+// The XU pipe (conversions, MUFU) is the scarce unit of the histogram pass, so floor() and both float <-> int conversions
+// are done with the 2^23 magic-number add on the FMA pipe (round-down for the floor); only ex2 remains on the XU pipe.
+// 2^-22 is the resolution of ex2.approx itself.
 __device__ __forceinline__ void bin0(float m, float s, int& j, uint32_t& rfix) {
-  const float t = __fmul_rn(__fsub_rn(m, s), 64.0f);
-  j = min(TP_NB - 1, __float2int_rz(t));
-  const float f = __fsub_rn(t, (float)j);                     // exact for j < TP_NB - 1; large in the overflow bin
-  rfix = __float2uint_rn(ex2_approx(fmaf(f, -0.022542110013890053f, 28.0f)));
+  const float t = __fmul_rn(__fsub_rn(m, s), 64.0f);          // >= 0
+  const float jm = __fadd_rd(fminf(t, (float)(TP_NB - 1)), 8388608.0f);   // 2^23 + min(floor(t), TP_NB - 1), exact
+  j = __float_as_int(jm) - 0x4B000000;
+  const float f = __fsub_rn(t, __fsub_rn(jm, 8388608.0f));    // exact for j < TP_NB - 1; large in the overflow bin
+  rfix = __float_as_uint(__fadd_rn(ex2_approx(fmaf(f, -0.022542110013890053f, 22.0f)), 8388608.0f)) - 0x4B000000u;
 }
 __device__ __forceinline__ u64 composite(float s, int t) {
   return ((u64)rbq_fkey(s) << 32) | (u64)(~(uint32_t)t);
 }
-// hist[j] += (count c, mass v): .x = low 32 bits of the mass, .y = (count << 12) | (mass >> 32)
-__device__ __forceinline__ void hist_add(uint2* hist, int j, u64 v, uint32_t c) {
+// Histogram = two u32 arrays (all 32 banks in use): hist[j] = low 32 bits of the mass, hist[TP_NB + j] = (count << 12) |
+// (mass >> 32).  hist[j] += (count c, mass v):
+__device__ __forceinline__ void hist_add(uint32_t* hist, int j, u64 v, uint32_t c) {
   const uint32_t lo = (uint32_t)v;
-  const uint32_t old = atomicAdd(&hist[j].x, lo);
+  const uint32_t old = atomicAdd(&hist[j], lo);
   const uint32_t carry = (old + lo < old) ? 1u : 0u;
-  atomicAdd(&hist[j].y, (c << 12) + (uint32_t)(v >> 32) + carry);
+  atomicAdd(&hist[TP_NB + j], (c << 12) + (uint32_t)(v >> 32) + carry);
 }
 __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
   cnt = v.y >> 12;
@@ -89,18 +94,18 @@ __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
 
 // totals of this thread's 4 bins over the CS histograms of the cluster (cluster-wide radix levels only)
 template <int CS>
-__device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint2* hist, int tid, uint32_t (&cnt)[4], u64 (&R)[4]) {
+__device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint32_t* hist, int tid, uint32_t (&cnt)[4], u64 (&R)[4]) {
 #pragma unroll
   for (int k = 0; k < 4; ++k) { cnt[k] = 0; R[k] = 0; }
 #pragma unroll
   for (int r = 0; r < CS; ++r) {
-    const uint4* rh = reinterpret_cast<const uint4*>(CS == 1 ? hist : cluster.map_shared_rank(hist, r)) + tid * 2;
-    const uint4 a = rh[0], b = rh[1];
+    const uint32_t* rh = CS == 1 ? hist : cluster.map_shared_rank(hist, r);
+    const uint4 a = reinterpret_cast<const uint4*>(rh)[tid], b = reinterpret_cast<const uint4*>(rh + TP_NB)[tid];
     uint32_t c; u64 v;
-    unpack_bin(make_uint2(a.x, a.y), c, v); cnt[0] += c; R[0] += v;
-    unpack_bin(make_uint2(a.z, a.w), c, v); cnt[1] += c; R[1] += v;
-    unpack_bin(make_uint2(b.x, b.y), c, v); cnt[2] += c; R[2] += v;
-    unpack_bin(make_uint2(b.z, b.w), c, v); cnt[3] += c; R[3] += v;
+    unpack_bin(make_uint2(a.x, b.x), c, v); cnt[0] += c; R[0] += v;
+    unpack_bin(make_uint2(a.y, b.y), c, v); cnt[1] += c; R[1] += v;
+    unpack_bin(make_uint2(a.z, b.z), c, v); cnt[2] += c; R[2] += v;
+    unpack_bin(make_uint2(a.w, b.w), c, v); cnt[3] += c; R[3] += v;
   }
 }
 
@@ -154,7 +159,7 @@ __device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4]
 }
 
 // grid = (CS, rows); cluster = CS CTAs along x.
-// smem: TpSmall | hist uint2[TP_NB] (later: selection words) | cand_all | cand_loc | scores slice [s_cap]
+// smem: TpSmall | hist u32[2][TP_NB] (later: selection words) | cand_all | cand_loc | scores slice [s_cap]
 template <int CS>
 __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
 topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
@@ -163,7 +168,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
-  uint2* hist = reinterpret_cast<uint2*>(smem_raw + TP_OFF_HIST);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);
   uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);          // aliases hist once the cut is known
   u64* all_comp = reinterpret_cast<u64*>(smem_raw + TP_OFF_A);
   uint32_t* all_rfix = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A + TP_CAND * 8);
@@ -202,7 +207,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
 
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
-  for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
+  for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
   if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
   else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
@@ -267,7 +272,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       uint32_t c; u64 R;
-      unpack_bin(hist[4 * tid + k], c, R);
+      unpack_bin(make_uint2(hist[4 * tid + k], hist[TP_NB + 4 * tid + k]), c, R);
       ms += (double)R * sh.tabB[(4 * tid + k) & 31];
       cs += c;
     }
@@ -319,9 +324,9 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     u64 R = 0;
 #pragma unroll
     for (int r = 0; r < CS; ++r) {
-      const uint2* rh = CS == 1 ? hist : cluster.map_shared_rank(hist, r);
+      const uint32_t* rh = CS == 1 ? hist : cluster.map_shared_rank(hist, r);
       uint32_t cc; u64 rr;
-      unpack_bin(rh[32 * kx + lane], cc, rr);
+      unpack_bin(make_uint2(rh[32 * kx + lane], rh[TP_NB + 32 * kx + lane]), cc, rr);
       c += cc; R += rr;
     }
     const double e = sh.tabA[kx] * sh.tabB[lane];
@@ -377,7 +382,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     while (cntx > TP_CAND) {
       const u64 range = hi64 - lo64;
       const int shift = max(0, (64 - __clzll((long long)range)) - 11);
-      for (int i = tid; i < TP_NB; i += TP_THREADS) hist[i] = make_uint2(0u, 0u);
+      for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
       __syncthreads();
       for (int base = warp * 32; base < len; base += TP_THREADS) {
         const int i = base + lane;
