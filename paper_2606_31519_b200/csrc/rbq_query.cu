@@ -31,18 +31,21 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   __shared__ int s_isum[RBQ_MAX_G][4];
   __shared__ float s_qn[RBQ_MAX_G];
   __shared__ double s_dot[RBQ_MAX_G][2];
+  __shared__ __align__(8) unsigned long long s_bar;
   __shared__ double s_dred[RBQ_MAX_G][2][4];
   __shared__ uint8_t s_qu[RBQ_MAX_G][RBQ_D];
 
-  if (rot_kind == RBQ_ROT_DENSE) {                 // P -> shared memory, asynchronously; awaited just before the rotation
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_rot);
-    for (int i = threadIdx.x; i < RBQ_D * RBQ_D / 4; i += blockDim.x)
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (uint32_t)i), "l"(rot + 4 * i) : "memory");
-    asm volatile("cp.async.commit_group;" ::: "memory");
-  }
   const float qv = rbq_ld_elem(q, row * RBQ_D + j);
   const float cqv = c_q ? c_q[row * RBQ_D + j] : 0.0f;
   const float ckv = c_k[(size_t)bg * RBQ_D + j];
+  if (rot_kind == RBQ_ROT_DENSE && threadIdx.x == 0) {   // P -> shared memory by ONE bulk copy (TMA); awaited just before the rotation
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)(RBQ_D * RBQ_D * 4)) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     (uint32_t)__cvta_generic_to_shared(s_rot)), "l"(rot), "r"((uint32_t)(RBQ_D * RBQ_D * 4)), "r"(bar) : "memory");
+  }
   const float xq = c_q ? __fsub_rn(qv, cqv) : qv;
   s_x[hs][j] = xq;
   s_y[hs][j] = qv;                               // staged for the fp64 dot chains below
@@ -85,34 +88,45 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   const float qn = s_qn[hs];
   const float u = (qn > 0.0f) ? __fdiv_rn(xq, qn) : 0.0f;
   s_x[hs][j] = u;
-  asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
+  if (rot_kind == RBQ_ROT_DENSE) {                 // P has landed (the barrier above also made the mbarrier init visible)
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n"
+        "@p bra LAB_DONE_%=;\n"
+        "bra LAB_WAIT_%=;\n"
+        "LAB_DONE_%=:\n"
+        "}\n" ::"r"(bar) : "memory");
+  }
 
   float qp;
   if (rot_kind == RBQ_ROT_DENSE) {
-    // Threads 0..127 own one output column each for ALL heads of the group: one shared-memory read of P[i][j] feeds G
-    // independent canonical chains (reading P once per head instead would be bound by shared-memory bandwidth).
-    if (threadIdx.x < RBQ_D) {
-      const int jj = threadIdx.x;
-      float acc[RBQ_MAX_G];
-#pragma unroll
-      for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) acc[h2] = 0.0f;
-#pragma unroll 1
+    // Threads 0..255: one output column for TWO heads of the group each: one shared-memory read of P[i][j] feeds two
+    // independent canonical chains (one read per head would be bound by shared-memory bandwidth, one read for all
+    // four heads by the FMA issue rate of four warps).
+    if (threadIdx.x < 2 * RBQ_D) {
+      const int jj = threadIdx.x & (RBQ_D - 1), hp = (threadIdx.x >> 7) * 2;
+      float a0 = 0.0f, a1 = 0.0f;
+#pragma unroll 2
       for (int i0 = 0; i0 < RBQ_D; i0 += 8) {
         float rv[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) rv[k] = s_rot[(i0 + k) * RBQ_D + jj];
-#pragma unroll
-        for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) {
-          const float4 xa = *reinterpret_cast<const float4*>(&s_x[h2][i0]), xb = *reinterpret_cast<const float4*>(&s_x[h2][i0 + 4]);
-          float a = acc[h2];
-          a = fmaf(xa.x, rv[0], a); a = fmaf(xa.y, rv[1], a); a = fmaf(xa.z, rv[2], a); a = fmaf(xa.w, rv[3], a);
-          a = fmaf(xb.x, rv[4], a); a = fmaf(xb.y, rv[5], a); a = fmaf(xb.z, rv[6], a); a = fmaf(xb.w, rv[7], a);
-          acc[h2] = a;
-        }
+        const float4 xa = *reinterpret_cast<const float4*>(&s_x[hp][i0]), xb = *reinterpret_cast<const float4*>(&s_x[hp][i0 + 4]);
+        const float4 ya = *reinterpret_cast<const float4*>(&s_x[hp + 1][i0]), yb = *reinterpret_cast<const float4*>(&s_x[hp + 1][i0 + 4]);
+        a0 = fmaf(xa.x, rv[0], a0); a1 = fmaf(ya.x, rv[0], a1);
+        a0 = fmaf(xa.y, rv[1], a0); a1 = fmaf(ya.y, rv[1], a1);
+        a0 = fmaf(xa.z, rv[2], a0); a1 = fmaf(ya.z, rv[2], a1);
+        a0 = fmaf(xa.w, rv[3], a0); a1 = fmaf(ya.w, rv[3], a1);
+        a0 = fmaf(xb.x, rv[4], a0); a1 = fmaf(yb.x, rv[4], a1);
+        a0 = fmaf(xb.y, rv[5], a0); a1 = fmaf(yb.y, rv[5], a1);
+        a0 = fmaf(xb.z, rv[6], a0); a1 = fmaf(yb.z, rv[6], a1);
+        a0 = fmaf(xb.w, rv[7], a0); a1 = fmaf(yb.w, rv[7], a1);
       }
-#pragma unroll
-      for (int h2 = 0; h2 < RBQ_MAX_G; ++h2) s_y[h2][jj] = acc[h2];
+      s_y[hp][jj] = a0; s_y[hp + 1][jj] = a1;
     }
     __syncthreads();
     qp = s_y[hs][j];
