@@ -48,8 +48,8 @@ typedef enum { RBQ_F32 = 0, RBQ_BF16 = 1 } rbq_dtype;
 typedef enum { RBQ_ROT_DENSE = 0, RBQ_ROT_WH = 1 } rbq_rot_kind;
 /* EXACT: canonical fp32 order (R1) -> codes/factors bit-identical to the oracle.
  * FAST : tensor-core rotation (bf16 hi/lo split, fp32 accumulate); codes may differ only where
- *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  NOT BUILT YET: rbq_create returns
- *        RBQ_ERR_UNSUPPORTED for it. */
+ *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  Built for bf16 K/V with the dense
+ *        rotation; other combinations: rbq_create returns RBQ_ERR_UNSUPPORTED. */
 typedef enum { RBQ_ENC_EXACT = 0, RBQ_ENC_FAST = 1 } rbq_enc_mode;
 
 /* flags of rbq_encode_keys */

@@ -122,6 +122,8 @@ inline cudaError_t rbq_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block,
 int rbq_launch_centroid(rbq_ctx*, const RbqKV&, const int32_t* seq_lens, float* c_k, cudaStream_t);
 int rbq_launch_encode(rbq_ctx*, const RbqKV&, const int32_t* t_begin, const int32_t* t_count_or_null,
                       int fixed_count, int max_count, const rbq_index*, cudaStream_t);
+int rbq_launch_encode_fast(rbq_ctx*, const RbqKV&, const int32_t* t_begin, const int32_t* t_count_or_null,
+                           int fixed_count, int max_count, const rbq_index*, cudaStream_t);   // RBQ_ENC_FAST, bf16 K, dense P
 int rbq_launch_set_counts(rbq_ctx*, const int32_t* seq_lens, int32_t* n_indexed, int32_t* n_total,
                           cudaStream_t);
 int rbq_launch_append_copy(rbq_ctx*, const void* k_new, const void* v_new, int n_new, const RbqKV&,

@@ -313,6 +313,7 @@ int rbq_launch_encode(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, con
                       int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
   if (max_count <= 0) return RBQ_OK;
   const bool bf = ctx->cfg.kv_dtype == RBQ_BF16, wh = ctx->cfg.rot_kind == RBQ_ROT_WH;
+  if (ctx->cfg.enc_mode == RBQ_ENC_FAST) return rbq_launch_encode_fast(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
   if (bf && !wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
   if (bf && wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
   if (!bf && !wh) return launch_encode_t<float, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);

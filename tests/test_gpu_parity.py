@@ -93,6 +93,42 @@ def test_encode_ck_given_and_zero_key(orc, rot128):
     c.close()
 
 
+@pytest.mark.parametrize("name", ["cfg1_small", "cfg3_small"])
+def test_encode_fast_guard_band(orc, rot128, name):
+    """RBQ_ENC_FAST (tensor-core rotation, bf16 hi/lo split): a code bit may differ from the oracle's only where the
+    fp64 rotated coordinate satisfies |y_j| <= 1e-5 ||x|| (expected fraction ~9e-5, fail above 3e-4); f_scale within
+    1e-5 relative."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb
+    w = get_case(name)
+    rot = rot128[0]
+    o = U.oracle_index(orc, w, rot, ROT_DENSE)
+    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(rot), enc_mode=rb.RBQ_ENC_FAST)
+    c.K.copy_(U.to_dev(w.K, torch.bfloat16))
+    c.encode_keys(U.to_dev(w.seq_lens))
+    torch.cuda.synchronize()
+    assert np.array_equal(c.c_k.cpu().numpy().view(np.uint32), o["c_k"].view(np.uint32))
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    P = rot.astype(np.float64)
+    n_bits = n_diff = 0
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        for g in range(w.Hkv):
+            x = w.K[b, g, :n].astype(np.float64) - o["c_k"][b, g].astype(np.float64)
+            y = x @ P
+            xn = np.linalg.norm(x, axis=1, keepdims=True)
+            diff = codes[b, g, :n] ^ o["codes"][b, g, :n]                       # [n, 4] words
+            bits = ((diff[:, :, None] >> np.arange(32, dtype=np.uint32)) & 1).reshape(n, 128).astype(bool)
+            assert (np.abs(y)[bits] <= 1e-5 * np.broadcast_to(xn, y.shape)[bits]).all(), "code bit differs outside the guard band"
+            n_bits += bits.size
+            n_diff += int(bits.sum())
+            ref = o["f_scale"][b, g, :n].astype(np.float64)
+            assert (np.abs(fs[b, g, :n] - ref) <= 1e-5 * np.abs(ref)).all(), "f_scale outside 1e-5 relative"
+    assert n_diff <= 3e-4 * n_bits, f"{n_diff} of {n_bits} bits differ"
+    c.close()
+
+
 # ---- S3: query prep + INT4 quantisation -------------------------------------------------------------------
 @pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
 @pytest.mark.parametrize("name", ["cfg0", "cfg0_cq", "cfg1_small", "cfg3_small"])
