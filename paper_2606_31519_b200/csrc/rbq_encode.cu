@@ -33,11 +33,28 @@ __device__ __forceinline__ void rbq_ld8(const float* p, float (&v)[8]) {
   v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
 }
 
-// grid = (B*Hkv, CEN_SPLIT), 256 threads: 16 threads per row (8 dims each), 16 rows per round, 4 rounds in flight.
+// raw 8-element pieces (kept unconverted while in flight: 4 registers for bf16, 8 for fp32)
+struct RbqRaw8F { float4 a, b; };
+__device__ __forceinline__ uint4 rbq_ldraw8(const __nv_bfloat16* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ RbqRaw8F rbq_ldraw8(const float* p) {
+  return {__ldg(reinterpret_cast<const float4*>(p)), __ldg(reinterpret_cast<const float4*>(p) + 1)};
+}
+__device__ __forceinline__ uint4 rbq_zero_raw(const __nv_bfloat16*) { return make_uint4(0u, 0u, 0u, 0u); }
+__device__ __forceinline__ RbqRaw8F rbq_zero_raw(const float*) { return {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)}; }
+__device__ __forceinline__ void rbq_raw_to_f(const uint4& u, float (&v)[8]) {
+  v[0] = rbq_bf16lo(u.x); v[1] = rbq_bf16hi(u.x); v[2] = rbq_bf16lo(u.y); v[3] = rbq_bf16hi(u.y);
+  v[4] = rbq_bf16lo(u.z); v[5] = rbq_bf16hi(u.z); v[6] = rbq_bf16lo(u.w); v[7] = rbq_bf16hi(u.w);
+}
+__device__ __forceinline__ void rbq_raw_to_f(const RbqRaw8F& u, float (&v)[8]) {
+  v[0] = u.a.x; v[1] = u.a.y; v[2] = u.a.z; v[3] = u.a.w; v[4] = u.b.x; v[5] = u.b.y; v[6] = u.b.z; v[7] = u.b.w;
+}
+
+// grid = (B*Hkv, CEN_SPLIT), 256 threads: 16 threads per row (8 dims each), 16 rows per round, CEN_FLIGHT rounds (raw
+// 16-byte pieces) in flight per thread; 4 CTAs per SM keep ~19 MB in flight over the chip.
 constexpr int CEN_THREADS = 256;
 
 template <typename T>
-__global__ void __launch_bounds__(CEN_THREADS)
+__global__ void __launch_bounds__(CEN_THREADS, 4)
 centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
                         const int32_t* __restrict__ seq_lens, int Hkv, double* __restrict__ part) {
   __shared__ double s_acc[CEN_THREADS / 16][RBQ_D];
@@ -47,24 +64,24 @@ centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, lon
   const int per = (n + CEN_SPLIT - 1) / CEN_SPLIT;
   const int t0 = s * per, t1 = min(n, t0 + per);
   const T* base = K + (long long)b * sb + (long long)g * sh + c8;
+  constexpr int CEN_FLIGHT = sizeof(T) == 2 ? 8 : 2;          // 32 / 16 registers of raw data in flight
   double acc[8];
 #pragma unroll
   for (int d = 0; d < 8; ++d) acc[d] = 0.0;
-  for (int t = t0 + r; t < t1; t += 4 * (CEN_THREADS / 16)) {
-    float v[4][8];
+  for (int t = t0 + r; t < t1; t += CEN_FLIGHT * (CEN_THREADS / 16)) {
+    decltype(rbq_ldraw8(base)) raw[CEN_FLIGHT];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < CEN_FLIGHT; ++u) {
       const int tt = t + u * (CEN_THREADS / 16);
-      if (tt < t1) rbq_ld8(base + (long long)tt * st, v[u]);
-      else {
-#pragma unroll
-        for (int d = 0; d < 8; ++d) v[u][d] = 0.0f;
-      }
+      raw[u] = (tt < t1) ? rbq_ldraw8(base + (long long)tt * st) : rbq_zero_raw(base);
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int u = 0; u < CEN_FLIGHT; ++u) {
+      float v[8];
+      rbq_raw_to_f(raw[u], v);
 #pragma unroll
-      for (int d = 0; d < 8; ++d) acc[d] += (double)v[u][d];
+      for (int d = 0; d < 8; ++d) acc[d] += (double)v[d];
+    }
   }
 #pragma unroll
   for (int d = 0; d < 8; ++d) s_acc[r][c8 + d] = acc[d];
