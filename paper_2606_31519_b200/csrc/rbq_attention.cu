@@ -36,11 +36,13 @@ __global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, cons
 
 // ---- plan: union list per KV group ---------------------------------------------------------------------------------
 constexpr int PL_THREADS = 1024;
-constexpr int PL_SPLIT = 16;
+constexpr int PL_MAX_SPLIT = 16;
 
-// grid = (PL_SPLIT, B*Hkv).  Every CTA of a group recomputes the prefix over the 128-token blocks (one block per
+// grid = (PL_SPLIT, B*Hkv); PL_SPLIT = the largest of 16, 8, 4, 2, 1 that keeps the grid within one wave (2 CTAs per
+// SM).  Every CTA of a group recomputes the prefix over the 128-token blocks (one block per
 // thread: 4 words x G heads), then its warps expand the blocks with blk % PL_SPLIT == blockIdx.x cooperatively
 // (lane = token bit of a word, position by popcount prefix).
+template <int PL_SPLIT>
 __global__ void __launch_bounds__(PL_THREADS)
 attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total,
                  int Hq, int Hkv, int Lcap, int wpr, uint32_t* __restrict__ ulist, int32_t* __restrict__ ucount,
@@ -86,7 +88,7 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
     // this warp's blocks: lb = blockIdx.x + PL_SPLIT * (warp + 32 i), i < PL_BPW.  Lane l < 16 prefetches word (l & 3) of head
     // (l >> 2) of each block first (one round of independent loads), then the words are broadcast by shuffles.
     const unsigned lt = (1u << lane) - 1u;
-    constexpr int PL_BPW = PL_THREADS / (PL_SPLIT * (PL_THREADS / 32));          // blocks per warp and iteration (4)
+    constexpr int PL_BPW = PL_THREADS / (PL_SPLIT * (PL_THREADS / 32));          // blocks per warp and iteration
     uint32_t pre[PL_BPW];
 #pragma unroll
     for (int i = 0; i < PL_BPW; ++i) {
@@ -710,9 +712,20 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   int32_t* ucount = reinterpret_cast<int32_t*>(ws + ctx->off_ucount);
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
   int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
-  RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_plan_kernel, dim3(PL_SPLIT, groups), dim3(PL_THREADS), 0, s, bits,
-                                  (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, ctx->cfg.n_q_heads,
-                                  ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount, gdone));
+  int split = PL_MAX_SPLIT;
+  while (split > 1 && (long long)groups * split > 2ll * ctx->sm_count) split >>= 1;
+#define RBQ_PLAN_LAUNCH(SP)                                                                                          \
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_plan_kernel<SP>, dim3(SP, groups), dim3(PL_THREADS), 0, s, bits,                \
+                                  (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, ctx->cfg.n_q_heads,   \
+                                  ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, wpr, ulist, ucount, gdone))
+  switch (split) {
+    case 16: RBQ_PLAN_LAUNCH(16); break;
+    case 8: RBQ_PLAN_LAUNCH(8); break;
+    case 4: RBQ_PLAN_LAUNCH(4); break;
+    case 2: RBQ_PLAN_LAUNCH(2); break;
+    default: RBQ_PLAN_LAUNCH(1); break;
+  }
+#undef RBQ_PLAN_LAUNCH
   RBQ_LAUNCH_OK(ctx);
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;

@@ -246,15 +246,17 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
     if (t < cnt) {
       load_tile(t);
       build_a(s_n2);
+      if (t + stride < cnt) load_tile(t + stride);
     }
     for (int it = 0; t < cnt; ++it) {
       const int tn = t + stride;
-      const bool next = tn < cnt;
-      if (next) load_tile(tn);
       wait_bar(s_bar, phase);
       phase ^= 1u;
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      if (next) build_a(s_n2 + ((it + 1) & 1) * T5_TOK);
+      if (tn < cnt) {
+        build_a(s_n2 + ((it + 1) & 1) * T5_TOK);                // tile tn (its raw K was loaded one epilogue ago)
+        if (tn + stride < cnt) load_tile(tn + stride);          // in flight during the epilogue below
+      }
       epilogue(t, it & 1, s_n2 + (it & 1) * T5_TOK);
       t = tn;
     }
