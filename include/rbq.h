@@ -140,6 +140,20 @@ int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float
 int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p,
                     int32_t* sel_idx, int32_t* sel_cnt, void* stream);
 
+/* ---- S6'  the paper's Top-p operator: Algorithm 3, ternary threshold search (L217-252; 4.1 L256-264;
+ *           App. B.1) -- alternative selector, SURVEY.md 8(f) row 2 --------------------- */
+/* Per row: prob = softmax(scores[b][h][0..n_indexed[b])) in fp64; low = 0, high = max(prob); repeat
+ * { pi0 = (high + 2 low)/3, pi1 = (2 high + low)/3, G0/G1 = mass above pi0/pi1, v_min = min{s > low},
+ * v_max = max{s <= high}; G1 >= p: low = pi1; else G0 >= p: low = pi0, high = min(pi1, v_max); else
+ * high = min(pi0, v_max) } until v_min = v_max (at most 4096 iterations); selected = {t : prob_t > low}.
+ * Unlike rbq_topp_select this keeps EVERY token tied with the boundary value (Alg.3's mask), so the set
+ * is the minimal one only when the boundary value is unique.  p >= 1 selects every indexed token.
+ * Same buffers as rbq_topp_select (device pointers; sel_idx ascending); iters int32 [B][Hq] or NULL
+ * receives the iteration counts.  Needs no workspace.  Rows longer than 204 800 tokens:
+ * RBQ_ERR_UNSUPPORTED.                                                                            */
+int rbq_topp_select_alg3(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p,
+                         int32_t* sel_idx, int32_t* sel_cnt, int32_t* iters, void* stream);
+
 /* ---- S7  hybrid attention over selected U pending tokens (Alg.2 lines 14-15, L188-190, L215) -- */
 /* out[b][h] = sum_{t in A} softmax_A(<q,k_t> sm_scale)_t v_t, A = sel_idx[b][h][0..cnt) U
  * [n_indexed[b], n_total[b]); out_dtype [B][Hq][D]; lse float [B][Hq] or NULL (log-sum-exp over A).

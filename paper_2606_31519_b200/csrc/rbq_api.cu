@@ -225,6 +225,15 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
                          (cudaStream_t)stream);
 }
 
+int rbq_topp_select_alg3(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
+                         int32_t* iters, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, false));
+  if (!scores || !sel_idx || !sel_cnt) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores/sel_idx/sel_cnt null");
+  if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
+  return rbq_launch_topp_alg3(ctx, scores, idx->n_indexed, p, sel_idx, sel_cnt, iters, (cudaStream_t)stream);
+}
+
 int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, const int32_t* sel_idx,
                          const int32_t* sel_cnt, void* out, float* lse, void* stream) {
   RBQ_CTX(ctx);

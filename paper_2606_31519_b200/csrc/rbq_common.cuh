@@ -135,6 +135,9 @@ int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot,
 // rowmax_key: order-preserving keys of the row maxima [B*Hq] (written by S5), or NULL to compute them here.
 int rbq_launch_topp(rbq_ctx*, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p,
                     uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
+// Alg.3 selector (ternary threshold search in fp64): ascending sel_idx, sel_cnt, optional iteration counts [B*Hq].
+int rbq_launch_topp_alg3(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx, int32_t* sel_cnt,
+                         int32_t* iters, cudaStream_t);
 int rbq_launch_bits_from_lists(rbq_ctx*, const rbq_index*, const int32_t* sel_idx, const int32_t* sel_cnt,
                                uint32_t* sel_bits, cudaStream_t);
 // S7 from the selection bitmaps: union plan -> gather attention -> merge.

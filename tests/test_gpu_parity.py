@@ -349,6 +349,60 @@ def test_topp_cluster_sizes(orc, rot128, B, L):
     c.close()
 
 
+@pytest.mark.parametrize("B,L", [(1, 5000), (2, 40000), (1, 131072)])
+def test_topp_alg3_selector(orc, rot128, B, L):
+    """rbq_topp_select_alg3 (the paper's Alg.3) against the oracle's Alg.3 on fp64 softmax probabilities:
+    identical masks (a mismatch is tolerated only for tokens within 1e-9 relative of the boundary probability), the
+    mask is a threshold set whose mass reaches p and is minimal up to ties, iteration counts agree, p >= 1 selects all."""
+    import torch
+    rng = np.random.default_rng(11 + L)
+    w = U.workload(3, L=L, B=B)
+    rows, Lc = w.B * w.Hq, w.Lcap
+    n_seq = w.seq_lens.copy()
+    scores = (rng.standard_normal((w.B, w.Hq, Lc)) * rng.uniform(0.5, 6.0, (w.B, w.Hq, 1))).astype(np.float32)
+    scores[:, 0, :] = np.round(scores[:, 0, :] * 2) / 2            # heavy ties: Alg.3 keeps every tied token
+    o = dict(codes=np.zeros((w.B, w.Hkv, Lc, 4), np.uint32), f_scale=np.zeros((w.B, w.Hkv, Lc), np.float32),
+             c_k=np.zeros((w.B, w.Hkv, 128), np.float32), n_indexed=n_seq, n_total=n_seq)
+    c = U.make_cache(w, rot128[0], upload_kv=False)
+    U.load_index(c, o)
+    sc_dev = U.to_dev(scores)
+    heads = range(w.Hq) if L <= 40000 else (0, 1, w.Hq - 1)
+    for p in (np.float32(0.5), np.float32(0.9)):
+        sel_idx, sel_cnt = c.new_sel()
+        sel_idx.fill_(-1)
+        iters = torch.zeros((w.B, w.Hq), dtype=torch.int32, device="cuda")
+        c.topp_select_alg3(sc_dev, float(p), sel_idx, sel_cnt, iters)
+        torch.cuda.synchronize()
+        idx, cnt, its = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy(), iters.cpu().numpy()
+        for b in range(w.B):
+            n = int(n_seq[b])
+            for h in heads:
+                s64 = scores[b, h, :n].astype(np.float64)
+                e = np.exp(s64 - s64.max())
+                prob = e / e.sum()
+                ref_mask, ref_it = orc.topp_alg3(prob, float(p))
+                g = idx[b, h, :cnt[b, h]]
+                assert (np.diff(g) > 0).all() and g.min() >= 0 and g.max() < n
+                mask = np.zeros(n, bool)
+                mask[g] = True
+                if not (mask == ref_mask).all():
+                    edge = prob[ref_mask].min()
+                    diff = mask != ref_mask
+                    assert (np.abs(prob[diff] - edge) <= 1e-9 * edge).all(), (b, h, int(diff.sum()))
+                else:
+                    assert abs(int(its[b, h]) - ref_it) <= 1, (its[b, h], ref_it)
+                # threshold set, mass >= p, minimal up to ties
+                thr = prob[mask].min()
+                assert (prob[~mask] < thr).all() or not (~mask).any()
+                assert prob[mask].sum() >= float(p) - 1e-12
+                assert prob[prob > thr].sum() < float(p) + 1e-12
+    sel_idx, sel_cnt = c.new_sel()
+    c.topp_select_alg3(sc_dev, 1.0, sel_idx, sel_cnt)
+    torch.cuda.synchronize()
+    assert (sel_cnt.cpu().numpy() == n_seq[:, None]).all()
+    c.close()
+
+
 def test_topp_literal_config_tie_break(orc, rot128):
     """P9: literal BASELINE config 0 (sink keys = 2 x query): Top-p(0.9) = {0,1,2,3}, Top-p(0.7) = {0,1,2}."""
     import torch
