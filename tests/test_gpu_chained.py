@@ -146,6 +146,45 @@ def test_append_flush_state_machine(orc, rot128, use_side, kind):
     c.close()
 
 
+def test_append_flush_enc_fast(orc, rot128):
+    """Lazy flush through RBQ_ENC_FAST (tcgen05 encode with per-sequence t_begin / t_count, tiles far from full): the
+    flushed rows carry the oracle's codes up to the guard band (|y_j| <= 1e-5 ||x||) and its factors within 1e-5."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb, synth
+    W = 64
+    w = U.workload(3, L=1500, B=3, extra_cap=256)
+    rot = rot128[0]
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, ROT_DENSE, rot, W)
+    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(rot), flush_tokens=W, enc_mode=rb.RBQ_ENC_FAST)
+    c.K.copy_(U.to_dev(w.K, torch.bfloat16))
+    c.V.copy_(U.to_dev(w.V, torch.bfloat16))
+    c.encode_keys(U.to_dev(w.seq_lens))
+    side = torch.cuda.Stream()
+    for s, n_new in enumerate([40, 40, 64, 30, 100]):
+        k_new, v_new = synth.append_rows(3, 90 + s, w.B, w.Hkv, n_new)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16), side_stream=side)
+        torch.cuda.synchronize()
+        assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all() and (c.n_total.cpu().numpy() == lazy.n_total).all()
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    P = rot.astype(np.float64)
+    n0 = w.seq_lens
+    for b in range(w.B):
+        n = int(lazy.n_indexed[b]) + lazy.in_flight
+        assert n > int(n0[b])
+        for g in range(w.Hkv):
+            x = lazy.K[b, g, :n].astype(np.float64) - lazy.c_k[b, g].astype(np.float64)
+            y = x @ P
+            xn = np.linalg.norm(x, axis=1, keepdims=True)
+            diff = codes[b, g, :n] ^ lazy.codes[b, g, :n]
+            bits = ((diff[:, :, None] >> np.arange(32, dtype=np.uint32)) & 1).reshape(n, 128).astype(bool)
+            assert (np.abs(y)[bits] <= 1e-5 * np.broadcast_to(xn, y.shape)[bits]).all()
+            ref = lazy.f_scale[b, g, :n].astype(np.float64)
+            assert (np.abs(fs[b, g, :n] - ref) <= 1e-5 * np.abs(ref)).all()
+    c.close()
+
+
 def test_append_many_tokens_per_call(orc, rot128):
     """n_new = 5 per call with W = 8 (flush of whole windows only), and n_new >= W in one call."""
     import torch

@@ -98,10 +98,21 @@ def test_encode_fast_guard_band(orc, rot128, name):
     """RBQ_ENC_FAST (tensor-core rotation, bf16 hi/lo split): a code bit may differ from the oracle's only where the
     fp64 rotated coordinate satisfies |y_j| <= 1e-5 ||x|| (expected fraction ~9e-5, fail above 3e-4); f_scale within
     1e-5 relative."""
+    _check_encode_fast(orc, rot128[0], get_case(name))
+
+
+def test_encode_fast_many_tiles(orc, rot128):
+    """The tcgen05 encode kernel over several 128-token tiles per CTA and pipeline group (double-buffered accumulators,
+    mbarrier phases, register prefetch), a ragged last tile, and a KV head whose keys are all identical (x = 0 for every
+    token: zero codes and zero factors, Alg.1 with ||x|| = 0)."""
+    w = U.workload(1, L=40077)
+    w.K[0, 0, :, :] = w.K[0, 0, :1, :]
+    _check_encode_fast(orc, rot128[0], w)
+
+
+def _check_encode_fast(orc, rot, w):
     import torch
     from paper_2606_31519_b200 import binding as rb
-    w = get_case(name)
-    rot = rot128[0]
     o = U.oracle_index(orc, w, rot, ROT_DENSE)
     c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(rot), enc_mode=rb.RBQ_ENC_FAST)
     c.K.copy_(U.to_dev(w.K, torch.bfloat16))
@@ -125,6 +136,8 @@ def test_encode_fast_guard_band(orc, rot128, name):
             n_diff += int(bits.sum())
             ref = o["f_scale"][b, g, :n].astype(np.float64)
             assert (np.abs(fs[b, g, :n] - ref) <= 1e-5 * np.abs(ref)).all(), "f_scale outside 1e-5 relative"
+            zero = (xn[:, 0] == 0.0)
+            assert (codes[b, g, :n][zero] == 0).all() and (fs[b, g, :n][zero] == 0.0).all()
     assert n_diff <= 3e-4 * n_bits, f"{n_diff} of {n_bits} bits differ"
     c.close()
 
