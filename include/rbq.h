@@ -49,8 +49,9 @@ typedef enum { RBQ_ROT_DENSE = 0, RBQ_ROT_WH = 1 } rbq_rot_kind;
 /* EXACT: canonical fp32 order (R1) -> codes/factors bit-identical to the oracle.
  * FAST : rotation on the tcgen05 tensor cores (bf16 hi/lo split, fp32 accumulate in TMEM: the kernel
  *        takes all 512 TMEM columns of its SM while it runs); codes may differ only where
- *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  Built for bf16 K/V with the dense
- *        rotation; other combinations: rbq_create returns RBQ_ERR_UNSUPPORTED. */
+ *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  Built for bf16 K/V (both
+ *        rotation kinds: the Walsh-Hadamard rotation runs as its dense matrix); fp32 K/V:
+ *        rbq_create returns RBQ_ERR_UNSUPPORTED. */
 typedef enum { RBQ_ENC_EXACT = 0, RBQ_ENC_FAST = 1 } rbq_enc_mode;
 
 /* flags of rbq_encode_keys */

@@ -82,7 +82,7 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
     if (d != RBQ_F32 && d != RBQ_BF16) return RBQ_ERR_INVALID_ARG;
   if (cfg->rot_kind != RBQ_ROT_DENSE && cfg->rot_kind != RBQ_ROT_WH) return RBQ_ERR_INVALID_ARG;
   // tensor-core rotation: built for bf16 K/V and the dense rotation (the WH path is already a fast transform)
-  if (cfg->enc_mode == RBQ_ENC_FAST && (cfg->kv_dtype != RBQ_BF16 || cfg->rot_kind != RBQ_ROT_DENSE)) return RBQ_ERR_UNSUPPORTED;
+  if (cfg->enc_mode == RBQ_ENC_FAST && cfg->kv_dtype != RBQ_BF16) return RBQ_ERR_UNSUPPORTED;
   if (cfg->enc_mode != RBQ_ENC_EXACT && cfg->enc_mode != RBQ_ENC_FAST) return RBQ_ERR_INVALID_ARG;
   if (!cfg->rot || !(cfg->sm_scale >= 0.0f)) return RBQ_ERR_INVALID_ARG;
   int dev = 0, sms = 0;

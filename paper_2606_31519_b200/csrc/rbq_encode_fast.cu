@@ -17,7 +17,8 @@
 //                 then the epilogue of the previous tile: tcgen05.ld (one token row per thread, 64 columns per warp),
 //                 l1 and sign bits, the two column halves meet in shared memory, codes / f_scale stored coalesced.
 //   issuer warp : waits "full", one lane issues the 24 MMAs of the tile, tcgen05.commit -> mbarrier "done".
-// P_hi / P_lo are staged once per CTA in the same layout (B operand, N x K).  MMA(t + 1) runs under epilogue(t) and
+// P_hi / P_lo are staged once per CTA in the same layout (B operand, N x K); for the Walsh-Hadamard rotation the dense
+// matrix diag(s) H / sqrt(D) is generated in that loop from the sign vector (the same kernel serves both rotations).  MMA(t + 1) runs under epilogue(t) and
 // under the other group's operand build.
 #include "rbq_common.cuh"
 
@@ -73,7 +74,7 @@ __device__ __forceinline__ void t5_split8(const float (&v)[8], uint4& hi, uint4&
 __global__ void __launch_bounds__(T5_THREADS, 1)
 encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long sh, long long st,
                   const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count, int fixed_count, int Hkv,
-                  int Lcap, const float* __restrict__ rot, const float* __restrict__ c_k, uint32_t* __restrict__ codes,
+                  int Lcap, const float* __restrict__ rot, int wh, const float* __restrict__ c_k, uint32_t* __restrict__ codes,
                   float* __restrict__ f_scale) {
   extern __shared__ __align__(128) unsigned char t5_smem[];
   const bool issuer = threadIdx.x >= T5_GROUPS * T5_GTHREADS;  // the last T5_GROUPS warps only issue MMAs
@@ -111,7 +112,16 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
   for (int e = threadIdx.x; e < RBQ_D * RBQ_D / 2; e += T5_THREADS) {
     const int j = e & 127, i2 = (e >> 7) * 2;
     uint32_t hi, lo;
-    ef_split(__ldg(rot + i2 * RBQ_D + j), __ldg(rot + (i2 + 1) * RBQ_D + j), hi, lo);
+    float p0, p1;
+    if (wh) {                                                   // Walsh-Hadamard: P = diag(s) H / sqrt(D), H_ij = (-1)^popc(i & j)
+      const float r = 1.0f / sqrtf((float)RBQ_D);
+      p0 = __ldg(rot + i2) * ((__popc(i2 & j) & 1) ? -r : r);
+      p1 = __ldg(rot + i2 + 1) * ((__popc((i2 + 1) & j) & 1) ? -r : r);
+    } else {
+      p0 = __ldg(rot + i2 * RBQ_D + j);
+      p1 = __ldg(rot + (i2 + 1) * RBQ_D + j);
+    }
+    ef_split(p0, p1, hi, lo);
     const int off = (i2 >> 3) * T5_LBO + (j >> 3) * T5_SBO + (j & 7) * 16 + (i2 & 7) * 2;
     *reinterpret_cast<uint32_t*>(s_bh + off) = hi;
     *reinterpret_cast<uint32_t*>(s_bl + off) = lo;
@@ -281,7 +291,8 @@ int rbq_launch_encode_fast(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin
   gx = gx < 1 ? 1 : (gx > tiles ? tiles : gx);
   encode_tc5_kernel<<<dim3(gx, BG), T5_THREADS, T5_SMEM, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count,
                                                              fixed_count, ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
-                                                             ctx->cfg.rot, idx->c_k, idx->codes, idx->f_scale);
+                                                             ctx->cfg.rot, ctx->cfg.rot_kind == RBQ_ROT_WH ? 1 : 0, idx->c_k,
+                                                             idx->codes, idx->f_scale);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

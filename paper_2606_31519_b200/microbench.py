@@ -39,7 +39,8 @@ def encode(reps):
     units = B * Hkv * L
     for name, r, kind, mode in (("dense RBQ_ENC_EXACT", rot, rb.RBQ_ROT_DENSE, rb.RBQ_ENC_EXACT),
                                 ("dense RBQ_ENC_FAST", rot, rb.RBQ_ROT_DENSE, rb.RBQ_ENC_FAST),
-                                ("Walsh-Hadamard RBQ_ENC_EXACT", wh, rb.RBQ_ROT_WH, rb.RBQ_ENC_EXACT)):
+                                ("Walsh-Hadamard RBQ_ENC_EXACT", wh, rb.RBQ_ROT_WH, rb.RBQ_ENC_EXACT),
+                                ("Walsh-Hadamard RBQ_ENC_FAST", wh, rb.RBQ_ROT_WH, rb.RBQ_ENC_FAST)):
         c = rb.RaBitQCache(B, Hq, Hkv, L, r, rot_kind=kind, enc_mode=mode)
         c.K.copy_(K)
         full = _time_us(lambda: c.encode_keys(sl), reps, warm=2)

@@ -93,12 +93,13 @@ def test_encode_ck_given_and_zero_key(orc, rot128):
     c.close()
 
 
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
 @pytest.mark.parametrize("name", ["cfg1_small", "cfg3_small"])
-def test_encode_fast_guard_band(orc, rot128, name):
+def test_encode_fast_guard_band(orc, rot128, wh_signs, name, kind):
     """RBQ_ENC_FAST (tensor-core rotation, bf16 hi/lo split): a code bit may differ from the oracle's only where the
     fp64 rotated coordinate satisfies |y_j| <= 1e-5 ||x|| (expected fraction ~9e-5, fail above 3e-4); f_scale within
     1e-5 relative."""
-    _check_encode_fast(orc, rot128[0], get_case(name))
+    _check_encode_fast(orc, _rot(kind, rot128, wh_signs), get_case(name), kind)
 
 
 def test_encode_fast_many_tiles(orc, rot128):
@@ -110,18 +111,19 @@ def test_encode_fast_many_tiles(orc, rot128):
     _check_encode_fast(orc, rot128[0], w)
 
 
-def _check_encode_fast(orc, rot, w):
+def _check_encode_fast(orc, rot, w, kind=ROT_DENSE):
     import torch
     from paper_2606_31519_b200 import binding as rb
-    o = U.oracle_index(orc, w, rot, ROT_DENSE)
-    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(rot), enc_mode=rb.RBQ_ENC_FAST)
+    o = U.oracle_index(orc, w, rot, kind)
+    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(np.ascontiguousarray(rot, dtype=np.float32)), rot_kind=kind,
+                       enc_mode=rb.RBQ_ENC_FAST)
     c.K.copy_(U.to_dev(w.K, torch.bfloat16))
     c.encode_keys(U.to_dev(w.seq_lens))
     torch.cuda.synchronize()
     assert np.array_equal(c.c_k.cpu().numpy().view(np.uint32), o["c_k"].view(np.uint32))
     codes = c.codes.cpu().numpy().view(np.uint32)
     fs = c.f_scale.cpu().numpy()
-    P = rot.astype(np.float64)
+    P = (rot if kind == ROT_DENSE else orc.rotation_wh(rot)).astype(np.float64)
     n_bits = n_diff = 0
     for b in range(w.B):
         n = int(w.seq_lens[b])
