@@ -604,11 +604,22 @@ int launch_cs(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, con
 
 }  // namespace
 
-// Cluster size: 8 CTAs per row while that still fills the GPU at most ~4 times over; fewer (down to 1) for many
-// short rows, as long as the slice of a CTA stays <= 16 K scores (two CTAs per SM).
+// Cluster size.  Few rows (<= one per SM): the largest of 8 / 4 / 2 / 1 CTAs per row that still gives every CTA an SM of its
+// own (measured at config 2: 4 CTAs per row on 128 SMs make the step 6 us shorter than 8 per row with two CTAs on most
+// SMs, although the kernel alone is 4 us longer -- its prologue overlaps the estimator's tail and it has half the exchange
+// partners), as long as the slice fits in shared memory.  Many rows: 8 per row while that fills the GPU at most ~4 times
+// over, fewer (down to 1) as long as the slice of a CTA stays <= 16 K scores (two CTAs per SM).
 int rbq_topp_cluster_size(const rbq_ctx* ctx) {
   const long long rows = (long long)ctx->cfg.batch * ctx->cfg.n_q_heads;
+  auto fits = [&](int c) {
+    const long long s_cap = ((((ctx->cfg.max_tokens + c - 1) / c) + 31) & ~31) + 32;
+    return TP_OFF_SC + (size_t)s_cap * 4 <= 227 * 1024 && s_cap <= 32 * TP_NB;
+  };
   int cs = 8;
+  if (rows <= ctx->sm_count) {
+    while (cs > 1 && rows * cs > ctx->sm_count && fits(cs >> 1)) cs >>= 1;
+    return cs;
+  }
   while (cs > 1 && rows * cs > 4ll * ctx->sm_count && (ctx->cfg.max_tokens + cs / 2 - 1) / (cs / 2) <= 16384) cs >>= 1;
   return cs;
 }

@@ -338,8 +338,9 @@ def test_topp_edge_rows(orc, rot128):
 
 @pytest.mark.parametrize("B,L", [(1, 40000), (8, 3000), (16, 2100), (3, 90)])
 def test_topp_cluster_sizes(orc, rot128, B, L):
-    """Every cluster size of the Top-p kernel (8 / 4 / 2 / 1 CTAs per row, chosen from the row count), rows
-    shorter than one bitmap word per CTA, and the fused step without index lists (sel_idx = NULL)."""
+    """Cluster sizes 4 / 2 / 1 / 1 of the Top-p kernel (chosen from the row count and the row length; 8 CTAs per row is
+    what the single-row config-0 cases run), rows shorter than one bitmap word per CTA, and the fused step without index
+    lists (sel_idx = NULL)."""
     import torch
     rng = np.random.default_rng(5 + B)
     w = U.workload(3, L=L, B=B)
