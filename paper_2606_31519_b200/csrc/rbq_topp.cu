@@ -81,11 +81,15 @@ __device__ __forceinline__ u64 composite(float s, int t) {
 }
 // Histogram = two u32 arrays (all 32 banks in use): hist[j] = low 32 bits of the mass, hist[TP_NB + j] = (count << 12) |
 // (mass >> 32).  hist[j] += (count c, mass v):
-__device__ __forceinline__ void hist_add(uint32_t* hist, int j, u64 v, uint32_t c) {
+// (explicit shared-space atomics on a 32-bit shared address: a generic-pointer atomicAdd makes the compiler rebuild the
+// shared-window address from SR_CgaCtaId for every atomic inside a cluster kernel)
+__device__ __forceinline__ void hist_add(uint32_t hist_sa, int j, u64 v, uint32_t c) {
+  const uint32_t sa = hist_sa + 4u * (uint32_t)j;
   const uint32_t lo = (uint32_t)v;
-  const uint32_t old = atomicAdd(&hist[j], lo);
+  uint32_t old;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(sa), "r"(lo) : "memory");
   const uint32_t carry = (old + lo < old) ? 1u : 0u;
-  atomicAdd(&hist[TP_NB + j], (c << 12) + (uint32_t)(v >> 32) + carry);
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 4u * TP_NB), "r"((c << 12) + (uint32_t)(v >> 32) + carry) : "memory");
 }
 __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
   cnt = v.y >> 12;
@@ -169,6 +173,8 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
   uint32_t* hist = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);
+  uint32_t hist_sa = (uint32_t)__cvta_generic_to_shared(hist);   // 32-bit shared address for the histogram atomics,
+  asm volatile("mov.u32 %0, %0;" : "+r"(hist_sa));               // opaque: kept in a register, not rebuilt from SR_CgaCtaId per atomic
   uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);          // aliases hist once the cut is known
   u64* all_comp = reinterpret_cast<u64*>(smem_raw + TP_OFF_A);
   uint32_t* all_rfix = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A + TP_CAND * 8);
@@ -248,7 +254,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
         if (lane == 0) {
-          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add(hist, j0, t, 128u);
+          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add(hist_sa, j0, t, 128u);
         }
       } else {
 #pragma unroll
@@ -256,13 +262,13 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
           const bool of = j[k] == TP_NB - 1;
           of_c += of ? 1u : 0u;
           of_r += of ? (u64)rf[k] : 0ull;
-          if (j[k] >= 0 && !of) hist_add(hist, j[k], (u64)rf[k], 1u);
+          if (j[k] >= 0 && !of) hist_add(hist_sa, j[k], (u64)rf[k], 1u);
         }
       }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { of_c += __shfl_xor_sync(FULL, of_c, o); of_r += __shfl_xor_sync(FULL, of_r, o); }
-    if (lane == 0 && of_c) hist_add(hist, TP_NB - 1, of_r, of_c);
+    if (lane == 0 && of_c) hist_add(hist_sa, TP_NB - 1, of_r, of_c);
   }
   __syncthreads();
   // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins 4t..4t+3, 8 threads per coarse bin
@@ -402,9 +408,9 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
           u64 v = rfix;
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-          if (lane == 0) hist_add(hist, j0, v, 32u);
+          if (lane == 0) hist_add(hist_sa, j0, v, 32u);
         } else if (j >= 0) {
-          hist_add(hist, j, (u64)rfix, 1u);
+          hist_add(hist_sa, j, (u64)rfix, 1u);
         }
       }
       csync();
