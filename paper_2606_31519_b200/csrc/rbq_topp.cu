@@ -91,6 +91,15 @@ __device__ __forceinline__ void hist_add(uint32_t hist_sa, int j, u64 v, uint32_
   const uint32_t carry = (old + lo < old) ? 1u : 0u;
   asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 4u * TP_NB), "r"((c << 12) + (uint32_t)(v >> 32) + carry) : "memory");
 }
+// Pass-1 form of the histogram: three u32 arrays (mass bits 0..11, mass >> 12, count) updated by three independent
+// reductions without return value -- no carry, so nothing waits for an atomic's result.  Sums stay below 2^32: at most
+// 2^16 tokens per CTA with r < 2^23.  Folded into the (lo, count | hi) form after the pass.
+__device__ __forceinline__ void hist_add3(uint32_t hist_sa, int j, u64 v, uint32_t c) {
+  const uint32_t sa = hist_sa + 4u * (uint32_t)j;
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa), "r"((uint32_t)v & 0xFFFu) : "memory");
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 4u * TP_NB), "r"((uint32_t)(v >> 12)) : "memory");
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 8u * TP_NB), "r"(c) : "memory");
+}
 __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
   cnt = v.y >> 12;
   R = ((u64)(v.y & 0xFFFu) << 32) | v.x;
@@ -213,7 +222,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
 
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
-  for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
+  for (int i = tid; i < 3 * TP_NB; i += TP_THREADS) hist[i] = 0u;   // third array: start of the candidate area, free until S1
   if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
   else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
@@ -254,7 +263,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
         if (lane == 0) {
-          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add(hist_sa, j0, t, 128u);
+          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add3(hist_sa, j0, t, 128u);
         }
       } else {
 #pragma unroll
@@ -262,13 +271,19 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
           const bool of = j[k] == TP_NB - 1;
           of_c += of ? 1u : 0u;
           of_r += of ? (u64)rf[k] : 0ull;
-          if (j[k] >= 0 && !of) hist_add(hist_sa, j[k], (u64)rf[k], 1u);
+          if (j[k] >= 0 && !of) hist_add3(hist_sa, j[k], (u64)rf[k], 1u);
         }
       }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { of_c += __shfl_xor_sync(FULL, of_c, o); of_r += __shfl_xor_sync(FULL, of_r, o); }
-    if (lane == 0 && of_c) hist_add(hist_sa, TP_NB - 1, of_r, of_c);
+    if (lane == 0 && of_c) hist_add3(hist_sa, TP_NB - 1, of_r, of_c);
+  }
+  __syncthreads();
+  for (int b = tid; b < TP_NB; b += TP_THREADS) {               // fold into hist[b] = mass lo, hist[TP_NB + b] = count << 12 | mass hi
+    const u64 mass = (u64)hist[b] + ((u64)hist[TP_NB + b] << 12);
+    hist[b] = (uint32_t)mass;
+    hist[TP_NB + b] = (hist[2 * TP_NB + b] << 12) | (uint32_t)(mass >> 32);
   }
   __syncthreads();
   // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins 4t..4t+3, 8 threads per coarse bin
