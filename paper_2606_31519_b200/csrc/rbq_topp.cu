@@ -242,6 +242,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
       asm volatile("cp.async.commit_group;" ::: "memory");
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
+#pragma unroll 2
     for (int base = warp * 32; base < n4; base += TP_THREADS) {
       const int i4 = base + lane;
       float v[4] = {0.f, 0.f, 0.f, 0.f};
@@ -533,6 +534,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     const float sstar = rbq_fkey_inv((uint32_t)(cstar >> 32));
     const int tstar = (int)(~(uint32_t)cstar);                // equal scores: indices <= tstar are selected
     const int n4r = nwords * 8;                               // float4 groups, rounded up to whole words
+#pragma unroll 2
     for (int base = warp * 32; base < n4r; base += TP_THREADS) {
       const int i4 = base + lane;
       const float4 v4 = (i4 < n4r) ? reinterpret_cast<const float4*>(sc)[i4] : make_float4(0.f, 0.f, 0.f, 0.f);
