@@ -316,10 +316,22 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
   const size_t ob = rows * RBQ_D * (ctx->cfg.out_dtype == RBQ_BF16 ? 2 : 4);
   void* dq = ws_ptr<char>(ctx, ctx->off_stage_q);
   void* dout = ws_ptr<char>(ctx, ctx->off_stage_out);
+  // out_host in pinned (page-locked, mapped) memory: the merge of S7 stores the result straight into it over PCIe and the
+  // device-to-host copy disappears; pageable memory goes through the staging buffer.  q is always staged: every warp of the
+  // gather reads it.
+  void* out_mapped = nullptr;
+  {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, out_host) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer &&
+        aligned16(at.devicePointer))
+      out_mapped = at.devicePointer;
+    else
+      cudaGetLastError();
+  }
   auto direct = [&]() -> int {
     RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
-    RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, dout, nullptr, nullptr, stream));
-    RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
+    RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, out_mapped ? out_mapped : dout, nullptr, nullptr, stream));
+    if (!out_mapped) RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
     return RBQ_OK;
   };
   // One CPU-side launch per step instead of seven: the sequence is captured once per argument set and replayed.

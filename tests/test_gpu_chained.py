@@ -232,6 +232,15 @@ def test_decode_step_host_buffers(orc, rot128):
     c.decode_step(q_host.cuda(), 0.9, out)
     torch.cuda.synchronize()
     assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+    # pageable host buffers take the staged path (pinned ones receive the result straight from the S7 merge)
+    q_page = torch.from_numpy(w.q).to(torch.bfloat16).clone()
+    out_page = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32)
+    assert not q_page.is_pinned() and not out_page.is_pinned()
+    for st in (None, side):
+        out_page.zero_()
+        c.decode_step_host(q_page, 0.9, out_page, stream=st)
+        (side if st is not None else torch.cuda.current_stream()).synchronize()
+        assert (out_page.numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
     assert c.launch_count() > 0
     c.close()
 
