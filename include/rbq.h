@@ -173,8 +173,9 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
 /* ---- host-buffer convenience used by the end-to-end measurement ------------------------------ */
 /* Same as rbq_decode_step but q_host / out_host are HOST buffers (pinned recommended): copies q
  * host->device, runs the step, copies out device->host, all on `stream`; staging device buffers
- * come from the workspace.  When out_host is page-locked (mapped) memory the last kernel stores
- * the result straight into it and the device->host copy is skipped.  Does not synchronise; the
+ * come from the workspace.  With page-locked (mapped) buffers the copies disappear: S3 reads
+ * q_host over PCIe (leaving a device copy for S7) and the last kernel stores the result straight
+ * into out_host; pageable buffers are staged with cudaMemcpyAsync.  Does not synchronise; the
  * caller synchronises the stream (the result is valid in out_host only after that).  On a
  * non-default stream the sequence is captured once per argument set and replayed as one CUDA graph
  * (one CPU-side launch per step); on the legacy default stream it is launched directly.        */

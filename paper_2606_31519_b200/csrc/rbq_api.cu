@@ -191,7 +191,7 @@ int rbq_query_quantize(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_
   RBQ_TRY(check_idx(ctx, idx, false));
   RBQ_TRY(need_ws(ctx));
   if (!q) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q null");
-  return rbq_launch_query(ctx, q, idx, qu, qparams, (cudaStream_t)stream);
+  return rbq_launch_query(ctx, q, idx, qu, qparams, nullptr, (cudaStream_t)stream);
 }
 
 int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32_t* dot, int32_t* pop, void* stream) {
@@ -199,7 +199,7 @@ int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32
   RBQ_TRY(check_idx(ctx, idx, true));
   RBQ_TRY(need_ws(ctx));
   if (!q || !dot || !pop) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/dot/pop null");
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, (cudaStream_t)stream));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
   return rbq_launch_estimate(ctx, idx, nullptr, dot, pop, (cudaStream_t)stream);
 }
 
@@ -209,7 +209,7 @@ int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float
   RBQ_TRY(need_ws(ctx));
   if (!q || !scores) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/scores null");
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, (cudaStream_t)stream));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
   return rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, (cudaStream_t)stream);
 }
 
@@ -246,8 +246,10 @@ int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const
   return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, lse, (cudaStream_t)stream);
 }
 
-int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, float p, void* out,
-                    int32_t* sel_idx, int32_t* sel_cnt, void* stream) {
+// q_copy != NULL: q is readable by the device but far away (mapped host memory): S3 reads it once and leaves a device copy
+// in q_copy, which S7 (every warp of the gather reads q) uses instead.
+static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq_kv* cache, const rbq_index* idx, float p, void* out,
+                            int32_t* sel_idx, int32_t* sel_cnt, void* stream) {
   RBQ_CTX(ctx);
   RBQ_TRY(check_kv(ctx, cache));
   RBQ_TRY(check_idx(ctx, idx, true));
@@ -262,16 +264,21 @@ int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_
   if (ctx->prof_on && ctx->prof_steps < RBQ_PROFILE_MAX_STEPS) ev = ctx->prof_ev + (size_t)ctx->prof_steps++ * (RBQ_N_STAGES + 1);
   ctx->stage_ev = ev;
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[0], s));
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, s));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, q_copy, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
   RBQ_TRY(rbq_launch_topp(ctx, scores, ws_ptr<uint32_t>(ctx, ctx->off_rowmax), idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
-  const int rc = rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
+  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
   ctx->stage_ev = nullptr;
   if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[RBQ_N_STAGES], s));
   return rc;
+}
+
+int rbq_decode_step(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx, float p, void* out,
+                    int32_t* sel_idx, int32_t* sel_cnt, void* stream) {
+  return decode_step_impl(ctx, q, nullptr, cache, idx, p, out, sel_idx, sel_cnt, stream);
 }
 
 int rbq_profile_enable(rbq_ctx* ctx, int enable) {
@@ -319,18 +326,19 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
   // out_host in pinned (page-locked, mapped) memory: the merge of S7 stores the result straight into it over PCIe and the
   // device-to-host copy disappears; pageable memory goes through the staging buffer.  q is always staged: every warp of the
   // gather reads it.
-  void* out_mapped = nullptr;
-  {
+  auto mapped = [&](const void* h) -> void* {
     cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, out_host) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer &&
-        aligned16(at.devicePointer))
-      out_mapped = at.devicePointer;
-    else
-      cudaGetLastError();
-  }
+    if (cudaPointerGetAttributes(&at, h) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer && aligned16(at.devicePointer))
+      return at.devicePointer;
+    cudaGetLastError();
+    return nullptr;
+  };
+  void* out_mapped = mapped(out_host);
+  const void* q_mapped = mapped(q_host);                       // S3 reads q over PCIe and leaves the device copy for S7
   auto direct = [&]() -> int {
-    RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
-    RBQ_TRY(rbq_decode_step(ctx, dq, cache, idx, p, out_mapped ? out_mapped : dout, nullptr, nullptr, stream));
+    if (!q_mapped) RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
+    RBQ_TRY(decode_step_impl(ctx, q_mapped ? q_mapped : dq, q_mapped ? dq : nullptr, cache, idx, p, out_mapped ? out_mapped : dout,
+                             nullptr, nullptr, stream));
     if (!out_mapped) RBQ_CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, s));
     return RBQ_OK;
   };

@@ -15,7 +15,7 @@ __global__ void __launch_bounds__(RBQ_MAX_G * RBQ_D)
 query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const float* __restrict__ c_k,
              const float* __restrict__ rot, int rot_kind, int Hq, int Hkv, float sm_scale,
              uint8_t* __restrict__ qu_out, float* __restrict__ qparams, RbqQConst* __restrict__ qc_out,
-             uint32_t* __restrict__ rowmax_key) {
+             uint32_t* __restrict__ rowmax_key, TQ* __restrict__ q_copy) {
   rbq_pdl_trigger();                               // S4/S5 may become resident while this kernel runs
   const int G = Hq / Hkv;
   const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv;
@@ -36,6 +36,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
   __shared__ uint8_t s_qu[RBQ_MAX_G][RBQ_D];
 
   const float qv = rbq_ld_elem(q, row * RBQ_D + j);
+  if (q_copy != nullptr && hs < G) q_copy[row * RBQ_D + j] = q[row * RBQ_D + j];   // q in mapped host memory: device copy for S7
   const float cqv = c_q ? c_q[row * RBQ_D + j] : 0.0f;
   const float ckv = c_k[(size_t)bg * RBQ_D + j];
   if (rot_kind == RBQ_ROT_DENSE && threadIdx.x == 0) {   // P -> shared memory by ONE bulk copy (TMA); awaited just before the rotation
@@ -228,7 +229,7 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
 
 }  // namespace
 
-int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, cudaStream_t s) {
+int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t s) {
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   RbqQConst* qc = reinterpret_cast<RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
   uint32_t* rk = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax);
@@ -242,10 +243,10 @@ int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t*
   }
   if (ctx->cfg.q_dtype == RBQ_BF16)
     query_kernel<<<BG, threads, smem, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk);
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk, (__nv_bfloat16*)q_copy);
   else
     query_kernel<<<BG, threads, smem, s>>>((const float*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,
-                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk);
+                                           ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, rk, (float*)q_copy);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
