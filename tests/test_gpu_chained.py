@@ -232,6 +232,20 @@ def test_decode_step_host_buffers(orc, rot128):
     c.decode_step(q_host.cuda(), 0.9, out)
     torch.cuda.synchronize()
     assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+    # new query values in the SAME pinned buffer (what a decode loop does): the replayed graph must read them afresh
+    from paper_2606_31519_b200 import synth
+    q_new = torch.from_numpy(synth.query_pool(w, 2)[1]).to(torch.bfloat16)
+    q_host.copy_(q_new)
+    c.decode_step_host(q_host, 0.9, out_host, stream=side)
+    side.synchronize()
+    c.decode_step(q_new.cuda(), 0.9, out)
+    torch.cuda.synchronize()
+    assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+    assert not (out_host.numpy() == outs[0].numpy()).all()
+    q_host.copy_(torch.from_numpy(w.q).to(torch.bfloat16))
+    c.decode_step_host(q_host, 0.9, out_host, stream=side)
+    side.synchronize()
+    assert (out_host.numpy().view(np.uint32) == outs[0].numpy().view(np.uint32)).all()
     # pageable host buffers take the staged path (pinned ones receive the result straight from the S7 merge)
     q_page = torch.from_numpy(w.q).to(torch.bfloat16).clone()
     out_page = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32)
