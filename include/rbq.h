@@ -17,7 +17,7 @@
  *     memory (rbq_index.n_indexed / n_total), so no host read-back happens inside a decode step.
  *   - Layouts are row-major and contiguous except K/V, which carry element strides.  head_dim must
  *     be 128 (64/256: RBQ_ERR_UNSUPPORTED).  n_q_heads must be a multiple of n_kv_heads, with
- *     group size G = n_q_heads/n_kv_heads in {1, 2, 4, 8}.  Inputs are assumed finite.
+ *     group size G = n_q_heads/n_kv_heads in {1, 2, 4} (8: RBQ_ERR_UNSUPPORTED).  Inputs are assumed finite.
  *   - There is no CPU fallback and no backend dispatch: without a CUDA device every compute call
  *     fails with RBQ_ERR_CUDA.
  *
@@ -96,8 +96,14 @@ int rbq_destroy(rbq_ctx* ctx);
 /* Bytes of device scratch the calls below need for this config (query constants, Top-p state,
  * split-K attention partials, scores of the fused step).                                       */
 int rbq_workspace_bytes(const rbq_ctx* ctx, size_t* bytes);
-/* `dev` must stay valid and 256-byte aligned until rbq_destroy or the next rbq_set_workspace.  */
+/* `dev` must stay valid and 256-byte aligned until rbq_destroy or the next rbq_set_workspace.  Setup call: clears the
+ * 4-byte device status word with a blocking cudaMemset and drops the CUDA graph of rbq_decode_step_host, if any.      */
 int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes);
+/* Sticky device-side status bits.  RBQ_FLAG_APPEND_OVERFLOW: an rbq_append_tokens call asked for rows beyond max_tokens;
+ * those rows were dropped and n_total clamped to max_tokens (nothing was written out of bounds).  BLOCKS: copies the
+ * word to flags_host on `stream` and synchronises that stream (like rbq_profile_read, not part of a decode step).     */
+#define RBQ_FLAG_APPEND_OVERFLOW 1u
+int rbq_status_flags(rbq_ctx* ctx, uint32_t* flags_host, void* stream);
 const char* rbq_last_error(const rbq_ctx* ctx);
 
 /* ---- S1  Alg.1 index construction (L106-147, L149-151, L485-487) ---------------------------- */
@@ -112,7 +118,9 @@ int rbq_encode_keys(rbq_ctx* ctx, const rbq_kv* cache, const int32_t* seq_lens, 
  * `stream` waits for it and n_indexed += flushed; (2) rows are copied to cache rows
  * [n_total, n_total+n_new), n_total += n_new; (3) if pending >= W, the oldest floor(pending/W)*W
  * pending rows are encoded with the frozen c_k on `side_stream` (ordered after the copy by an
- * event); they stay pending until the next rbq_append_tokens call.  side_stream may equal stream. */
+ * event); they stay pending until the next rbq_append_tokens call.  side_stream may equal stream.
+ * Every sequence of the batch appends the same n_new rows per call (the pending count is uniform over the batch and
+ * is shadowed on the host); rows that would exceed max_tokens are dropped and flagged (rbq_status_flags).            */
 int rbq_append_tokens(rbq_ctx* ctx, const void* k_new, const void* v_new, int32_t n_new,
                       rbq_kv* cache, rbq_index* idx, void* stream, void* side_stream);
 

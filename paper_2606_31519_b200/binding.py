@@ -28,7 +28,7 @@ RBQ_CK_GIVEN = 1
 EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspace", "rbq_last_error",
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
            "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_topp_select_alg3", "rbq_sparse_attention",
-           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read"]
+           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags"]
 N_STAGES = 5
 STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather"]
 
@@ -83,6 +83,7 @@ def load():
         "rbq_decode_step_host": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), f32, vp, vp], C.c_int),
         "rbq_profile_enable": ([vp, C.c_int], C.c_int),
         "rbq_profile_read": ([vp, C.POINTER(C.c_float), C.POINTER(i32)], C.c_int),
+        "rbq_status_flags": ([vp, C.POINTER(u32), vp], C.c_int),
     }
     for name, (args, res) in sig.items():
         fn = getattr(lib, name)
@@ -213,6 +214,13 @@ def rbq_profile_read(ctx):
     return dict(zip(STAGE_NAMES, [float(x) for x in ms])), n.value
 
 
+def rbq_status_flags(ctx, stream=None) -> int:
+    """Blocks: the sticky device status word (RBQ_FLAG_APPEND_OVERFLOW = 1)."""
+    f = C.c_uint32()
+    _check(ctx, load().rbq_status_flags(ctx, C.byref(f), _stream(stream)), "rbq_status_flags")
+    return int(f.value)
+
+
 # ---- convenience bundle ----------------------------------------------------------------------------
 class RaBitQCache:
     """Context + workspace + caller-owned tensors (K/V cache, index) for one attention layer."""
@@ -309,6 +317,9 @@ class RaBitQCache:
 
     def launch_count(self):
         return rbq_launch_count(self.ctx)
+
+    def status_flags(self, stream=None):
+        return rbq_status_flags(self.ctx, stream)
 
     def profile_enable(self, on=True):
         rbq_profile_enable(self.ctx, on)

@@ -27,6 +27,7 @@ void layout_workspace(rbq_ctx* c) {
   c->off_stage_q = take(rows * RBQ_D * sizeof(float));
   c->off_stage_out = take(rows * RBQ_D * sizeof(float));
   c->off_centroid = take(B * Hkv * 64 * RBQ_D * sizeof(double));
+  c->off_flags = take(sizeof(uint32_t));
   c->total_bytes = off;
 }
 
@@ -81,7 +82,7 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
   for (int d : {cfg->kv_dtype, cfg->q_dtype, cfg->out_dtype})
     if (d != RBQ_F32 && d != RBQ_BF16) return RBQ_ERR_INVALID_ARG;
   if (cfg->rot_kind != RBQ_ROT_DENSE && cfg->rot_kind != RBQ_ROT_WH) return RBQ_ERR_INVALID_ARG;
-  // tensor-core rotation: built for bf16 K/V and the dense rotation (the WH path is already a fast transform)
+  // tensor-core rotation: built for bf16 K/V (either rotation kind: the WH rotation runs as its dense matrix)
   if (cfg->enc_mode == RBQ_ENC_FAST && cfg->kv_dtype != RBQ_BF16) return RBQ_ERR_UNSUPPORTED;
   if (cfg->enc_mode != RBQ_ENC_EXACT && cfg->enc_mode != RBQ_ENC_FAST) return RBQ_ERR_INVALID_ARG;
   if (!cfg->rot || !(cfg->sm_scale >= 0.0f)) return RBQ_ERR_INVALID_ARG;
@@ -128,8 +129,23 @@ int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes) {
   RBQ_CTX(ctx);
   if (!dev || (reinterpret_cast<uintptr_t>(dev) & 255u)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   if (bytes < ctx->total_bytes) RBQ_FAIL(ctx, RBQ_ERR_WORKSPACE, "workspace too small: %zu < %zu", bytes, ctx->total_bytes);
+  // a captured host-step graph holds pointers into the old workspace: drop it
+  if (ctx->host_graph_state == 1) { cudaGraphExecDestroy(ctx->host_graph); ctx->host_graph = nullptr; }
+  if (ctx->host_graph_state > 0) ctx->host_graph_state = 0;
   ctx->ws = dev;
   ctx->ws_bytes = bytes;
+  // the sticky status word starts clear (setup call: a blocking 4-byte memset on the legacy stream)
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_flags, 0, sizeof(uint32_t)));
+  return RBQ_OK;
+}
+
+int rbq_status_flags(rbq_ctx* ctx, uint32_t* flags_host, void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(need_ws(ctx));
+  if (!flags_host) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "flags_host null");
+  cudaStream_t s = (cudaStream_t)stream;
+  RBQ_CUDA_OK(ctx, cudaMemcpyAsync(flags_host, ws_ptr<char>(ctx, ctx->off_flags), sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+  RBQ_CUDA_OK(ctx, cudaStreamSynchronize(s));
   return RBQ_OK;
 }
 
@@ -345,9 +361,12 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
   // One CPU-side launch per step instead of seven: the sequence is captured once per argument set and replayed.
   // Not on the legacy default stream (capture is illegal there), not while stage profiling is on (events between kernels).
   if (ctx->prof_on || ctx->host_graph_state < 0 || s == nullptr || s == cudaStreamLegacy || s == cudaStreamPerThread) return direct();
-  decltype(ctx->host_key) key = {q_host, out_host, cache->k, cache->v, idx->codes, idx->f_scale, idx->f_bias, idx->c_k, idx->c_q,
-                                 idx->n_indexed, idx->n_total, stream, (long long)cache->stride_b, (long long)cache->stride_h,
-                                 (long long)cache->stride_t, p};
+  decltype(ctx->host_key) key;
+  memset(&key, 0, sizeof(key));                               // padding bytes take part in the memcmp below
+  key.q = q_host; key.out = out_host; key.k = cache->k; key.v = cache->v; key.codes = idx->codes; key.f_scale = idx->f_scale;
+  key.f_bias = idx->f_bias; key.c_k = idx->c_k; key.c_q = idx->c_q; key.n_indexed = idx->n_indexed; key.n_total = idx->n_total;
+  key.stream = stream; key.ws = ctx->ws; key.sb = (long long)cache->stride_b; key.sh = (long long)cache->stride_h;
+  key.st = (long long)cache->stride_t; key.p = p;
   if (ctx->host_graph_state == 1 && memcmp(&key, &ctx->host_key, sizeof(key)) == 0) {
     RBQ_CUDA_OK(ctx, cudaGraphLaunch(ctx->host_graph, s));
     ctx->launches += ctx->host_graph_launches;

@@ -730,11 +730,7 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
   if (kbf && qbf) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(attn_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GA_SMEM));
-      attr_set = true;
-    }
+    RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_GATHER, attn_gather_kernel, GA_SMEM);
     const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the arrival count uses one thread per CTA
     RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_gather_kernel, dim3(nc), dim3(GA_THREADS), (size_t)GA_SMEM, s, (const __nv_bfloat16*)q,
                                     (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st,

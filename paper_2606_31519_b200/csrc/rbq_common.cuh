@@ -43,7 +43,10 @@ struct rbq_ctx {
   size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_gdone, off_rowmax, off_part,
       off_stage_q, off_stage_out, off_centroid, total_bytes;
   cudaEvent_t ev_copy, ev_flush;
-  int pending;               // host shadow of n_total - n_indexed (uniform over the batch)
+  unsigned attr_mask;        // kernels whose MaxDynamicSharedMemorySize was set for THIS context's device (RBQ_ATTR_*)
+  size_t attr_topp_smem;     // largest dynamic shared memory size set for the Top-p kernels so far
+  size_t off_flags;          // device status word (RBQ_FLAG_*), sticky
+  int pending;               // host shadow of n_total - n_indexed (uniform over the batch: every sequence appends n_new rows per call)
   int in_flight;             // rows encoded by an enqueued flush, not yet committed
   long long launches;
   int prof_on, prof_steps;                                   // stage timing (rbq_profile_*)
@@ -53,10 +56,14 @@ struct rbq_ctx {
   cudaGraphExec_t host_graph;
   int host_graph_state;      // 0 = none yet, 1 = valid, -1 = capture not possible on this stream / driver: direct launches
   int host_graph_launches;   // kernel launches one replay stands for
-  struct { const void *q, *out, *k, *v, *codes, *f_scale, *f_bias, *c_k, *c_q, *n_indexed, *n_total, *stream;
+  struct { const void *q, *out, *k, *v, *codes, *f_scale, *f_bias, *c_k, *c_q, *n_indexed, *n_total, *stream, *ws;
            long long sb, sh, st; float p; } host_key;
   char err[256];
 };
+
+// per-context "function attribute set" bits (the attribute is per device; a context lives on one device)
+enum { RBQ_ATTR_QUERY = 1u, RBQ_ATTR_ENC_EXACT = 2u, RBQ_ATTR_ENC_FAST = 4u, RBQ_ATTR_GATHER = 8u, RBQ_ATTR_ALG3 = 16u,
+       RBQ_ATTR_EST = 32u, RBQ_ATTR_FUSED = 64u };
 
 #define RBQ_FAIL(ctx, code, ...)                                   \
   do {                                                             \
@@ -117,6 +124,19 @@ inline cudaError_t rbq_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block,
   cfg.attrs = at; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
+
+// MaxDynamicSharedMemorySize is a per-device attribute of a function: it is set once per CONTEXT (a context lives on the
+// device that was current at rbq_create), always to the same per-kernel maximum, so that contexts with different
+// configurations on one device never lower each other's limit.
+#define RBQ_SET_SMEM_ATTR(ctx, bit, func, bytes)                                                          \
+  do {                                                                                                    \
+    if (!((ctx)->attr_mask & (bit))) {                                                                    \
+      RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes))); \
+      (ctx)->attr_mask |= (bit);                                                                          \
+    }                                                                                                     \
+  } while (0)
+#define RBQ_MAX_DYN_SMEM (227 * 1024)
+
 
 // ---- kernel launchers (defined in the .cu files, called from rbq_api.cu) ------------------------
 int rbq_launch_centroid(rbq_ctx*, const RbqKV&, const int32_t* seq_lens, float* c_k, cudaStream_t);

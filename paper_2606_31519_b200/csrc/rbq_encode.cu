@@ -119,7 +119,7 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
 
   const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
   const int tb = t_begin ? t_begin[b] : 0;
-  const int cnt = t_count ? t_count[b] : fixed_count;
+  const int cnt = min(t_count ? t_count[b] : fixed_count, Lcap - tb);   // never past the capacity (append overflow, rbq_status_flags)
   const int tile0 = blockIdx.x * ENC_TOK;
   if (tile0 >= cnt) return;
   const int ntok = min(ENC_TOK, cnt - tile0);
@@ -238,22 +238,56 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
   }
 }
 
-// f_bias[b][hq][t] = <c_q[b][hq], k_t>, fma chain i ascending.  Parity-only path.
+// f_bias[b][hq][t] = <c_q[b][hq], k_t> ("<c_q,k> ... can all be pre-calculated"), one canonical fma chain
+// per (token, query head), i ascending (R1) -- bit-identical to the oracle in both encode modes.
+// grid = (ceil(max_count / FB_TOK), B*Hkv), FB_TOK threads: the K rows of FB_TOK tokens are staged in shared memory with
+// coalesced 16-byte loads (padded rows: conflict-free per-token reads), c_q of the group's G heads next to them; a
+// thread owns one token and runs the G chains side by side (each staged k_i feeds G independent FMAs).
+constexpr int FB_TOK = 128;
+constexpr int FB_XS = RBQ_D + 1;
+
 template <typename T>
-__global__ void fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
-                             const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count,
-                             int fixed_count, int Hq, int Hkv, int Lcap, const float* __restrict__ c_q,
-                             float* __restrict__ f_bias) {
-  const int bh = blockIdx.y, b = bh / Hq, h = bh % Hq, g = h / (Hq / Hkv);
+__global__ void __launch_bounds__(FB_TOK)
+fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st, const int32_t* __restrict__ t_begin,
+             const int32_t* __restrict__ t_count, int fixed_count, int Hq, int Hkv, int Lcap, const float* __restrict__ c_q,
+             float* __restrict__ f_bias) {
+  extern __shared__ __align__(16) float fb_smem[];
+  float* ks = fb_smem;                              // [FB_TOK][FB_XS]
+  float* cq = ks + FB_TOK * FB_XS;                  // [G][D]
+  const int G = Hq / Hkv;
+  const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
   const int tb = t_begin ? t_begin[b] : 0;
-  const int cnt = t_count ? t_count[b] : fixed_count;
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= cnt) return;
-  const T* k = K + (long long)b * sb + (long long)g * sh + (long long)(tb + r) * st;
-  const float* cq = c_q + (size_t)bh * RBQ_D;
-  float acc = 0.0f;
-  for (int i = 0; i < RBQ_D; ++i) acc = fmaf(cq[i], rbq_ld_elem(k, i), acc);
-  f_bias[(size_t)bh * Lcap + tb + r] = acc;
+  const int cnt = min(t_count ? t_count[b] : fixed_count, Lcap - tb);
+  const int tile0 = blockIdx.x * FB_TOK;
+  if (tile0 >= cnt) return;
+  const int ntok = min(FB_TOK, cnt - tile0);
+  const int tid = threadIdx.x;
+  const T* base = K + (long long)b * sb + (long long)g * sh + (long long)(tb + tile0) * st;
+  for (int e = tid; e < FB_TOK * RBQ_D / 8; e += FB_TOK) {
+    const int wv = e >> 5, ln = e & 31;
+    const int r = (wv >> 2) * 8 + (ln >> 2), d = ((wv & 3) * 4 + (ln & 3)) * 8;
+    float v[8];
+    if (r < ntok) rbq_ld8(base + (long long)r * st + d, v);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) ks[r * FB_XS + d + k] = (r < ntok) ? v[k] : 0.0f;
+  }
+  for (int e = tid; e < G * RBQ_D; e += FB_TOK) cq[e] = c_q[((size_t)b * Hq + (size_t)g * G) * RBQ_D + e];
+  __syncthreads();
+  if (tid >= ntok) return;
+  const float* kr = ks + tid * FB_XS;
+  float acc[RBQ_MAX_G];
+#pragma unroll
+  for (int h = 0; h < RBQ_MAX_G; ++h) acc[h] = 0.0f;
+#pragma unroll 8
+  for (int i = 0; i < RBQ_D; ++i) {
+    const float kv = kr[i];
+#pragma unroll
+    for (int h = 0; h < RBQ_MAX_G; ++h)
+      if (h < G) acc[h] = fmaf(cq[h * RBQ_D + i], kv, acc[h]);
+  }
+#pragma unroll
+  for (int h = 0; h < RBQ_MAX_G; ++h)
+    if (h < G) f_bias[((size_t)b * Hq + (size_t)g * G + h) * Lcap + tb + tile0 + tid] = acc[h];
 }
 
 __global__ void set_counts_kernel(const int32_t* __restrict__ seq_lens, int32_t* n_indexed, int32_t* n_total, int B) {
@@ -261,26 +295,35 @@ __global__ void set_counts_kernel(const int32_t* __restrict__ seq_lens, int32_t*
   if (b < B) { n_indexed[b] = seq_lens[b]; n_total[b] = seq_lens[b]; }
 }
 
-// S2: commit an earlier flush (n_indexed += commit), copy n_new rows per (b, kv head) to the cache
-// tail [n_total, n_total + n_new), then n_total += n_new (done by the last block via a second launch
-// of this kernel family: see append_bump_kernel).  16-byte vector copies.
+// S2: commit an earlier flush (n_indexed += commit), copy n_new rows per (b, kv head) to the cache tail
+// [n_total, n_total + n_new), then n_total += n_new (append_bump_kernel, launched after the copy).  16-byte vector copies.
+// Rows that would land at or beyond the capacity Lcap are dropped and the sticky RBQ_FLAG_APPEND_OVERFLOW bit is set
+// (rbq_status_flags): the counts never exceed Lcap, so no later stage indexes past an allocation.
 __global__ void append_copy_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, int n_new,
                                    int row_vec, char* __restrict__ kc, char* __restrict__ vc, long long sb_bytes,
-                                   long long sh_bytes, long long st_bytes, int Hkv,
+                                   long long sh_bytes, long long st_bytes, int Hkv, int Lcap,
                                    const int32_t* __restrict__ n_total) {
   const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n_new * row_vec) return;
   const int r = e / row_vec, c = e % row_vec;
-  const long long dst = (long long)b * sb_bytes + (long long)g * sh_bytes + (long long)(n_total[b] + r) * st_bytes + c * 16;
+  const int t = n_total[b] + r;
+  if (t >= Lcap) return;
+  const long long dst = (long long)b * sb_bytes + (long long)g * sh_bytes + (long long)t * st_bytes + c * 16;
   const size_t src = ((size_t)bg * n_new + r) * row_vec + c;
   *reinterpret_cast<uint4*>(kc + dst) = k_new[src];
   *reinterpret_cast<uint4*>(vc + dst) = v_new[src];
 }
 
-__global__ void append_bump_kernel(int32_t* n_indexed, int32_t* n_total, int B, int commit, int n_new) {
+__global__ void append_bump_kernel(int32_t* n_indexed, int32_t* n_total, int B, int commit, int n_new, int Lcap,
+                                   uint32_t* __restrict__ flags) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b < B) { n_indexed[b] += commit; n_total[b] += n_new; }
+  if (b < B) {
+    int nt = n_total[b] + n_new;
+    if (nt > Lcap) { nt = Lcap; atomicOr(flags, RBQ_FLAG_APPEND_OVERFLOW); }
+    n_total[b] = nt;
+    n_indexed[b] = min(n_indexed[b] + commit, nt);
+  }
 }
 
 }  // namespace
@@ -306,23 +349,27 @@ static int launch_encode_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin
                            int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
   const size_t smem = (size_t)(ENC_TOK * XS + ENC_TOK + (ROT == RBQ_ROT_DENSE ? RBQ_D * RBQ_D : RBQ_D)) * sizeof(float);
   auto kern = encode_kernel<T, ROT>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
+  const unsigned bit = RBQ_ATTR_ENC_EXACT << (8 + 16 + (sizeof(T) == 2 ? 0 : 2) + (ROT == RBQ_ROT_DENSE ? 0 : 1));   // one bit per instantiation
+  RBQ_SET_SMEM_ATTR(ctx, bit, kern, smem);
   dim3 grid((max_count + ENC_TOK - 1) / ENC_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
   kern<<<grid, ENC_THREADS, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
                                        ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->cfg.rot, idx->c_k,
                                        idx->codes, idx->f_scale);
   RBQ_LAUNCH_OK(ctx);
-  if (idx->c_q) {
-    dim3 g2((max_count + 127) / 128, ctx->cfg.batch * ctx->cfg.n_q_heads);
-    fbias_kernel<T><<<g2, 128, 0, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
-                                       ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, idx->c_q,
-                                       idx->f_bias);
-    RBQ_LAUNCH_OK(ctx);
-  }
+  return RBQ_OK;
+}
+
+// f_bias = <c_q, k> for the same token ranges (either encode mode)
+template <typename T>
+static int launch_fbias_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count, int fixed_count,
+                          int max_count, const rbq_index* idx, cudaStream_t s) {
+  const size_t smem = (size_t)(FB_TOK * FB_XS + ctx->G * RBQ_D) * sizeof(float);
+  auto kern = fbias_kernel<T>;
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_EXACT << (8 + 16 + 4 + (sizeof(T) == 2 ? 0 : 1)), kern, smem);
+  dim3 grid((max_count + FB_TOK - 1) / FB_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
+  kern<<<grid, FB_TOK, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count, ctx->cfg.n_q_heads,
+                                  ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, idx->c_q, idx->f_bias);
+  RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
@@ -330,11 +377,15 @@ int rbq_launch_encode(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, con
                       int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
   if (max_count <= 0) return RBQ_OK;
   const bool bf = ctx->cfg.kv_dtype == RBQ_BF16, wh = ctx->cfg.rot_kind == RBQ_ROT_WH;
-  if (ctx->cfg.enc_mode == RBQ_ENC_FAST) return rbq_launch_encode_fast(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  if (bf && !wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  if (bf && wh) return launch_encode_t<__nv_bfloat16, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  if (!bf && !wh) return launch_encode_t<float, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  return launch_encode_t<float, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  int rc;
+  if (ctx->cfg.enc_mode == RBQ_ENC_FAST) rc = rbq_launch_encode_fast(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  else if (bf && !wh) rc = launch_encode_t<__nv_bfloat16, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  else if (bf && wh) rc = launch_encode_t<__nv_bfloat16, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  else if (!bf && !wh) rc = launch_encode_t<float, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  else rc = launch_encode_t<float, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  if (rc != RBQ_OK || !idx->c_q) return rc;
+  return bf ? launch_fbias_t<__nv_bfloat16>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s)
+            : launch_fbias_t<float>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
 }
 
 int rbq_launch_set_counts(rbq_ctx* ctx, const int32_t* seq_lens, int32_t* n_indexed, int32_t* n_total, cudaStream_t s) {
@@ -351,10 +402,11 @@ int rbq_launch_append_copy(rbq_ctx* ctx, const void* k_new, const void* v_new, i
     dim3 grid((n_new * row_vec + 127) / 128, ctx->cfg.batch * ctx->cfg.n_kv_heads);
     append_copy_kernel<<<grid, 128, 0, s>>>((const uint4*)k_new, (const uint4*)v_new, n_new, row_vec,
                                             (char*)kv.k, (char*)kv.v, kv.sb * esz, kv.sh * esz, kv.st * esz,
-                                            ctx->cfg.n_kv_heads, n_total);
+                                            ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, n_total);
     RBQ_LAUNCH_OK(ctx);
   }
-  append_bump_kernel<<<(ctx->cfg.batch + 127) / 128, 128, 0, s>>>(n_indexed, n_total, ctx->cfg.batch, commit, n_new);
+  append_bump_kernel<<<(ctx->cfg.batch + 127) / 128, 128, 0, s>>>(n_indexed, n_total, ctx->cfg.batch, commit, n_new, ctx->cfg.max_tokens,
+                                                                  reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_flags));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

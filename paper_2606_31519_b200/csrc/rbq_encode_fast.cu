@@ -40,7 +40,7 @@ constexpr int T5_TOK = 128;
 constexpr int T5_LBO = 2048 + 32;                            // bytes between K chunks (8 elements) of an operand tile
 constexpr int T5_SBO = 128;                                  // bytes between 8-row groups
 constexpr int T5_TILE = 16 * T5_LBO;                         // one 128 x 128 bf16 operand tile
-constexpr int T5_SMEM = (2 + 2 * T5_GROUPS) * T5_TILE + RBQ_D * 4 + T5_GROUPS * (2 * T5_TOK * 4 + T5_TOK * 16) + 64;   // B_hi B_lo | per group A_hi A_lo | c_k | per group n2, exchange | misc
+constexpr int T5_SMEM = (2 + 2 * T5_GROUPS) * T5_TILE + RBQ_D * 4 + T5_GROUPS * (2 * T5_TOK * 4 + 2 * T5_TOK * 16) + 64;   // B_hi B_lo | per group A_hi A_lo | c_k | per group n2 x 2, exchange x 2 (tile parity) | misc
 constexpr uint32_t T5_IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(RBQ_D >> 3) << 17) | ((uint32_t)(T5_TOK >> 4) << 24);
 
 __device__ __forceinline__ uint64_t t5_desc(uint32_t smem_addr) {
@@ -85,15 +85,17 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
   unsigned char* s_al = s_ah + T5_TILE;
   float* s_ck = reinterpret_cast<float*>(t5_smem + (2 + 2 * T5_GROUPS) * T5_TILE);
   float* s_n2 = s_ck + RBQ_D + grp * 2 * T5_TOK;                // two buffers (tile parity)
-  uint4* s_ex = reinterpret_cast<uint4*>(s_ck + RBQ_D + T5_GROUPS * 2 * T5_TOK) + grp * T5_TOK;   // per row: {l1 bits, word 2, word 3, -} of the upper column half
-  uint64_t* s_bar0 = reinterpret_cast<uint64_t*>(reinterpret_cast<uint4*>(s_ck + RBQ_D + T5_GROUPS * 2 * T5_TOK) + T5_GROUPS * T5_TOK);
+  // per row: {l1 bits, word 2, word 3, -} of the upper column half; two buffers (tile parity), so that the hc == 1 warps of
+  // tile t + 1 never overwrite what a slow hc == 0 warp of tile t has not read yet (one group barrier per tile)
+  uint4* s_ex = reinterpret_cast<uint4*>(s_ck + RBQ_D + T5_GROUPS * 2 * T5_TOK) + grp * 2 * T5_TOK;
+  uint64_t* s_bar0 = reinterpret_cast<uint64_t*>(reinterpret_cast<uint4*>(s_ck + RBQ_D + T5_GROUPS * 2 * T5_TOK) + T5_GROUPS * 2 * T5_TOK);
   uint64_t* s_bar = s_bar0 + grp;                             // accumulator ready (tcgen05.commit)
   uint64_t* s_full = s_bar0 + T5_GROUPS + grp;                // A operands written (all threads of the group arrive)
   uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_bar0 + 2 * T5_GROUPS);
 
   const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
   const int tb = t_begin ? t_begin[b] : 0;
-  const int cnt = t_count ? t_count[b] : fixed_count;
+  const int cnt = min(t_count ? t_count[b] : fixed_count, Lcap - tb);   // never past the capacity (append overflow, rbq_status_flags)
   if ((int)blockIdx.x * T5_GROUPS * T5_TOK >= cnt) return;
   const int tid = threadIdx.x % T5_GTHREADS, warp = tid >> 5, lane = tid & 31;   // indices inside the group
 
@@ -218,10 +220,11 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
     for (int j = 31; j >= 0; --j) { l1 += fabsf(__uint_as_float(y[j])); w1 = __funnelshift_l(y[j], w1, 1); }
     w0 = ~w0;
     w1 = ~w1;
-    if (hc == 1) s_ex[r] = make_uint4(__float_as_uint(l1), w0, w1, 0u);
+    uint4* ex_buf = s_ex + buf * T5_TOK;
+    if (hc == 1) ex_buf[r] = make_uint4(__float_as_uint(l1), w0, w1, 0u);
     t5_group_sync(grp);
     if (hc == 0 && r < ntok) {
-      const uint4 ex = s_ex[r];
+      const uint4 ex = ex_buf[r];
       const float l1t = l1 + __uint_as_float(ex.x);
       const size_t tok = (size_t)bg * Lcap + tb + tile0 + r;
       const bool zero = l1t == 0.0f;
@@ -280,11 +283,7 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
 
 int rbq_launch_encode_fast(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count, int fixed_count,
                            int max_count, const rbq_index* idx, cudaStream_t s) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(encode_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, T5_SMEM));
-    attr_set = true;
-  }
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_FAST, encode_tc5_kernel, T5_SMEM);
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   const int tiles = (max_count + T5_GROUPS * T5_TOK - 1) / (T5_GROUPS * T5_TOK);
   int gx = ctx->sm_count / BG;                                // one CTA per SM, a single wave; each CTA loops over its tiles

@@ -235,11 +235,10 @@ int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t*
   uint32_t* rk = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax);
   const int threads = max(256, ctx->G * RBQ_D);
   const size_t smem = ctx->cfg.rot_kind == RBQ_ROT_DENSE ? (size_t)RBQ_D * RBQ_D * sizeof(float) : 0;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(ctx->attr_mask & RBQ_ATTR_QUERY)) {
     RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(query_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_D * RBQ_D * 4));
     RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(query_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_D * RBQ_D * 4));
-    attr_set = true;
+    ctx->attr_mask |= RBQ_ATTR_QUERY;
   }
   if (ctx->cfg.q_dtype == RBQ_BF16)
     query_kernel<<<BG, threads, smem, s>>>((const __nv_bfloat16*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind,

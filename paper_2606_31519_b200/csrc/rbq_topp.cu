@@ -613,10 +613,9 @@ int launch_cs(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, con
   const int s_cap = ((((ctx->cfg.max_tokens + CS - 1) / CS) + 31) & ~31) + 32;
   const size_t smem = TP_OFF_SC + (size_t)s_cap * 4;
   auto kern = topp_kernel<CS>;
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
+  if (!(ctx->attr_mask & (0x100u << CS))) {                    // one bit per instantiation (CS = 1, 2, 4, 8)
+    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_MAX_DYN_SMEM));
+    ctx->attr_mask |= 0x100u << CS;
   }
   dim3 grid(CS, rows);
   RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, grid, dim3(TP_THREADS), smem, s, scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads,

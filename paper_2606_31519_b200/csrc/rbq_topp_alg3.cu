@@ -185,11 +185,7 @@ int rbq_launch_topp_alg3(rbq_ctx* ctx, const float* scores, const int32_t* n_ind
   const size_t smem = (size_t)s_cap * sizeof(double);
   if (smem > 200 * 1024 || s_cap > 32 * 2 * A3_THREADS)
     RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "rbq_topp_select_alg3: max_tokens %d exceeds the cluster-resident limit", ctx->cfg.max_tokens);
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(topp_alg3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
-  }
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ALG3, topp_alg3_kernel, 200 * 1024);
   topp_alg3_kernel<<<dim3(A3_CS, rows), A3_THREADS, smem, s>>>(scores, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, (double)p,
                                                               sel_idx, sel_cnt, iters);
   RBQ_LAUNCH_OK(ctx);

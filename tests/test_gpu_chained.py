@@ -185,6 +185,76 @@ def test_append_flush_enc_fast(orc, rot128):
     c.close()
 
 
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+def test_encode_fast_with_cq(orc, rot128, kind):
+    """RBQ_ENC_FAST with a query centroid: f_bias = <c_q, k> must be written by rbq_encode_keys AND by
+    the lazy flush in the tensor-core encode mode too, bit-identical to the oracle's canonical chain (it does not go
+    through the rotation); the logits of the fused path then carry the Eq.2 term <c_q, k>."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb, synth
+    W = 64
+    w = U.workload(1, L=3001, with_cq=True, extra_cap=192)
+    rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, kind, rot, W, c_q=w.c_q)
+    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(np.ascontiguousarray(rot, dtype=np.float32)), flush_tokens=W,
+                       rot_kind=kind, enc_mode=rb.RBQ_ENC_FAST, with_cq=True)
+    c.K.copy_(U.to_dev(w.K, torch.bfloat16))
+    c.V.copy_(U.to_dev(w.V, torch.bfloat16))
+    c.c_q.copy_(U.to_dev(w.c_q))
+    c.f_bias.fill_(float("nan"))
+    c.encode_keys(U.to_dev(w.seq_lens))
+    for s_, n_new in enumerate([70, 60]):                        # two flushes (64 rows each), the second commits the first
+        k_new, v_new = synth.append_rows(1, 300 + s_, w.B, w.Hkv, n_new)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16))
+    torch.cuda.synchronize()
+    fb = c.f_bias.cpu().numpy()
+    n = int(lazy.n_indexed[0]) + lazy.in_flight
+    assert n == 3001 + 128
+    assert (fb[0, :, :n].view(np.uint32) == lazy.f_bias[0, :, :n].view(np.uint32)).all(), "f_bias differs in RBQ_ENC_FAST"
+    # logits through the GPU's own (guard-band) index: compare with the oracle's logits on the GPU's codes / factors
+    scores = c.new_scores()
+    q = U.to_dev(w.q, torch.bfloat16)
+    c.estimate_scores(q, scores)
+    torch.cuda.synchronize()
+    ni = c.n_indexed.cpu().numpy()
+    ref, _, _, _ = orc.estimate_scores(w.q, c.codes.cpu().numpy().view(np.uint32), c.f_scale.cpu().numpy(), fb, c.c_k.cpu().numpy(),
+                                       w.c_q, ni, kind, rot, U.SM_SCALE)
+    U.assert_logits_close(scores.cpu().numpy(), ref, ni, w.Hq)
+    c.close()
+
+
+def test_append_beyond_capacity_is_dropped_and_flagged(orc, rot128):
+    """Appending past max_tokens: the extra rows are dropped, n_total is clamped to Lcap, the sticky status bit is
+    set, nothing outside the sequence's own cache rows is touched, and a decode step still runs on the clamped state."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    w = U.workload(3, L=500, B=2)                       # Lcap = 512 (seq_lens <= 500)
+    c = U.make_cache(w, rot128[0], flush_tokens=8)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    assert c.status_flags() == 0
+    guard_k = c.K.clone()
+    room = int(w.Lcap - w.seq_lens.max())
+    k_new, v_new = synth.append_rows(3, 7, w.B, w.Hkv, room + 24)
+    c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16))
+    out = c.new_out()
+    c.decode_step(U.to_dev(w.q, torch.bfloat16), 0.9, out)
+    torch.cuda.synchronize()
+    assert c.status_flags() == 1
+    nt = c.n_total.cpu().numpy()
+    assert (nt <= w.Lcap).all() and nt.max() == w.Lcap and (c.n_indexed.cpu().numpy() <= nt).all()
+    for b in range(w.B):
+        n0 = int(w.seq_lens[b])
+        m = int(nt[b]) - n0
+        assert (c.K[b, :, :n0] == guard_k[b, :, :n0]).all(), "old rows were overwritten"
+        assert (c.K[b, :, n0:n0 + m].float().cpu().numpy() == k_new[b, :, :m]).all()
+    assert torch.isfinite(out).all()
+    c.append_tokens(U.to_dev(k_new[:, :, :8], torch.bfloat16), U.to_dev(v_new[:, :, :8], torch.bfloat16))   # commits the flush
+    torch.cuda.synchronize()
+    assert (c.n_indexed.cpu().numpy() <= c.n_total.cpu().numpy()).all() and (c.n_total.cpu().numpy() <= w.Lcap).all()
+    c.close()
+
+
 def test_append_many_tokens_per_call(orc, rot128):
     """n_new = 5 per call with W = 8 (flush of whole windows only), and n_new >= W in one call."""
     import torch

@@ -1,0 +1,131 @@
+"""Full-size GPU parity for the configurations BASELINE.json names that the small-case files do not reach
+(VERDICT r1 weak #2): config 1 at L = 32 768 for p in {0.8, 0.9, 0.95}; config 4 at B = 4 x 131 072 keys (index build
+EXACT / FAST x dense / Walsh-Hadamard, then the decode loop across two lazy flushes); and the 8-CTA Top-p cluster with
+16 K scores per CTA and thousands of ties at the boundary.  Expected values come from `oracle/` only.
+"""
+import numpy as np
+import pytest
+
+from tests import gpu_util as U
+from tests.test_gpu_chained import _chained
+from tests.test_gpu_parity import _check_encode_fast
+
+pytestmark = pytest.mark.gpu
+
+ROT_DENSE, ROT_WH = 0, 1
+
+
+@pytest.mark.parametrize("p", [0.8, 0.9, 0.95])
+def test_config1_full_size(orc, rot128, p):
+    """BASELINE config 1 (32 q / 8 KV heads, L = 32 768, bf16) in the launch configuration the bench times: the whole
+    chain against the oracle at every p the config names."""
+    _chained(orc, U.workload(1), rot128[0], ROT_DENSE, p)
+
+
+@pytest.fixture(scope="module")
+def w4():
+    return U.workload(4, extra_cap=192)
+
+
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+def test_config4_encode_exact_full_size(orc, rot128, w4, kind):
+    """Config 4 (i): 4 x 8 x 131 072 bf16 keys, canonical-order encode, dense QR and Walsh-Hadamard: bit for bit."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    w = w4
+    rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
+    o = U.oracle_index(orc, w, rot, kind)
+    c = U.make_cache(w, rot, rot_kind=kind)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    torch.cuda.synchronize()
+    assert np.array_equal(c.c_k.cpu().numpy().view(np.uint32), o["c_k"].view(np.uint32))
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        assert (codes[b, :, :n] == o["codes"][b, :, :n]).all(), f"codes differ (seq {b})"
+        assert (fs[b, :, :n].view(np.uint32) == o["f_scale"][b, :, :n].view(np.uint32)).all(), "f_scale differs"
+    c.close()
+
+
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+def test_config4_encode_fast_full_size(orc, rot128, w4, kind):
+    """Config 4 (i) in RBQ_ENC_FAST (tcgen05 rotation): guard band of SURVEY 8(c) C1 at full size."""
+    from paper_2606_31519_b200 import synth
+    rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
+    _check_encode_fast(orc, rot, w4, kind)
+
+
+def test_config4_decode_loop_full_size(orc, rot128, w4):
+    """Config 4 (ii) at full size: batch 4 x 131 072, W = 64, 130 decode steps with one token per sequence appended per
+    step, the flush encodes on a side stream (two flushes, two commits); counts, outputs and budgets against the oracle's
+    state machine at the steps around each flush, flushed codes bit for bit at the end."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    W, steps = 64, 130
+    w, rot = w4, rot128[0]
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, ROT_DENSE, rot, W)
+    c = U.make_cache(w, rot, flush_tokens=W)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream()
+    pool = synth.query_pool(w, 4)
+    q_dev = [U.to_dev(pool[i], torch.bfloat16) for i in range(4)]
+    out = c.new_out()
+    sel_cnt = c.new_sel()[1]
+    check = {0, W - 1, W, W + 1, 2 * W, steps - 1}
+    for s in range(steps):
+        k_new, v_new = synth.append_rows(4, s, w.B, w.Hkv, 1)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16), stream=main, side_stream=side)
+        c.decode_step(q_dev[s % 4], w.p, out, None, sel_cnt)
+        if s in check:
+            torch.cuda.synchronize()
+            assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all() and (c.n_total.cpu().numpy() == lazy.n_total).all()
+            ref = orc.decode_step(pool[s % 4], lazy.K, lazy.V, lazy.codes, lazy.f_scale, None, lazy.c_k, None, lazy.n_indexed,
+                                  lazy.n_total, ROT_DENSE, rot, w.p, U.SM_SCALE)
+            U.assert_attention_close(out.cpu().numpy(), ref["out"], "bf16")
+            assert np.abs(sel_cnt.cpu().numpy().astype(np.int64) - ref["sel_cnt"]).max() <= max(2, int(0.002 * ref["sel_cnt"].max()))
+    torch.cuda.synchronize()
+    assert c.status_flags() == 0
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    n0 = int(w.seq_lens[0])
+    for b in range(w.B):
+        n = int(lazy.n_indexed[b]) + lazy.in_flight
+        assert n == n0 + 2 * W
+        assert (codes[b, :, n0:n] == lazy.codes[b, :, n0:n]).all()
+    c.close()
+
+
+def test_topp_cluster8_long_slices_and_boundary_ties(orc, rot128):
+    """topp_kernel<8>: B = 1, Hq = 16, L = 131 072 (16 384 scores per CTA), with rows whose boundary value is shared by far
+    more than the 1 024 candidates a row gathers (the cluster-wide radix narrowing at CS = 8), rows of plain Gaussian
+    logits, an all-equal row and a row with one dominant token."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb
+    L, Hq, Hkv = 131072, 16, 4
+    rng = np.random.default_rng(77)
+    scores = (rng.standard_normal((1, Hq, L)) * rng.uniform(0.5, 5.0, (1, Hq, 1))).astype(np.float32)
+    scores[0, 0] = np.round(scores[0, 0] * 2) / 2                # ~10^4 tokens per distinct value
+    scores[0, 1] = np.round(scores[0, 1])
+    scores[0, 2] = 0.75                                           # all equal: the cut is an index
+    scores[0, 3, 4321] = 200.0                                    # one dominant token
+    scores[0, 4, 1000:9000] = scores[0, 4].max() + 1.0            # 8 000 ties at the top
+    c = rb.RaBitQCache(1, Hq, Hkv, L, torch.from_numpy(rot128[0]))
+    n = np.array([L], np.int32)
+    c.n_indexed.copy_(U.to_dev(n))
+    c.n_total.copy_(U.to_dev(n))
+    sc_dev = U.to_dev(scores)
+    for p in (0.5, 0.9):
+        ref_idx, ref_cnt = orc.topp(scores.reshape(Hq, L), np.repeat(n, Hq), p)
+        sel_idx, sel_cnt = c.new_sel()
+        sel_idx.fill_(-1)
+        c.topp_select(sc_dev, p, sel_idx, sel_cnt)
+        torch.cuda.synchronize()
+        idx, cnt = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy()
+        for h in range(Hq):
+            g = idx[0, h, :cnt[0, h]]
+            assert (np.diff(g) > 0).all() and g.min() >= 0 and g.max() < L
+            U.assert_topp_row(scores[0, h], g, ref_idx[h, :ref_cnt[h]], p)
+        k = int(ref_cnt[2])                                       # exact ties: the lowest indices are kept (R8)
+        assert cnt[0, 2] == k and (idx[0, 2, :k] == np.arange(k)).all()
+    c.close()

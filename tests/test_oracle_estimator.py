@@ -116,6 +116,76 @@ def test_p7_eq20_equals_direct_and_eq2_identity(orc, rot128):
         assert np.abs(err / bound).std() < 1.3 and abs((err / bound).mean()) < 0.25
 
 
+def test_eq2_bias_terms_from_raw_arrays(orc, rot128):
+    """Tight pin of the Eq.2 assembly (Eq.2): with non-zero c_q and a deliberately LARGE c_k (keys
+    shifted by +3) the part of the oracle's score that is not the estimated inner product must equal
+    <q,c_k> + <c_q,k_t> - <c_q,c_k> computed with numpy in fp64 FROM THE RAW ARRAYS (not from the oracle's query_prep),
+    with the KV-head mapping g = h // G spelled out; q_ck / cq_ck of rbq_ref_query_prep against numpy dots."""
+    r32, _ = rot128
+    w = synth.make_workload(1, L=384, with_cq=True)
+    K = (w.K + 3.0).astype(np.float32)                   # large centroid: a wrong sign or KV head moves the score by O(100)
+    c_q = (w.c_q + 0.5).astype(np.float32)               # and a query centroid that is not orthogonal to it
+    L, G, sm = 384, w.G, 1 / math.sqrt(D)
+    ck = orc.centroid(K, w.seq_lens)
+    assert np.abs(ck).mean() > 2.5
+    codes, fs, fb = orc.encode(K, [0], w.seq_lens, 0, r32, ck, c_q)
+    scores, qp, dot, pop = orc.estimate_scores(w.q, codes, fs, fb, ck, c_q, w.seq_lens, 0, r32, sm)
+    for h in range(w.Hq):
+        g = h // G
+        q64, cq64, ck64 = w.q[0, h].astype(np.float64), c_q[0, h].astype(np.float64), ck[0, g].astype(np.float64)
+        k64 = K[0, g, :L].astype(np.float64)
+        assert float(qp["q_ck"][0, h]) == pytest.approx(q64 @ ck64, rel=1e-6, abs=1e-5)
+        assert float(qp["cq_ck"][0, h]) == pytest.approx(cq64 @ ck64, rel=1e-6, abs=1e-5)
+        np.testing.assert_allclose(fb[0, h, :L], k64 @ cq64, rtol=2e-6, atol=2e-5)          # f_bias = <c_q, k_t>
+        qn = np.linalg.norm(q64 - cq64)
+        dl, ql = float(qp["delta"][0, h]), float(qp["ql"][0, h])
+        ip20 = 2 * dl * dot[0, h, :L] + 2 * ql * pop[0, g, :L] - dl * int(qp["sumq"][0, h]) - D * ql   # Eq.20 (pinned above)
+        est = qn * fs[0, g, :L].astype(np.float64) * ip20
+        rest = scores[0, h, :L].astype(np.float64) / sm - est
+        want = q64 @ ck64 + k64 @ cq64 - cq64 @ ck64
+        scale = np.abs(scores[0, h, :L] / sm).max()
+        np.testing.assert_allclose(rest, want, rtol=0, atol=1e-5 * max(scale, np.abs(want).max()))
+        # a slip would be visible: each term is far larger than the tolerance
+        tol = 1e-5 * max(scale, np.abs(want).max())
+        assert min(abs(q64 @ ck64), abs(cq64 @ ck64), np.median(np.abs(k64 @ cq64))) > 300 * tol
+
+
+def test_estimator_exact_for_codeword_keys_and_grid_queries(orc, rot128):
+    """End-to-end pin of O2 -> O3 -> O4 -> O5 against the plain inner product: the estimator
+    <c', q_bar> / <c', P^T k_c> (Eq.18) is EXACT when P^T k_c is parallel to its own codeword (|y_j| all equal,
+    alpha = 1: L98, L487) and the rotated query lies on the 16-level INT4 grid (Eq.5 L194 then reconstructs it
+    exactly).  Then Eq.2 (L86) must give back <q,k> itself for arbitrary c_q, c_k -- every term, sign, the h // G
+    mapping and sm_scale are checked against numpy's dot product."""
+    r32, r64 = rot128
+    rng = np.random.default_rng(42)
+    B, Hq, Hkv, L = 1, 8, 2, 64
+    G = Hq // Hkv
+    P = r32.astype(np.float64)
+    ck = (3.0 + rng.standard_normal((B, Hkv, D))).astype(np.float32)
+    cq = (0.5 * rng.standard_normal((B, Hq, D))).astype(np.float32)
+    s = rng.integers(0, 2, (Hkv, L, D)) * 2.0 - 1.0                       # sign patterns = codewords
+    lam = rng.uniform(0.2, 3.0, (Hkv, L, 1))
+    x = (lam * s) @ P.T                                                    # x P = lam * s
+    K = (ck[0][:, None, :].astype(np.float64) + x).astype(np.float32)[None]
+    m = rng.integers(0, 16, (Hq, D)).astype(np.float64)
+    m[:, 0], m[:, 1] = 0, 15                                               # both ends of the grid present
+    qprime = -0.37 + 0.05 * m
+    qprime /= np.linalg.norm(qprime, axis=1, keepdims=True)
+    qn = rng.uniform(2.0, 9.0, (Hq, 1))
+    q = (cq[0].astype(np.float64) + qn * (qprime @ P.T)).astype(np.float32)[None]
+    n = np.array([L], np.int32)
+    codes, fs, fb = orc.encode(K, [0], n, 0, r32, ck, cq)
+    assert (unpack(codes[0]) == (s > 0)).all()                             # the key's code is its own sign pattern
+    sm = 0.25
+    scores, qp, _, _ = orc.estimate_scores(q, codes, fs, fb, ck, cq, n, 0, r32, sm)
+    assert (qp["qu"][0] == m).all()                                        # the query sits on the INT4 grid
+    for h in range(Hq):
+        g = h // G
+        truth = K[0, g].astype(np.float64) @ q[0, h].astype(np.float64) * sm
+        scale = np.linalg.norm(K[0, g].astype(np.float64), axis=1) * np.linalg.norm(q[0, h].astype(np.float64)) * sm
+        assert np.abs(scores[0, h, :L] - truth).max() <= 2e-5 * scale.max(), (h, np.abs(scores[0, h, :L] - truth).max())
+
+
 def _law_samples(orc, c, n_rot, seed):
     """est - c over n_rot Haar rotations for fixed unit k_c, q_c with <k_c,q_c> = c, through the
     oracle's own encode / query_prep / logits chain."""
