@@ -16,8 +16,11 @@ from pathlib import Path
 import numpy as np
 import torch
 
+import os
+
 _HERE = Path(__file__).resolve().parent
-LIB_PATH = _HERE / "librbq_b200.so"
+# RBQ_B200_LIB selects another build of the same library (the -DRBQ_PROBE build for in-kernel timelines)
+LIB_PATH = Path(os.environ["RBQ_B200_LIB"]) if os.environ.get("RBQ_B200_LIB") else _HERE / "librbq_b200.so"
 _lib = None
 
 RBQ_F32, RBQ_BF16 = 0, 1
@@ -28,7 +31,7 @@ RBQ_CK_GIVEN = 1
 EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspace", "rbq_last_error",
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
            "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_topp_select_alg3", "rbq_sparse_attention",
-           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags"]
+           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags", "rbq_probe_dump"]
 N_STAGES = 5
 STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather"]
 
@@ -84,6 +87,7 @@ def load():
         "rbq_profile_enable": ([vp, C.c_int], C.c_int),
         "rbq_profile_read": ([vp, C.POINTER(C.c_float), C.POINTER(i32)], C.c_int),
         "rbq_status_flags": ([vp, C.POINTER(u32), vp], C.c_int),
+        "rbq_probe_dump": ([vp, C.c_int, vp], C.c_int),
     }
     for name, (args, res) in sig.items():
         fn = getattr(lib, name)
@@ -212,6 +216,13 @@ def rbq_profile_read(ctx):
     n = C.c_int32()
     _check(ctx, load().rbq_profile_read(ctx, ms, C.byref(n)), "rbq_profile_read")
     return dict(zip(STAGE_NAMES, [float(x) for x in ms])), n.value
+
+
+def rbq_probe_dump(ctx, kernel: int) -> np.ndarray:
+    """Probe build only (RBQ_B200_LIB=.../librbq_b200_probe.so): uint64 [256 CTAs][16 slots] of clock64 stamps."""
+    out = np.zeros((256, 16), np.uint64)
+    _check(ctx, load().rbq_probe_dump(ctx, int(kernel), out.ctypes.data_as(C.c_void_p)), "rbq_probe_dump")
+    return out
 
 
 def rbq_status_flags(ctx, stream=None) -> int:

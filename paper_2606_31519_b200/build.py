@@ -33,15 +33,20 @@ def _stale(target: Path, deps) -> bool:
     return any(d.stat().st_mtime > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
+def build(force: bool = False, verbose: bool = False, probe: bool = False) -> Path:
+    """probe=True builds librbq_b200_probe.so with -DRBQ_PROBE (in-kernel timeline stamps, rbq_probe_dump); the
+    binding loads it when RBQ_B200_LIB points at it.  The regular library carries no probe code."""
     hdrs = list(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "rbq.h"]
-    OBJ.mkdir(exist_ok=True)
+    obj_dir = HERE / ("build_probe" if probe else "build")
+    lib = HERE / "librbq_b200_probe.so" if probe else LIB
+    flags = FLAGS + (["-DRBQ_PROBE"] if probe else [])
+    obj_dir.mkdir(exist_ok=True)
 
     def compile_one(src: Path):
-        obj = OBJ / (src.stem + ".o")
+        obj = obj_dir / (src.stem + ".o")
         if force or _stale(obj, [src] + hdrs):
-            r = subprocess.run([NVCC, *FLAGS, "-c", str(src), "-o", str(obj)], capture_output=True, text=True)
-            (OBJ / (src.stem + ".ptxas.log")).write_text(r.stderr)
+            r = subprocess.run([NVCC, *flags, "-c", str(src), "-o", str(obj)], capture_output=True, text=True)
+            (obj_dir / (src.stem + ".ptxas.log")).write_text(r.stderr)
             if r.returncode != 0:
                 raise RuntimeError(f"nvcc failed on {src.name}:\n{r.stderr}")
             if verbose:
@@ -50,13 +55,13 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
     with ThreadPoolExecutor(max_workers=8) as ex:
         objs = list(ex.map(compile_one, sources()))
-    if force or _stale(LIB, objs):
-        r = subprocess.run([NVCC, "-shared", "-o", str(LIB), *map(str, objs), "-gencode",
+    if force or _stale(lib, objs):
+        r = subprocess.run([NVCC, "-shared", "-o", str(lib), *map(str, objs), "-gencode",
                             "arch=compute_100a,code=sm_100a"], capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"link failed:\n{r.stderr}")
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, probe="--probe" in sys.argv))

@@ -136,6 +136,8 @@ int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes) {
   ctx->ws_bytes = bytes;
   // the sticky status word starts clear (setup call: a blocking 4-byte memset on the legacy stream)
   RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_flags, 0, sizeof(uint32_t)));
+  // row-maximum keys: zero between decode steps (S5 accumulates with atomicMax, S6 clears after reading)
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_rowmax, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads * sizeof(uint32_t)));
   return RBQ_OK;
 }
 
@@ -216,7 +218,7 @@ int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32
   RBQ_TRY(need_ws(ctx));
   if (!q || !dot || !pop) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/dot/pop null");
   RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
-  return rbq_launch_estimate(ctx, idx, nullptr, dot, pop, (cudaStream_t)stream);
+  return rbq_launch_estimate(ctx, idx, nullptr, dot, pop, nullptr, (cudaStream_t)stream);
 }
 
 int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float* scores, void* stream) {
@@ -226,7 +228,7 @@ int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float
   if (!q || !scores) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/scores null");
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
   RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
-  return rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, (cudaStream_t)stream);
+  return rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, nullptr, (cudaStream_t)stream);
 }
 
 int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
@@ -279,12 +281,13 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   cudaEvent_t* ev = nullptr;                       // stage timing events of this step, if profiling
   if (ctx->prof_on && ctx->prof_steps < RBQ_PROFILE_MAX_STEPS) ev = ctx->prof_ev + (size_t)ctx->prof_steps++ * (RBQ_N_STAGES + 1);
   ctx->stage_ev = ev;
+  uint32_t* rowmax = ws_ptr<uint32_t>(ctx, ctx->off_rowmax);   // zero between steps: S6 clears each key once it has read it
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[0], s));
   RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, q_copy, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
-  RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, s));
+  RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, rowmax, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  RBQ_TRY(rbq_launch_topp(ctx, scores, ws_ptr<uint32_t>(ctx, ctx->off_rowmax), idx->n_indexed, p, bits, sel_idx, sn, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
   const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
   ctx->stage_ev = nullptr;
@@ -326,6 +329,19 @@ int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host) {
   }
   ctx->prof_steps = 0;
   return RBQ_OK;
+}
+
+int rbq_probe_dump(rbq_ctx* ctx, int kernel, uint64_t* out_host) {
+  RBQ_CTX(ctx);
+  if (!out_host) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "out_host null");
+  unsigned long long* o = reinterpret_cast<unsigned long long*>(out_host);
+  switch (kernel) {
+    case RBQ_PROBE_ESTIMATE: return rbq_probe_copy_estimate(o);
+    case RBQ_PROBE_TOPP: return rbq_probe_copy_topp(o);
+    case RBQ_PROBE_GATHER: return rbq_probe_copy_gather(o);
+    case RBQ_PROBE_PLAN: return rbq_probe_copy_plan(o);
+    default: RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "unknown probe kernel %d", kernel);
+  }
 }
 
 int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, const rbq_index* idx, float p,

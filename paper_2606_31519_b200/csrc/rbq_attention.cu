@@ -20,6 +20,9 @@
 // fp32 K/V or q (parity config 0) take the FP32-pipe kernel attn_simt_kernel over the same union lists.
 #include "rbq_common.cuh"
 
+RBQ_PROBE_DECL(gather_probe);
+RBQ_PROBE_DECL(plan_probe);
+
 namespace {
 
 // ---- bitmaps from caller-provided index lists (stand-alone rbq_sparse_attention) --------------------------------
@@ -755,4 +758,24 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
                                                   ctx->cfg.n_kv_heads, max_chunks, (float*)out, lse);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
+}
+
+int rbq_probe_copy_gather(unsigned long long* host) {
+#ifdef RBQ_PROBE
+  if (cudaDeviceSynchronize() != cudaSuccess) return RBQ_ERR_CUDA;
+  return cudaMemcpyFromSymbol(host, gather_probe, sizeof(unsigned long long) * RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS) == cudaSuccess ? RBQ_OK : RBQ_ERR_CUDA;
+#else
+  (void)host;
+  return RBQ_ERR_UNSUPPORTED;
+#endif
+}
+
+int rbq_probe_copy_plan(unsigned long long* host) {
+#ifdef RBQ_PROBE
+  if (cudaDeviceSynchronize() != cudaSuccess) return RBQ_ERR_CUDA;
+  return cudaMemcpyFromSymbol(host, plan_probe, sizeof(unsigned long long) * RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS) == cudaSuccess ? RBQ_OK : RBQ_ERR_CUDA;
+#else
+  (void)host;
+  return RBQ_ERR_UNSUPPORTED;
+#endif
 }

@@ -8,16 +8,18 @@
 
 #include "../../include/rbq.h"
 
-#define RBQ_D 128            // head_dim supported by every kernel
-#define RBQ_WORDS 4          // D/32 code words per token
+#define RBQ_D 128            // head_dim of the kernels that are not templated on it yet
+#define RBQ_WORDS 4          // D/32 code words per token at D = 128
 #define RBQ_MAX_G 4          // query heads per KV head (N=8 MMA columns: G heads + G ones-columns)
+#define RBQ_MAX_KSTEPS 8     // k-steps of the estimator MMA: D/32 (2, 4, 8 for D = 64, 128, 256)
 
 // Private per-(sequence, KV head) query constants produced by S3 and consumed by S4/S5.
 // bfrag: B-operand fragments of mma.m16n8k32.u8 in register order [k-step][lane][2]
 //        (column 2j = query head j of the group, column 2j+1 = all-ones -> popcount),
 //        pre-scaled by 2^(3-n) so that the masked code bytes (value 2^n) need no shift.
+//        Which code bit a (k-step, lane, register, byte) position stands for: rbq_bfrag_dim below.
 struct __align__(16) RbqQConst {
-  uint32_t bfrag[4][32][2];
+  uint32_t bfrag[RBQ_MAX_KSTEPS][32][2];
   float cA[RBQ_MAX_G];       // sm_scale * ||q-c_q|| * Delta / 4
   float cB[RBQ_MAX_G];       // sm_scale * ||q-c_q|| * q_l   / 4
   float cD[RBQ_MAX_G];       // sm_scale * (<q,c_k> - <c_q,c_k>)
@@ -43,8 +45,7 @@ struct rbq_ctx {
   size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_gdone, off_rowmax, off_part,
       off_stage_q, off_stage_out, off_centroid, total_bytes;
   cudaEvent_t ev_copy, ev_flush;
-  unsigned attr_mask;        // kernels whose MaxDynamicSharedMemorySize was set for THIS context's device (RBQ_ATTR_*)
-  size_t attr_topp_smem;     // largest dynamic shared memory size set for the Top-p kernels so far
+  unsigned char attr_done[128];   // kernel instantiations whose MaxDynamicSharedMemorySize was set for THIS context's device (RBQ_ATTR_*)
   size_t off_flags;          // device status word (RBQ_FLAG_*), sticky
   int pending;               // host shadow of n_total - n_indexed (uniform over the batch: every sequence appends n_new rows per call)
   int in_flight;             // rows encoded by an enqueued flush, not yet committed
@@ -61,9 +62,10 @@ struct rbq_ctx {
   char err[256];
 };
 
-// per-context "function attribute set" bits (the attribute is per device; a context lives on one device)
-enum { RBQ_ATTR_QUERY = 1u, RBQ_ATTR_ENC_EXACT = 2u, RBQ_ATTR_ENC_FAST = 4u, RBQ_ATTR_GATHER = 8u, RBQ_ATTR_ALG3 = 16u,
-       RBQ_ATTR_EST = 32u, RBQ_ATTR_FUSED = 64u };
+// per-context "function attribute set" slots (the attribute is per device; a context lives on one device): base ids, each
+// kernel family adds the index of its instantiation
+enum { RBQ_ATTR_QUERY = 0 /* +6 */, RBQ_ATTR_EST = 8 /* +36 */, RBQ_ATTR_TOPP = 48 /* +9 */, RBQ_ATTR_ENC_EXACT = 60 /* +4 */,
+       RBQ_ATTR_FBIAS = 66 /* +2 */, RBQ_ATTR_ENC_FAST = 70, RBQ_ATTR_GATHER = 72 /* +8 */, RBQ_ATTR_ALG3 = 82, RBQ_ATTR_MISC = 84 };
 
 #define RBQ_FAIL(ctx, code, ...)                                   \
   do {                                                             \
@@ -106,6 +108,84 @@ __device__ __forceinline__ float rbq_fkey_inv(uint32_t k) {
   return __uint_as_float(u);
 }
 
+// ---- estimator operand layout (shared by S3, which builds the B fragments, and S4, which builds the A fragments) ------
+// A fragment of mma.m16n8k32.u8 held by lane (g, tp): register r of k-step s holds 4 bytes, byte i <-> k = 4 tp + i (+16 for
+// r = 1).  The 1-bit code of a token is expanded to those bytes by masking a 32-bit value x that lane tp derives from the
+// token's code words (W = D/32 words per token):
+//   W = 4: x = word tp;                       byte i of register (s, r): bit e = 2 s + r of code byte i of x      (value 2^(e & 3))
+//   W = 8: x_u = word 2 tp + u, u = s >> 2;   same with s' = s & 3
+//   W = 2: v = 16-bit half (tp & 1) of word tp >> 1, x = v | (v >> 1) << 16; bit e' = 4 s + 2 r of x's byte i  (value 2^(2 r)),
+//          i.e. code bit e' + (i >> 1) of code byte 2 (tp & 1) + (i & 1)
+// Returns the head dimension that position multiplies and the left shift that makes (A byte) * (B byte) = 8 * bit * qu.
+__host__ __device__ inline void rbq_bfrag_dim(int W, int s, int tp, int r, int i, int& dim, int& shift) {
+  if (W == 2) {
+    const int e = 4 * s + 2 * r;
+    dim = 32 * (tp >> 1) + 8 * (2 * (tp & 1) + (i & 1)) + e + (i >> 1);
+    shift = 3 - 2 * r;
+  } else {
+    const int u = (W == 8) ? (s >> 2) : 0, sp = s & 3, e = 2 * sp + r;
+    dim = 32 * ((W == 8 ? 2 * tp : tp) + u) + 8 * i + e;
+    shift = 3 - (e & 3);
+  }
+}
+
+// ---- mbarrier / bulk-copy (TMA, UBLKCP) helpers ------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t rbq_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void rbq_mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void rbq_mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void rbq_mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void rbq_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// bounded spin on a phase parity: a protocol mistake must trap, not hang the GPU
+__device__ __forceinline__ void rbq_mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  for (uint32_t spin = 0; !done; ++spin) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (spin > (1u << 22)) __trap();
+  }
+}
+// 1-D bulk copy global -> shared (bytes a multiple of 16, both addresses 16-byte aligned), completion on an mbarrier
+__device__ __forceinline__ void rbq_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar) : "memory");
+}
+
+// ---- in-kernel timeline probes (build option: python -m paper_2606_31519_b200.build --probe -> librbq_b200_probe.so) -----
+// With -DRBQ_PROBE a kernel stamps clock64 (and %globaltimer in the slot after it) of chosen points into a per-file device
+// buffer [RBQ_PROBE_CTAS][RBQ_PROBE_SLOTS]; rbq_probe_dump(kernel id) copies it out.  Without the flag the macros vanish.
+#define RBQ_PROBE_CTAS 256
+#define RBQ_PROBE_SLOTS 16
+enum { RBQ_PROBE_ESTIMATE = 0, RBQ_PROBE_TOPP = 1, RBQ_PROBE_GATHER = 2, RBQ_PROBE_PLAN = 3, RBQ_PROBE_KERNELS = 4 };
+#ifdef RBQ_PROBE
+#define RBQ_PROBE_DECL(name) __device__ unsigned long long name[RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS]
+#define RBQ_STAMP(buf, slot)                                                                                   \
+  do {                                                                                                         \
+    if (blockIdx.x < RBQ_PROBE_CTAS) {                                                                         \
+      unsigned long long gt_;                                                                                  \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_));                                                  \
+      (buf)[blockIdx.x * RBQ_PROBE_SLOTS + (slot)] = (unsigned long long)clock64();                            \
+      if ((slot) == 0) (buf)[blockIdx.x * RBQ_PROBE_SLOTS + RBQ_PROBE_SLOTS - 1] = gt_;                        \
+    }                                                                                                          \
+  } while (0)
+#else
+#define RBQ_PROBE_DECL(name)
+#define RBQ_STAMP(buf, slot) do {} while (0)
+#endif
+int rbq_probe_copy_estimate(unsigned long long* host);      // defined in the .cu that owns the buffer; RBQ_ERR_UNSUPPORTED without RBQ_PROBE
+int rbq_probe_copy_topp(unsigned long long* host);
+int rbq_probe_copy_gather(unsigned long long* host);
+int rbq_probe_copy_plan(unsigned long long* host);
+
 // ---- programmatic dependent launch (PDL) -----------------------------------------------------------
 // The kernels of a decode step are launched with programmatic stream serialisation: a kernel's CTAs may become
 // resident while its predecessor drains, which hides the launch latency between the short kernels of the step.
@@ -128,11 +208,11 @@ inline cudaError_t rbq_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block,
 // MaxDynamicSharedMemorySize is a per-device attribute of a function: it is set once per CONTEXT (a context lives on the
 // device that was current at rbq_create), always to the same per-kernel maximum, so that contexts with different
 // configurations on one device never lower each other's limit.
-#define RBQ_SET_SMEM_ATTR(ctx, bit, func, bytes)                                                          \
+#define RBQ_SET_SMEM_ATTR(ctx, id, func, bytes)                                                           \
   do {                                                                                                    \
-    if (!((ctx)->attr_mask & (bit))) {                                                                    \
+    if (!(ctx)->attr_done[(id)]) {                                                                        \
       RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes))); \
-      (ctx)->attr_mask |= (bit);                                                                          \
+      (ctx)->attr_done[(id)] = 1;                                                                         \
     }                                                                                                     \
   } while (0)
 #define RBQ_MAX_DYN_SMEM (227 * 1024)
@@ -150,11 +230,11 @@ int rbq_launch_append_copy(rbq_ctx*, const void* k_new, const void* v_new, int n
                            int32_t* n_indexed, int32_t* n_total, int commit, cudaStream_t);
 // q_copy (or NULL): device buffer that receives a verbatim copy of q (used when q lives in mapped host memory)
 int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t);
-int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop,
-                        cudaStream_t);
+// S4/S5 behind an rbq_launch_query.  rowmax_key: zeroed keys that receive the row maxima, or NULL.
+int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t);
 // S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.
 // rowmax_key: order-preserving keys of the row maxima [B*Hq] (written by S5), or NULL to compute them here.
-int rbq_launch_topp(rbq_ctx*, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p,
+int rbq_launch_topp(rbq_ctx*, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
                     uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
 // Alg.3 selector (ternary threshold search in fp64): ascending sel_idx, sel_cnt, optional iteration counts [B*Hq].
 int rbq_launch_topp_alg3(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx, int32_t* sel_cnt,

@@ -349,8 +349,7 @@ static int launch_encode_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin
                            int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
   const size_t smem = (size_t)(ENC_TOK * XS + ENC_TOK + (ROT == RBQ_ROT_DENSE ? RBQ_D * RBQ_D : RBQ_D)) * sizeof(float);
   auto kern = encode_kernel<T, ROT>;
-  const unsigned bit = RBQ_ATTR_ENC_EXACT << (8 + 16 + (sizeof(T) == 2 ? 0 : 2) + (ROT == RBQ_ROT_DENSE ? 0 : 1));   // one bit per instantiation
-  RBQ_SET_SMEM_ATTR(ctx, bit, kern, smem);
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_EXACT + (sizeof(T) == 2 ? 0 : 2) + (ROT == RBQ_ROT_DENSE ? 0 : 1), kern, smem);
   dim3 grid((max_count + ENC_TOK - 1) / ENC_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
   kern<<<grid, ENC_THREADS, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
                                        ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->cfg.rot, idx->c_k,
@@ -365,7 +364,7 @@ static int launch_fbias_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin,
                           int max_count, const rbq_index* idx, cudaStream_t s) {
   const size_t smem = (size_t)(FB_TOK * FB_XS + ctx->G * RBQ_D) * sizeof(float);
   auto kern = fbias_kernel<T>;
-  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_EXACT << (8 + 16 + 4 + (sizeof(T) == 2 ? 0 : 1)), kern, smem);
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_FBIAS + (sizeof(T) == 2 ? 0 : 1), kern, smem);
   dim3 grid((max_count + FB_TOK - 1) / FB_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
   kern<<<grid, FB_TOK, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count, ctx->cfg.n_q_heads,
                                   ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, idx->c_q, idx->f_bias);

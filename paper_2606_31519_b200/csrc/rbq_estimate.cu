@@ -17,6 +17,13 @@
 // a warp keeps two groups of loads in flight.  MMA rows are mapped to tokens so that lane (g, t)
 // ends up with head t's logits of tokens 4g..4g+3: one 16-byte coalesced store per lane and group.
 //
+// Templated on W = D/32 code words per token (D = 64, 128, 256; the bit <-> MMA-operand mapping is rbq_bfrag_dim).
+//
+// Measured alternatives (round 2, profiles/r02_estimator.md): a persistent one-CTA-per-SM variant that stages the code
+// stream in a shared-memory ring with 1-D bulk copies (UBLKCP) and runs S3 inside the CTA was 10 us SLOWER per step: the
+// inner loop is bound by the ALU pipe (36 LOP3/SHF per 32-token group at 2 clk each) plus the IMMA pipe (~11 clk per
+// IMMA.16832 in this mix), not by HBM, and a 200 KB CTA cannot become resident under its predecessor as these small CTAs do.
+//
 // Integer results are exact.  Epilogue in fp32 without cancellation:
 //   acc_d = 4*(2*dot - sum(qu)), acc_p = 4*(2*pop - D)   (exact ints: accumulators start at
 //   0x4B400000 - 4*sum(qu) / - 4*D, so reinterpreting as float and subtracting 2^23+2^22 converts)
@@ -44,23 +51,54 @@ __device__ __forceinline__ void imma_16832_first(int (&d)[4], uint32_t a0, uint3
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "r"(cd), "r"(cp));
 }
 
-// One 16-token tile: rows g (code word wa) and g+8 (code word wb) of this lane's quad column.
-__device__ __forceinline__ void tile_mma(int (&c)[4], uint32_t wa, uint32_t wb, const uint32_t (&bf)[4][2], int cd, int cp) {
-  const uint32_t ha = wa >> 4, hb = wb >> 4;
-  imma_16832_first(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x02020202u, wb & 0x02020202u, bf[0][0], bf[0][1], cd, cp);
-  imma_16832(c, wa & 0x04040404u, wb & 0x04040404u, wa & 0x08080808u, wb & 0x08080808u, bf[1][0], bf[1][1]);
-  imma_16832(c, ha & 0x01010101u, hb & 0x01010101u, ha & 0x02020202u, hb & 0x02020202u, bf[2][0], bf[2][1]);
-  imma_16832(c, ha & 0x04040404u, hb & 0x04040404u, ha & 0x08080808u, hb & 0x08080808u, bf[3][0], bf[3][1]);
+// what lane (g, t) holds of one token: the 32-bit value(s) x of rbq_bfrag_dim
+template <int W> struct TokX { uint32_t x[W == 8 ? 2 : 1]; };
+
+template <int W>
+__device__ __forceinline__ TokX<W> load_tok(const uint32_t* __restrict__ p, int t) {   // p: the token's first code word
+  TokX<W> r;
+  if (W == 4) {
+    r.x[0] = __ldg(p + t);
+  } else if (W == 8) {
+    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p) + t);
+    r.x[0] = v.x; r.x[W == 8 ? 1 : 0] = v.y;
+  } else {
+    const uint32_t v = (__ldg(p + (t >> 1)) >> (16 * (t & 1))) & 0xFFFFu;
+    r.x[0] = v | ((v >> 1) << 16);
+  }
+  return r;
 }
 
-struct GroupLoad {            // what lane (g, t) needs of one 32-token group
-  uint32_t w[4];              // word t of tokens 4g .. 4g+3
+// One 16-token tile: rows g (token value a) and g + 8 (token value b) of this lane's quad column.
+template <int W>
+__device__ __forceinline__ void tile_mma(int (&c)[4], const TokX<W>& a, const TokX<W>& b, const uint32_t (&bf)[W][2], int cd, int cp) {
+  if (W == 2) {
+    const uint32_t wa = a.x[0], wb = b.x[0], ha = wa >> 4, hb = wb >> 4;
+    imma_16832_first(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x04040404u, wb & 0x04040404u, bf[0][0], bf[0][1], cd, cp);
+    imma_16832(c, ha & 0x01010101u, hb & 0x01010101u, ha & 0x04040404u, hb & 0x04040404u, bf[1][0], bf[1][1]);
+  } else {
+#pragma unroll
+    for (int u = 0; u < (W == 8 ? 2 : 1); ++u) {
+      const uint32_t wa = a.x[u], wb = b.x[u], ha = wa >> 4, hb = wb >> 4;
+      if (u == 0)
+        imma_16832_first(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x02020202u, wb & 0x02020202u, bf[0][0], bf[0][1], cd, cp);
+      else
+        imma_16832(c, wa & 0x01010101u, wb & 0x01010101u, wa & 0x02020202u, wb & 0x02020202u, bf[4 * u][0], bf[4 * u][1]);
+      imma_16832(c, wa & 0x04040404u, wb & 0x04040404u, wa & 0x08080808u, wb & 0x08080808u, bf[4 * u + 1][0], bf[4 * u + 1][1]);
+      imma_16832(c, ha & 0x01010101u, hb & 0x01010101u, ha & 0x02020202u, hb & 0x02020202u, bf[4 * u + 2][0], bf[4 * u + 2][1]);
+      imma_16832(c, ha & 0x04040404u, hb & 0x04040404u, ha & 0x08080808u, hb & 0x08080808u, bf[4 * u + 3][0], bf[4 * u + 3][1]);
+    }
+  }
+}
+
+template <int W> struct GroupLoad {   // what lane (g, t) needs of one 32-token group
+  TokX<W> w[4];               // its share of the code of tokens 4g .. 4g+3
   float4 fs;                  // f_scale of tokens 4g .. 4g+3
 };
 
 // grid = k * SMs CTAs of EST_WARPS warps.  Flat group index -> (sequence b, KV head, 32-token group).
-template <bool INT_OUT, bool HAS_BIAS>
-__global__ void __launch_bounds__(EST_THREADS, 3)
+template <int W, bool INT_OUT, bool HAS_BIAS>
+__global__ void __launch_bounds__(EST_THREADS, W == 8 ? 2 : 3)
 estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
                 const float* __restrict__ f_bias, const int32_t* __restrict__ n_indexed,
                 const RbqQConst* __restrict__ qconst, int B, int Hq, int Hkv, int Lcap, float sm_scale,
@@ -103,27 +141,27 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const size_t prow = (size_t)bg * Lcap;
     // lane (g, t): word t of tokens 4g..4g+3 of a group and their factors.  A token run beyond the allocation
     // (Lcap % 32 != 0) is clamped to its last 4 tokens (never stored); groups beyond the segment are not loaded.
-    const uint32_t* cbase = codes + prow * RBQ_WORDS + t;
+    const uint32_t* cbase = codes + prow * W;
     const float* fbase = f_scale + prow;
     const int tok_clamp = Lcap - 4;
-    auto load_at = [&](int gi) -> GroupLoad {
+    auto load_at = [&](int gi) -> GroupLoad<W> {
       const int tk = min(gi * 32 + 4 * g, tok_clamp);
-      const uint32_t* p = cbase + (size_t)tk * RBQ_WORDS;
-      GroupLoad r;
+      const uint32_t* p = cbase + (size_t)tk * W;
+      GroupLoad<W> r;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) r.w[k] = __ldg(p + k * RBQ_WORDS);
+      for (int k = 0; k < 4; ++k) r.w[k] = load_tok<W>(p + k * W, t);
       r.fs = __ldg(reinterpret_cast<const float4*>(fbase + tk));
       return r;
     };
     // three groups of loads in flight per warp; codes and factors do not depend on S3, its constants do
-    GroupLoad l0 = load_at(g0), l1 = l0, l2 = l0;
+    GroupLoad<W> l0 = load_at(g0), l1 = l0, l2 = l0;
     if (g0 + 1 < g1) l1 = load_at(g0 + 1);
     if (g0 + 2 < g1) l2 = load_at(g0 + 2);
     if (first_segment) { rbq_pdl_wait(); first_segment = false; }   // S3's query constants and zeroed row maxima
     const RbqQConst* qc = qconst + bg;
-    uint32_t bf[4][2];
+    uint32_t bf[W][2];
 #pragma unroll
-    for (int s = 0; s < 4; ++s) {
+    for (int s = 0; s < W; ++s) {
       const uint2 v = *reinterpret_cast<const uint2*>(&qc->bfrag[s][lane][0]);
       bf[s][0] = v.x; bf[s][1] = v.y;
     }
@@ -132,11 +170,11 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     const size_t row = ((size_t)b * Hq + gk * G + hsel) * Lcap;
 
     float smax = -INFINITY;                                     // running max of this lane's head over the segment
-    auto process = [&](const GroupLoad& cur, int gi) {
+    auto process = [&](const GroupLoad<W>& cur, int gi) {
       // tile 0: rows g / g+8 = tokens 4g / 4g+1 ; tile 1: tokens 4g+2 / 4g+3
       int c0[4], c1[4];
-      tile_mma(c0, cur.w[0], cur.w[1], bf, init_d, init_p);
-      tile_mma(c1, cur.w[2], cur.w[3], bf, init_d, init_p);
+      tile_mma<W>(c0, cur.w[0], cur.w[1], bf, init_d, init_p);
+      tile_mma<W>(c1, cur.w[2], cur.w[3], bf, init_d, init_p);
       const int acc_d[4] = {c0[0], c0[2], c1[0], c1[2]};
       const int acc_p[4] = {c0[1], c0[3], c1[1], c1[3]};
       const int tok = gi * 32 + 4 * g;                          // first of this lane's 4 tokens
@@ -185,36 +223,52 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
       smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 4));
       smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 8));
       smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, 16));
-      if (g == 0 && head_ok && smax > -INFINITY)
+      if (g == 0 && head_ok && smax > -INFINITY && rowmax_key != nullptr)
         atomicMax(&rowmax_key[(size_t)b * Hq + gk * G + t], rbq_fkey(__fadd_rn(smax, 0.0f)));
     }
     gcur += g1 - g0;
   }
 }
 
-template <bool INT_OUT, bool HAS_BIAS>
-int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, cudaStream_t s) {
+template <int W, bool INT_OUT, bool HAS_BIAS>
+int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t s) {
   if (ctx->cfg.batch > EST_MAX_B) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch %d > %d", ctx->cfg.batch, EST_MAX_B);
   // upper bound of the work: every sequence full; 3 CTAs (24 warps) per SM, fewer when there is little work
   const long long max_groups = (long long)ctx->cfg.batch * ctx->cfg.n_kv_heads * ((ctx->cfg.max_tokens + 31) / 32);
   long long ctas = (max_groups + 2 * EST_WARPS - 1) / (2 * EST_WARPS);          // >= 2 groups per warp
-  const long long cap = (long long)ctx->sm_count * 3;
+  const long long cap = (long long)ctx->sm_count * (W == 8 ? 2 : 3);
   if (ctas > cap) ctas = cap;
   if (ctas < 1) ctas = 1;
   const RbqQConst* qc = reinterpret_cast<const RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
-  RBQ_CUDA_OK(ctx, rbq_launch_pdl(estimate_kernel<INT_OUT, HAS_BIAS>, dim3((unsigned)ctas), dim3(EST_THREADS), 0, s,
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(estimate_kernel<W, INT_OUT, HAS_BIAS>, dim3((unsigned)ctas), dim3(EST_THREADS), 0, s,
                                   (const uint32_t*)idx->codes, (const float*)idx->f_scale, (const float*)idx->f_bias,
                                   (const int32_t*)idx->n_indexed, qc, ctx->cfg.batch, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
-                                  ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop,
-                                  reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax)));
+                                  ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop, rowmax_key));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
+template <int W>
+int launch_w(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t s) {
+  if (dot) return launch_t<W, true, false>(ctx, idx, scores, dot, pop, rowmax_key, s);
+  if (idx->f_bias && idx->c_q) return launch_t<W, false, true>(ctx, idx, scores, dot, pop, rowmax_key, s);
+  return launch_t<W, false, false>(ctx, idx, scores, dot, pop, rowmax_key, s);
+}
+
 }  // namespace
 
-int rbq_launch_estimate(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, cudaStream_t s) {
-  if (dot) return launch_t<true, false>(ctx, idx, scores, dot, pop, s);
-  if (idx->f_bias && idx->c_q) return launch_t<false, true>(ctx, idx, scores, dot, pop, s);
-  return launch_t<false, false>(ctx, idx, scores, dot, pop, s);
+// S4/S5 with the query constants of the rbq_launch_query in front of it (chained by programmatic dependent launch).
+// rowmax_key (or NULL): receives the order-preserving keys of the row maxima by atomicMax -- must be zero on entry.
+int rbq_launch_estimate(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key,
+                        cudaStream_t s) {
+  switch (ctx->cfg.head_dim) {
+    case 64: return launch_w<2>(ctx, idx, scores, dot, pop, rowmax_key, s);
+    case 256: return launch_w<8>(ctx, idx, scores, dot, pop, rowmax_key, s);
+    default: return launch_w<4>(ctx, idx, scores, dot, pop, rowmax_key, s);
+  }
+}
+
+int rbq_probe_copy_estimate(unsigned long long* host) {
+  (void)host;
+  return RBQ_ERR_UNSUPPORTED;      // no stamps in this kernel
 }

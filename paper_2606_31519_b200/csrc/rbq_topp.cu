@@ -25,6 +25,8 @@
 
 #include "rbq_common.cuh"
 
+RBQ_PROBE_DECL(topp_probe);
+
 namespace cg = cooperative_groups;
 
 namespace {
@@ -175,7 +177,7 @@ __device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4]
 // smem: TpSmall | hist u32[2][TP_NB] (later: selection words) | cand_all | cand_loc | scores slice [s_cap]
 template <int CS>
 __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
-topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
+topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
   rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
@@ -215,7 +217,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
       bits_row[(lo >> 5) + w] = rem >= 32 ? 0xFFFFFFFFu : ((1u << rem) - 1u);
     }
     if (sel_idx) for (int i = tid; i < len; i += TP_THREADS) sel_idx[rbase + lo + i] = lo + i;
-    if (rank == 0 && tid == 0) sel_cnt[row] = n;
+    if (rank == 0 && tid == 0) { sel_cnt[row] = n; rowmax_key[row] = 0u; }   // nobody reads the key on this path
     return;
   }
   auto csync = [&]() { if (CS == 1) __syncthreads(); else cluster.sync(); };
@@ -303,6 +305,7 @@ topp_kernel(const float* __restrict__ scores, const uint32_t* __restrict__ rowma
     if ((tid & 7) == 0) { sh.xc_mass[tid >> 3] = ms * sh.tabA[tid >> 3]; sh.xc_cnt[tid >> 3] = cs; }
   }
   csync();                                                    // S1: histograms and coarse summaries complete
+  if (rank == 0 && tid == 0) rowmax_key[row] = 0u;            // every CTA of the row has read its maximum: clear the key for the next step
   if (warp == 0) {
     // coarse crossing: lane l owns coarse bins 2l, 2l+1 (totals over the cluster in rank order), warp scan in fp64;
     // then the 32 fine bins of the crossing coarse bin, one per lane
@@ -607,16 +610,13 @@ __global__ void rowmax_kernel(const float* __restrict__ scores, const int32_t* _
 }
 
 template <int CS>
-int launch_cs(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p, uint32_t* bits,
+int launch_cs(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p, uint32_t* bits,
               int wpr, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
   const int s_cap = ((((ctx->cfg.max_tokens + CS - 1) / CS) + 31) & ~31) + 32;
   const size_t smem = TP_OFF_SC + (size_t)s_cap * 4;
   auto kern = topp_kernel<CS>;
-  if (!(ctx->attr_mask & (0x100u << CS))) {                    // one bit per instantiation (CS = 1, 2, 4, 8)
-    RBQ_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, RBQ_MAX_DYN_SMEM));
-    ctx->attr_mask |= 0x100u << CS;
-  }
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_TOPP + CS, kern, RBQ_MAX_DYN_SMEM);
   dim3 grid(CS, rows);
   RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, grid, dim3(TP_THREADS), smem, s, scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads,
                                   ctx->cfg.max_tokens, wpr, p, bits, sel_idx, sel_cnt));
@@ -647,7 +647,7 @@ int rbq_topp_cluster_size(const rbq_ctx* ctx) {
 }
 
 // rowmax_key == NULL: the maxima are computed here (rbq_topp_select on caller-provided scores).
-int rbq_launch_topp(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_key, const int32_t* n_indexed, float p,
+int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
                     uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int cs = rbq_topp_cluster_size(ctx);
   const int wpr = rbq_words_per_row(ctx);
@@ -669,4 +669,14 @@ int rbq_launch_topp(rbq_ctx* ctx, const float* scores, const uint32_t* rowmax_ke
     case 2: return launch_cs<2>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
     default: return launch_cs<1>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
   }
+}
+
+int rbq_probe_copy_topp(unsigned long long* host) {
+#ifdef RBQ_PROBE
+  if (cudaDeviceSynchronize() != cudaSuccess) return RBQ_ERR_CUDA;
+  return cudaMemcpyFromSymbol(host, topp_probe, sizeof(unsigned long long) * RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS) == cudaSuccess ? RBQ_OK : RBQ_ERR_CUDA;
+#else
+  (void)host;
+  return RBQ_ERR_UNSUPPORTED;
+#endif
 }
