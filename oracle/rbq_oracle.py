@@ -121,6 +121,15 @@ def encode(K, t_begin, t_end, rot_kind, rot, c_k, c_q=None, Hq=0, codes=None, f_
     return codes, f_scale, f_bias
 
 
+def round_factors_f16(f_scale: np.ndarray) -> np.ndarray:
+    """O2c: the stored factors rounded to IEEE binary16 (RNE) and widened back; returns a new array."""
+    f = _f32(f_scale).copy()
+    fn = lib().rbq_ref_round_factors_f16
+    fn.argtypes = [C.c_void_p, C.c_longlong]
+    assert fn(f.ctypes.data, f.size) == 0
+    return f
+
+
 # --- O3 -----------------------------------------------------------------------------------
 def query_prep(q, Hkv, rot_kind, rot, c_k, c_q=None):
     q = _f32(q)
@@ -249,13 +258,16 @@ class LazyIndex:
     one batch with the frozen c_k; they stay pending (attended exactly, excluded from Top-p) until
     the NEXT append call commits them (n_indexed += flushed)."""
 
-    def __init__(self, K, V, seq_lens, rot_kind, rot, W, c_q=None):
+    def __init__(self, K, V, seq_lens, rot_kind, rot, W, c_q=None, factor_f16=False):
         self.K, self.V = _f32(K).copy(), _f32(V).copy()
         self.rot_kind, self.rot, self.W, self.c_q = rot_kind, _f32(rot), int(W), c_q
+        self.factor_f16 = factor_f16
         sl = _i32(seq_lens)
         self.c_k = centroid(self.K, sl)
         self.codes, self.f_scale, self.f_bias = encode(self.K, np.zeros_like(sl), sl, rot_kind, self.rot,
                                                        self.c_k, c_q)
+        if factor_f16:
+            self.f_scale = round_factors_f16(self.f_scale)
         self.n_indexed = sl.copy()
         self.n_total = sl.copy()
         self.in_flight = 0
@@ -275,4 +287,6 @@ class LazyIndex:
             nf = pending // self.W * self.W
             encode(self.K, self.n_indexed, self.n_indexed + nf, self.rot_kind, self.rot, self.c_k, self.c_q,
                    codes=self.codes, f_scale=self.f_scale, f_bias=self.f_bias)
+            if self.factor_f16:       # idempotent on the already rounded prefix
+                self.f_scale = round_factors_f16(self.f_scale)
             self.in_flight = nf

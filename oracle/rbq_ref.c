@@ -261,6 +261,22 @@ int rbq_ref_encode(const float* K, int B, int Hkv, int Lcap, int D, const int32_
 }
 
 /* ------------------------------------------------------------------------- */
+/* O2c 2-byte correction factors ("B_alpha ... typically FP16",   */
+/*     L756-766: the 3.5 % space figure assumes an FP16 factor per token and    */
+/*     head).  The stored factor f_scale (R4) is rounded to IEEE binary16,      */
+/*     round-to-nearest-even, and widened back: every later step (O5) then      */
+/*     uses the rounded value exactly as it uses the fp32 one.  Overflow to inf */
+/*     cannot happen for finite keys of the workloads (f_scale ~ ||x||/sqrt(D)); */
+/*     values below the binary16 subnormal range round to 0 (the estimated part */
+/*     of such a logit is then dropped, as for x = 0, R15).                     */
+/* ------------------------------------------------------------------------- */
+int rbq_ref_round_factors_f16(float* f_scale, long long n) {
+  if (!f_scale || n < 0) return RBQ_REF_ERR;
+  for (long long i = 0; i < n; ++i) f_scale[i] = (float)(_Float16)f_scale[i];
+  return RBQ_REF_OK;
+}
+
+/* ------------------------------------------------------------------------- */
 /* O3  query pre-processing and INT4 quantisation                              */
 /*     (Alg.2 lines 4-6; L192-197 Eq.5; L524).               */
 /*   xq = q - c_q ; qn = ||xq||_2 ; u = xq/qn      (Alg.2 line 4, R12)         */

@@ -176,3 +176,29 @@ def test_f_bias_is_cq_dot_k(orc, rot128):
     for h in (0, 5, 31):
         ref = w.K[0, h // G, :256].astype(np.float64) @ w.c_q[0, h].astype(np.float64)
         np.testing.assert_allclose(fb[0, h, :256], ref, rtol=1e-5, atol=1e-4)
+
+
+def test_factors_f16_rounding_and_logit_bound(orc, rot128):
+    """O2c (PAPER.md:L752 FP16 factors; L756-766 space accounting): the rounded factor equals numpy's float32 -> float16 ->
+    float32 conversion (an independent RNE implementation) bit for bit, is idempotent, moves each factor by at most 2^-11
+    relative, and therefore moves the ESTIMATED part of every logit by at most 2^-11 relative (the Eq.2 bias terms do
+    not involve the factor); the space overhead with 2-byte factors is the paper's 3.5 %."""
+    import math
+    from paper_2606_31519_b200 import synth
+    r32, _ = rot128
+    w = synth.make_workload(1, L=777)
+    ck = orc.centroid(w.K, w.seq_lens)
+    codes, fs, _ = orc.encode(w.K, [0], w.seq_lens, 0, r32, ck)
+    fs16 = orc.round_factors_f16(fs)
+    assert (fs16.view(np.uint32) == fs.astype(np.float16).astype(np.float32).view(np.uint32)).all()
+    assert (orc.round_factors_f16(fs16).view(np.uint32) == fs16.view(np.uint32)).all()
+    n = int(w.seq_lens[0])
+    live = fs[0, :, :n]
+    assert (np.abs(fs16[0, :, :n] - live) <= 2.0 ** -11 * np.abs(live)).all() and (fs16 != fs).any()
+    sm = 1 / math.sqrt(128)
+    s32, qp, dot, pop = orc.estimate_scores(w.q, codes, fs, None, ck, None, w.seq_lens, 0, r32, sm)
+    s16, _, _, _ = orc.estimate_scores(w.q, codes, fs16, None, ck, None, w.seq_lens, 0, r32, sm)
+    const = (qp["q_ck"] - qp["cq_ck"])[..., None].astype(np.float64) * sm        # Eq.2 terms that carry no factor
+    est = s32[..., :n].astype(np.float64) - const
+    assert (np.abs(s16[..., :n].astype(np.float64) - s32[..., :n]) <= 2.0 ** -11 * np.abs(est) * (1 + 1e-3) + 1e-6).all()
+    assert (128 / 8 + 2) / (2 * 128 * 2) == pytest.approx(0.035, abs=5e-4)
