@@ -15,8 +15,8 @@
  *   - Calls only ENQUEUE work on the given stream (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream) and never synchronise the device.  Token counts are read from device
  *     memory (rbq_index.n_indexed / n_total), so no host read-back happens inside a decode step.
- *   - Layouts are row-major and contiguous except K/V, which carry element strides.  head_dim must
- *     be 128 (64/256: RBQ_ERR_UNSUPPORTED).  n_q_heads must be a multiple of n_kv_heads, with
+ *   - Layouts are row-major and contiguous except K/V, which carry element strides.  head_dim is 64,
+ *     128 or 256 (other multiples of 32: RBQ_ERR_UNSUPPORTED).  n_q_heads must be a multiple of n_kv_heads, with
  *     group size G = n_q_heads/n_kv_heads in {1, 2, 4} (8: RBQ_ERR_UNSUPPORTED).  Inputs are assumed finite.
  *   - There is no CPU fallback and no backend dispatch: without a CUDA device every compute call
  *     fails with RBQ_ERR_CUDA.
@@ -44,14 +44,14 @@ typedef enum {
   RBQ_ERR_CUDA = -4
 } rbq_status;
 
-typedef enum { RBQ_F32 = 0, RBQ_BF16 = 1 } rbq_dtype;
+typedef enum { RBQ_F32 = 0, RBQ_BF16 = 1, RBQ_F16 = 2 /* factor_dtype only */ } rbq_dtype;
 typedef enum { RBQ_ROT_DENSE = 0, RBQ_ROT_WH = 1 } rbq_rot_kind;
 /* EXACT: canonical fp32 order (R1) -> codes/factors bit-identical to the oracle.
  * FAST : rotation on the tcgen05 tensor cores (bf16 hi/lo split, fp32 accumulate in TMEM: the kernel
  *        takes all 512 TMEM columns of its SM while it runs); codes may differ only where
- *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  Built for bf16 K/V (both
- *        rotation kinds: the Walsh-Hadamard rotation runs as its dense matrix); fp32 K/V:
- *        rbq_create returns RBQ_ERR_UNSUPPORTED. */
+ *        |y_j| <= 1e-5 ||x||, factors within 1e-5 relative.  Built for bf16 K/V and head_dim 128 (both
+ *        rotation kinds: the Walsh-Hadamard rotation runs as its dense matrix); fp32 K/V or head_dim
+ *        64 / 256: rbq_create returns RBQ_ERR_UNSUPPORTED. */
 typedef enum { RBQ_ENC_EXACT = 0, RBQ_ENC_FAST = 1 } rbq_enc_mode;
 
 /* flags of rbq_encode_keys */
@@ -69,6 +69,9 @@ typedef struct {
   const float* rot;          /* DEVICE. DENSE: P[D][D] row-major, y_j = sum_i x_i P[i][j] (L149); */
                              /*         WH   : s[D] in {-1,+1}, y = H(s.*x)/sqrt(D), H Sylvester  */
   int32_t enc_mode;          /* rbq_enc_mode                                                     */
+  int32_t factor_dtype;      /* rbq_dtype of rbq_index.f_scale: RBQ_F32 (default) or RBQ_F16 -- the paper's 2-byte     */
+                             /* correction factor (L752, L756-766: 3.5 % index overhead); the factor is computed in  */
+                             /* fp32 exactly as before and rounded to binary16 (RNE) when stored                      */
 } rbq_config;
 
 typedef struct {             /* K/V cache; strides in ELEMENTS; one row = D contiguous elements  */
@@ -79,8 +82,9 @@ typedef struct {             /* K/V cache; strides in ELEMENTS; one row = D cont
 
 typedef struct {
   uint32_t* codes;           /* [B][Hkv][Lcap][D/32]; bit (j%32) of word j/32 = [y_j > 0] (L270, L485) */
-  float*    f_scale;         /* [B][Hkv][Lcap] = ||k-c_k||^2 / ||(k-c_k)P||_1 = ||k-c_k|| / <c',P^T k_c> */
-                             /*   (Eq.18); 0 when k == c_k                             */
+  void*     f_scale;         /* [B][Hkv][Lcap] = ||k-c_k||^2 / ||(k-c_k)P||_1 = ||k-c_k|| / <c',P^T k_c> */
+                             /*   (Eq.18); 0 when k == c_k; float, or IEEE binary16 when   */
+                             /*   factor_dtype = RBQ_F16                                              */
   float*    f_bias;          /* [B][Hq][Lcap] = <c_q[b,h], k_t> (L89); NULL iff c_q is NULL      */
   float*    c_k;             /* [B][Hkv][D] key centroids (Alg.1 line 4, L116)                   */
   const float* c_q;          /* [B][Hq][D] query centroids or NULL (= zero centroid)             */

@@ -23,7 +23,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = Path(os.environ["RBQ_B200_LIB"]) if os.environ.get("RBQ_B200_LIB") else _HERE / "librbq_b200.so"
 _lib = None
 
-RBQ_F32, RBQ_BF16 = 0, 1
+RBQ_F32, RBQ_BF16, RBQ_F16 = 0, 1, 2
 RBQ_ROT_DENSE, RBQ_ROT_WH = 0, 1
 RBQ_ENC_EXACT, RBQ_ENC_FAST = 0, 1
 RBQ_CK_GIVEN = 1
@@ -44,7 +44,7 @@ class rbq_config(C.Structure):
     _fields_ = [("batch", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("max_tokens", C.c_int32), ("flush_tokens", C.c_int32), ("kv_dtype", C.c_int32),
                 ("q_dtype", C.c_int32), ("out_dtype", C.c_int32), ("sm_scale", C.c_float), ("rot_kind", C.c_int32),
-                ("rot", C.c_void_p), ("enc_mode", C.c_int32)]
+                ("rot", C.c_void_p), ("enc_mode", C.c_int32), ("factor_dtype", C.c_int32)]
 
 
 class rbq_kv(C.Structure):
@@ -238,7 +238,7 @@ class RaBitQCache:
 
     def __init__(self, batch, n_q_heads, n_kv_heads, max_tokens, rot: torch.Tensor, *, head_dim=128, flush_tokens=0,
                  kv_dtype=torch.bfloat16, q_dtype=None, out_dtype=None, sm_scale=0.0, rot_kind=RBQ_ROT_DENSE,
-                 enc_mode=RBQ_ENC_EXACT, with_cq=False, device="cuda", interleave_kv=True):
+                 enc_mode=RBQ_ENC_EXACT, with_cq=False, device="cuda", interleave_kv=True, factor_dtype=torch.float32):
         self.dev = torch.device(device)
         self.B, self.Hq, self.Hkv, self.D, self.Lcap = batch, n_q_heads, n_kv_heads, head_dim, max_tokens
         self.kv_dtype = kv_dtype
@@ -247,7 +247,7 @@ class RaBitQCache:
         self.rot = rot.to(self.dev, torch.float32).contiguous()
         self.cfg = rbq_config(batch, n_q_heads, n_kv_heads, head_dim, max_tokens, flush_tokens, _dt(kv_dtype),
                               _dt(self.q_dtype), _dt(self.out_dtype), float(sm_scale), rot_kind,
-                              self.rot.data_ptr(), enc_mode)
+                              self.rot.data_ptr(), enc_mode, RBQ_F16 if factor_dtype == torch.float16 else RBQ_F32)
         self.ctx = rbq_create(self.cfg)
         self.ws = torch.empty(rbq_workspace_bytes(self.ctx), dtype=torch.uint8, device=self.dev)
         rbq_set_workspace(self.ctx, self.ws)
@@ -261,7 +261,7 @@ class RaBitQCache:
             self.K = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
             self.V = torch.zeros(batch, n_kv_heads, max_tokens, head_dim, dtype=kv_dtype, **z)
         self.codes = torch.zeros(batch, n_kv_heads, max_tokens, head_dim // 32, dtype=torch.int32, **z)
-        self.f_scale = torch.zeros(batch, n_kv_heads, max_tokens, dtype=torch.float32, **z)
+        self.f_scale = torch.zeros(batch, n_kv_heads, max_tokens, dtype=factor_dtype, **z)   # float32 or float16
         self.c_k = torch.zeros(batch, n_kv_heads, head_dim, dtype=torch.float32, **z)
         self.c_q = torch.zeros(batch, n_q_heads, head_dim, dtype=torch.float32, **z) if with_cq else None
         self.f_bias = torch.zeros(batch, n_q_heads, max_tokens, dtype=torch.float32, **z) if with_cq else None

@@ -24,9 +24,10 @@ void layout_workspace(rbq_ctx* c) {
   c->off_gdone = take(B * Hkv * sizeof(int32_t));
   c->off_rowmax = take(rows * sizeof(uint32_t));
   c->off_part = take(rbq_attention_part_bytes(c));
-  c->off_stage_q = take(rows * RBQ_D * sizeof(float));
-  c->off_stage_out = take(rows * RBQ_D * sizeof(float));
-  c->off_centroid = take(B * Hkv * 64 * RBQ_D * sizeof(double));
+  const size_t D = g.head_dim;
+  c->off_stage_q = take(rows * D * sizeof(float));
+  c->off_stage_out = take(rows * D * sizeof(float));
+  c->off_centroid = take(B * Hkv * 64 * D * sizeof(double));
   c->off_flags = take(sizeof(uint32_t));
   c->total_bytes = off;
 }
@@ -35,7 +36,7 @@ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 
 int check_kv(rbq_ctx* ctx, const rbq_kv* kv) {
   if (!kv || !kv->k || !kv->v) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: null pointer");
-  if (kv->stride_t < RBQ_D || (kv->stride_t % 8) || (kv->stride_h % 8) || (kv->stride_b % 8))
+  if (kv->stride_t < ctx->cfg.head_dim || (kv->stride_t % 8) || (kv->stride_h % 8) || (kv->stride_b % 8))
     RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: strides must be multiples of 8 elements and stride_t >= head_dim");
   if (!aligned16(kv->k) || !aligned16(kv->v)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "rbq_kv: k/v must be 16-byte aligned");
   return RBQ_OK;
@@ -74,7 +75,8 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
   *out = nullptr;
   if (cfg->batch <= 0 || cfg->n_q_heads <= 0 || cfg->n_kv_heads <= 0 || cfg->max_tokens <= 0) return RBQ_ERR_INVALID_ARG;
   if (cfg->n_q_heads % cfg->n_kv_heads) return RBQ_ERR_INVALID_ARG;
-  if (cfg->head_dim != RBQ_D) return (cfg->head_dim == 64 || cfg->head_dim == 256) ? RBQ_ERR_UNSUPPORTED : RBQ_ERR_INVALID_ARG;
+  if (cfg->head_dim != 64 && cfg->head_dim != 128 && cfg->head_dim != 256)
+    return (cfg->head_dim > 0 && cfg->head_dim % 32 == 0) ? RBQ_ERR_UNSUPPORTED : RBQ_ERR_INVALID_ARG;
   const int G = cfg->n_q_heads / cfg->n_kv_heads;
   if (G != 1 && G != 2 && G != 4) return RBQ_ERR_UNSUPPORTED;
   if (cfg->max_tokens % 4) return RBQ_ERR_INVALID_ARG;
@@ -82,8 +84,9 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
   for (int d : {cfg->kv_dtype, cfg->q_dtype, cfg->out_dtype})
     if (d != RBQ_F32 && d != RBQ_BF16) return RBQ_ERR_INVALID_ARG;
   if (cfg->rot_kind != RBQ_ROT_DENSE && cfg->rot_kind != RBQ_ROT_WH) return RBQ_ERR_INVALID_ARG;
+  if (cfg->factor_dtype != RBQ_F32 && cfg->factor_dtype != RBQ_F16) return RBQ_ERR_INVALID_ARG;
   // tensor-core rotation: built for bf16 K/V (either rotation kind: the WH rotation runs as its dense matrix)
-  if (cfg->enc_mode == RBQ_ENC_FAST && cfg->kv_dtype != RBQ_BF16) return RBQ_ERR_UNSUPPORTED;
+  if (cfg->enc_mode == RBQ_ENC_FAST && (cfg->kv_dtype != RBQ_BF16 || cfg->head_dim != 128)) return RBQ_ERR_UNSUPPORTED;
   if (cfg->enc_mode != RBQ_ENC_EXACT && cfg->enc_mode != RBQ_ENC_FAST) return RBQ_ERR_INVALID_ARG;
   if (!cfg->rot || !(cfg->sm_scale >= 0.0f)) return RBQ_ERR_INVALID_ARG;
   int dev = 0, sms = 0;
@@ -351,8 +354,8 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
   if (!q_host || !out_host || !cache || !idx) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q_host/out_host/cache/idx null");
   cudaStream_t s = (cudaStream_t)stream;
   const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads;
-  const size_t qb = rows * RBQ_D * (ctx->cfg.q_dtype == RBQ_BF16 ? 2 : 4);
-  const size_t ob = rows * RBQ_D * (ctx->cfg.out_dtype == RBQ_BF16 ? 2 : 4);
+  const size_t qb = rows * ctx->cfg.head_dim * (ctx->cfg.q_dtype == RBQ_BF16 ? 2 : 4);
+  const size_t ob = rows * ctx->cfg.head_dim * (ctx->cfg.out_dtype == RBQ_BF16 ? 2 : 4);
   void* dq = ws_ptr<char>(ctx, ctx->off_stage_q);
   void* dout = ws_ptr<char>(ctx, ctx->off_stage_out);
   // out_host in pinned (page-locked, mapped) memory: the merge of S7 stores the result straight into it over PCIe and the

@@ -173,10 +173,15 @@ constexpr int GA_WARPS = RBQ_GA_WARPS;
 constexpr int GA_THREADS = GA_WARPS * 32;
 constexpr int GA_STAGES = RBQ_GA_STAGES;
 constexpr int GA_TILE = 16;                                   // rows per warp tile
-constexpr int GA_TILE_BYTES = GA_TILE * RBQ_D * 2;            // 4 KB per operand
-constexpr int GA_STAGE_BYTES = 2 * GA_TILE_BYTES;             // K + V
-constexpr int GA_SMEM = GA_WARPS * GA_STAGES * GA_STAGE_BYTES;   // 192 KB
-constexpr int GA_PART = RBQ_D + 4;                            // floats per (partial, head): o[128], m (base-2 units), l, pad (16-byte rows)
+// per head_dim D (template parameter, 64 or 128; D = 256 takes the FP32-pipe kernel below):
+template <int D> struct GaCfg {
+  static constexpr int ROW_BYTES = D * 2;                     // one bf16 K or V row
+  static constexpr int CPR = D / 8;                           // 16-byte chunks per row
+  static constexpr int TILE_BYTES = GA_TILE * ROW_BYTES;      // 4 KB per operand at D = 128
+  static constexpr int STAGE_BYTES = 2 * TILE_BYTES;          // K + V
+  static constexpr int SMEM = GA_WARPS * GA_STAGES * STAGE_BYTES;   // 192 KB at D = 128
+  static constexpr int PART = D + 4;                          // floats per (partial, head): o[D], m (base-2 units), l, pad (16-byte rows)
+};
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
@@ -203,8 +208,9 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&v);
 }
 
-// grid = number of SMs (persistent), GA_THREADS threads, GA_SMEM dynamic shared memory.
+// grid = number of SMs (persistent), GA_THREADS threads, GaCfg<D>::SMEM dynamic shared memory.
 // part: [gridDim.x + ngroups][G][GA_PART]; the partial of (CTA c, group gi) lives in slot c + gi.
+template <int D>
 __global__ void __launch_bounds__(GA_THREADS, 1)
 attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ K, const __nv_bfloat16* __restrict__ V,
                    long long sb, long long sh, long long st, const uint32_t* __restrict__ ulist,
@@ -212,6 +218,9 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
                    const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int Lcap, float scale_log2,
                    float* __restrict__ part, int32_t* __restrict__ gdone, void* __restrict__ out, int out_bf16,
                    float* __restrict__ lse) {
+  using C = GaCfg<D>;
+  constexpr int GA_TILE_BYTES = C::TILE_BYTES, GA_STAGE_BYTES = C::STAGE_BYTES, GA_PART = C::PART, RB = C::ROW_BYTES, CPR = C::CPR;
+  constexpr int LSH = (D == 64) ? 3 : 4;                       // log2(CPR)
   extern __shared__ __align__(128) unsigned char ga_smem[];
   __shared__ int s_start[AT_MAX_GROUPS + 1];
   __shared__ int s_warp[GA_WARPS];
@@ -227,11 +236,11 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
     for (int gq = 0; gq < ngroups; ++gq) {
       if (s_start[gq + 1] != s_start[gq]) continue;
-      for (int hd = tid; hd < G * RBQ_D; hd += GA_THREADS) {
-        const size_t orow = (size_t)(gq / Hkv) * Hq + (size_t)(gq % Hkv) * G + hd / RBQ_D;
-        if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * RBQ_D + hd % RBQ_D] = __float2bfloat16_rn(0.0f);
-        else reinterpret_cast<float*>(out)[orow * RBQ_D + hd % RBQ_D] = 0.0f;
-        if (lse && hd % RBQ_D == 0) lse[orow] = -INFINITY;
+      for (int hd = tid; hd < G * D; hd += GA_THREADS) {
+        const size_t orow = (size_t)(gq / Hkv) * Hq + (size_t)(gq % Hkv) * G + hd / D;
+        if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * D + hd % D] = __float2bfloat16_rn(0.0f);
+        else reinterpret_cast<float*>(out)[orow * D + hd % D] = 0.0f;
+        if (lse && hd % D == 0) lse[orow] = -INFINITY;
       }
     }
   }
@@ -261,19 +270,19 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     const uint32_t* ul = ulist + (size_t)gi * Lcap;
 
     // A operand: Q rows of the group's heads (rows >= G are zero)
-    uint32_t qa[8][2];
+    uint32_t qa[D / 16][2];
     {
-      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * RBQ_D);
+      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * D);
 #pragma unroll
-      for (int ks = 0; ks < 8; ++ks) {
+      for (int ks = 0; ks < D / 16; ++ks) {
         qa[ks][0] = (g4 < G) ? qp[8 * ks + t4] : 0u;
         qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
       }
     }
     float m_run = -INFINITY, l_run = 0.0f;
-    float o[16][4];
+    float o[D / 8][4];
 #pragma unroll
-    for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.0f; o[nt][1] = 0.0f; o[nt][2] = 0.0f; o[nt][3] = 0.0f; }
+    for (int nt = 0; nt < D / 8; ++nt) { o[nt][0] = 0.0f; o[nt][1] = 0.0f; o[nt][2] = 0.0f; o[nt][3] = 0.0f; }
 
     const int ntiles = (e - a + GA_TILE - 1) / GA_TILE;
     const int my_tiles = (ntiles > warp) ? (ntiles - warp + GA_WARPS - 1) / GA_WARPS : 0;
@@ -288,11 +297,11 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     auto issue = [&](int i, uint32_t ent) {
       const uint32_t sbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES);
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const int row = 2 * k + (lane >> 4), ch = lane & 15;
+      for (int k = 0; k < GA_TILE * CPR / 32; ++k) {           // 32 lanes cover 32 / CPR rows per step
+        const int row = (32 / CPR) * k + (lane >> LSH), ch = lane & (CPR - 1);
         const uint32_t re = __shfl_sync(0xffffffffu, ent, row);
         const long long off = (long long)(re & 0x0FFFFFFFu) * st + ch * 8;
-        const uint32_t d = sbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4));
+        const uint32_t d = sbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4));
         cp_async16(d, Kb + off);
         cp_async16(d + GA_TILE_BYTES, Vb + off);
       }
@@ -328,10 +337,10 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         s[nt][0] = 0.0f; s[nt][1] = 0.0f; s[nt][2] = 0.0f; s[nt][3] = 0.0f;
         const int row = nt * 8 + (lane & 7);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < D / 32; ++j) {
           uint32_t bf[4];
           const int ch = 4 * j + (lane >> 3);
-          ldsm_x4(bf, kbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4)));
+          ldsm_x4(bf, kbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4)));
           mma_bf16(s[nt], qa[2 * j][0], 0u, qa[2 * j][1], 0u, bf[0], bf[1]);
           mma_bf16(s[nt], qa[2 * j + 1][0], 0u, qa[2 * j + 1][1], 0u, bf[2], bf[3]);
         }
@@ -362,10 +371,10 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       const uint32_t pb2 = pack_bf16(p10 - rbq_bf16lo(pa2), p11 - rbq_bf16hi(pa2));
       // O = O * resc + P V
 #pragma unroll
-      for (int c2 = 0; c2 < 8; ++c2) {
+      for (int c2 = 0; c2 < D / 16; ++c2) {
         uint32_t bf[4];
         const int row = (lane & 7) + ((lane >> 3) & 1) * 8, ch = 2 * c2 + (lane >> 4);
-        ldsm_x4_t(bf, vbase + (uint32_t)(row * 256 + ((ch ^ (row & 7)) << 4)));
+        ldsm_x4_t(bf, vbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4)));
         o[2 * c2][0] *= resc; o[2 * c2][1] *= resc;
         o[2 * c2 + 1][0] *= resc; o[2 * c2 + 1][1] *= resc;
         mma_bf16(o[2 * c2], pa0, 0u, pa2, 0u, bf[0], bf[1]);
@@ -385,26 +394,26 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     if (g4 < G) {
       float* dst = stg + ((size_t)warp * G + g4) * GA_PART;
 #pragma unroll
-      for (int nt = 0; nt < 16; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
-      if (t4 == 0) { dst[RBQ_D] = m_run; dst[RBQ_D + 1] = l_run; }
+      for (int nt = 0; nt < D / 8; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
+      if (t4 == 0) { dst[D] = m_run; dst[D + 1] = l_run; }
     }
     __syncthreads();
     float* pdst = part + (size_t)(blockIdx.x + gi) * G * GA_PART;
-    for (int idx = tid; idx < G * RBQ_D; idx += GA_THREADS) {
-      const int h = idx / RBQ_D, d = idx % RBQ_D;
+    for (int idx = tid; idx < G * D; idx += GA_THREADS) {
+      const int h = idx / D, d = idx % D;
       float mm = -INFINITY;
 #pragma unroll
-      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[((size_t)w * G + h) * GA_PART + RBQ_D]);
+      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[((size_t)w * G + h) * GA_PART + D]);
       float oo = 0.0f, ll = 0.0f;
 #pragma unroll
       for (int w = 0; w < GA_WARPS; ++w) {
         const float* sp = stg + ((size_t)w * G + h) * GA_PART;
-        const float f = (sp[RBQ_D] == -INFINITY) ? 0.0f : exp2f(sp[RBQ_D] - mm);
+        const float f = (sp[D] == -INFINITY) ? 0.0f : exp2f(sp[D] - mm);
         oo = fmaf(f, sp[d], oo);
-        ll = fmaf(f, sp[RBQ_D + 1], ll);
+        ll = fmaf(f, sp[D + 1], ll);
       }
       pdst[(size_t)h * GA_PART + d] = oo;
-      if (d == 0) { pdst[(size_t)h * GA_PART + RBQ_D] = mm; pdst[(size_t)h * GA_PART + RBQ_D + 1] = ll; }
+      if (d == 0) { pdst[(size_t)h * GA_PART + D] = mm; pdst[(size_t)h * GA_PART + D + 1] = ll; }
     }
     // ---- arrival: the last CTA that finishes a group merges the group's partials into out / lse -------------------------
     __threadfence();
@@ -418,17 +427,19 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     if (s_last) {
       __threadfence();
       float* s_f = stg;                                        // [G][GA_THREADS]: factor 2^(m - max) of slot c
-      float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [128] second half's partial sums
+      constexpr int TPH = D / 4, ITEMS = RBQ_MAX_G * TPH;     // threads per head (4 dims each), (head, dim group) items
+      constexpr int NH = GA_THREADS / ITEMS;                   // slot subsets worked on in parallel (2 at D = 128, 4 at D = 64)
+      float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [NH - 1][ITEMS] partial sums of subsets 1 ..
       const int clo = s_clo, chi = s_chi;
       // thread tid owns slot tid: per-head maximum and normaliser by block reductions (warp shuffles + one shared round)
-      float* s_red = stg + 2 * RBQ_MAX_G * GA_THREADS + 4 * RBQ_D;   // [2][RBQ_MAX_G][GA_WARPS]
+      float* s_red = stg + 2 * RBQ_MAX_G * GA_THREADS + 4 * (NH > 1 ? (NH - 1) * ITEMS : 1);   // [2][RBQ_MAX_G][GA_WARPS]
       float pm[RBQ_MAX_G], pl[RBQ_MAX_G];
 #pragma unroll
       for (int h = 0; h < RBQ_MAX_G; ++h) {
         pm[h] = -INFINITY; pl[h] = 0.0f;
         if (h < G && touches) {
           const float* pp = part + ((size_t)(tid + gi) * G + h) * GA_PART;
-          pm[h] = __ldcg(pp + RBQ_D); pl[h] = __ldcg(pp + RBQ_D + 1);
+          pm[h] = __ldcg(pp + D); pl[h] = __ldcg(pp + D + 1);
         }
       }
 #pragma unroll
@@ -454,9 +465,8 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         if (lane == 0) s_red[(RBQ_MAX_G + h) * GA_WARPS + warp] = fl;
       }
       __syncthreads();
-      constexpr int NH = GA_THREADS >= 256 ? 2 : 1;             // slot halves worked on in parallel
-      const int item = tid & 127, half = tid >> 7, d4 = (item & 31) * 4;
-      const int h = (half < NH) ? (item >> 5) : RBQ_MAX_G;      // threads beyond NH * 128 only take part in the barriers
+      const int item = tid % ITEMS, half = tid / ITEMS, d4 = (item % TPH) * 4;
+      const int h = (half < NH) ? (item / TPH) : RBQ_MAX_G;     // threads beyond NH * ITEMS only take part in the barriers
       float mm = -INFINITY;
 #pragma unroll
       for (int hh = 0; hh < RBQ_MAX_G; ++hh) mm = (hh == h) ? mall[hh] : mm;
@@ -484,11 +494,12 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 #pragma unroll
         for (int w = 0; w < GA_WARPS; ++w) ll += s_red[(RBQ_MAX_G + h) * GA_WARPS + w];
       }
-      if (half == 1 && NH == 2) s_o[item] = acc;
+      if (half >= 1 && half < NH) s_o[(half - 1) * ITEMS + item] = acc;
       __syncthreads();
       if (half == 0 && h < G) {
-        if (NH == 2) {
-          const float4 o2 = s_o[item];
+#pragma unroll
+        for (int k = 1; k < NH; ++k) {
+          const float4 o2 = s_o[(k - 1) * ITEMS + item];
           acc.x += o2.x; acc.y += o2.y; acc.z += o2.z; acc.w += o2.w;
         }
         const bool empty = !(ll > 0.0f);
@@ -497,8 +508,8 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         const float r4[4] = {acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv};
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * RBQ_D + d4 + k] = __float2bfloat16_rn(r4[k]);
-          else reinterpret_cast<float*>(out)[orow * RBQ_D + d4 + k] = r4[k];
+          if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * D + d4 + k] = __float2bfloat16_rn(r4[k]);
+          else reinterpret_cast<float*>(out)[orow * D + d4 + k] = r4[k];
         }
         if (lse && d4 == 0) lse[orow] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(ll);
       }
@@ -508,39 +519,42 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   }
 }
 
-// ---- FP32-pipe kernel for fp32 K/V or q (parity config 0): split-K over the group's union list ---------------------
+// ---- FP32-pipe kernel for fp32 K/V or q (parity config 0) and for head_dim 256: split-K over the group's union list ------
 constexpr int AT_THREADS = 256;
 constexpr int AT_WARPS = AT_THREADS / 32;
 constexpr int AT_CHUNK = AT_WARPS * 32;       // union rows per chunk: one 32-row strip per warp
-constexpr int AT_PART = RBQ_D + 2;            // floats per partial: o[128], m, l
 
-struct Row8 { float v[8]; };
-
-__device__ __forceinline__ Row8 load8(const __nv_bfloat16* p) {
-  const uint4 u = *reinterpret_cast<const uint4*>(p);
-  Row8 r;
-  r.v[0] = rbq_bf16lo(u.x); r.v[1] = rbq_bf16hi(u.x); r.v[2] = rbq_bf16lo(u.y); r.v[3] = rbq_bf16hi(u.y);
-  r.v[4] = rbq_bf16lo(u.z); r.v[5] = rbq_bf16hi(u.z); r.v[6] = rbq_bf16lo(u.w); r.v[7] = rbq_bf16hi(u.w);
-  return r;
+// N consecutive elements of a row as floats, in 4-element pieces (8-byte loads for bf16, 16-byte loads for fp32)
+template <int N>
+__device__ __forceinline__ void load_row(const __nv_bfloat16* p, float (&v)[N]) {
+#pragma unroll
+  for (int k = 0; k < N / 4; ++k) {
+    const uint2 u = *reinterpret_cast<const uint2*>(p + 4 * k);
+    v[4 * k] = rbq_bf16lo(u.x); v[4 * k + 1] = rbq_bf16hi(u.x); v[4 * k + 2] = rbq_bf16lo(u.y); v[4 * k + 3] = rbq_bf16hi(u.y);
+  }
 }
-__device__ __forceinline__ Row8 load8(const float* p) {
-  const float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
-  Row8 r;
-  r.v[0] = a.x; r.v[1] = a.y; r.v[2] = a.z; r.v[3] = a.w; r.v[4] = b.x; r.v[5] = b.y; r.v[6] = b.z; r.v[7] = b.w;
-  return r;
+template <int N>
+__device__ __forceinline__ void load_row(const float* p, float (&v)[N]) {
+#pragma unroll
+  for (int k = 0; k < N / 4; ++k) {
+    const float4 a = *reinterpret_cast<const float4*>(p + 4 * k);
+    v[4 * k] = a.x; v[4 * k + 1] = a.y; v[4 * k + 2] = a.z; v[4 * k + 3] = a.w;
+  }
 }
 
 // grid = (max chunks per group, B*Hq rows).  Chunk ch of row (b,h) covers union rows [ch*256, ch*256+256) of the
-// row's KV group; rows whose head-mask bit is clear are skipped.  part: [rows][max_chunks][AT_PART].
-template <typename T, typename TQ>
+// row's KV group; rows whose head-mask bit is clear are skipped.  part: [rows][max_chunks][D + 2] (o, m, l).
+template <typename T, typename TQ, int D>
 __global__ void __launch_bounds__(AT_THREADS)
 attn_simt_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __restrict__ V, long long sb, long long sh,
                  long long st, const uint32_t* __restrict__ ulist, const int32_t* __restrict__ ucount,
                  const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total, int Hq, int Hkv, int Lcap,
                  float sm_scale, int max_chunks, float* __restrict__ part) {
+  constexpr int AT_PART = D + 2, DPL = D / 16;                // dims per lane: a half-warp covers a row
+  constexpr int NJ = DPL >= 16 ? 2 : 4;                       // rows per half-warp and step (register budget)
   __shared__ float s_part[AT_WARPS][AT_PART];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int half = lane >> 4, c = lane & 15;                  // half-warp per row, 8 dims per lane
+  const int half = lane >> 4, c = lane & 15;
   const int G = Hq / Hkv;
   const int row = blockIdx.y, b = row / Hq, h = row % Hq, g = h / G, hl = h % G;
   const int gi = b * Hkv + g;
@@ -549,7 +563,7 @@ attn_simt_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __r
   const int ch = blockIdx.x;
   float* dst = part + ((size_t)row * max_chunks + ch) * AT_PART;
   if (ch * AT_CHUNK >= na) {
-    if (tid == 0) { dst[RBQ_D] = -INFINITY; dst[RBQ_D + 1] = 0.0f; }
+    if (tid == 0) { dst[D] = -INFINITY; dst[D + 1] = 0.0f; }
     return;
   }
   const int i0 = ch * AT_CHUNK + warp * 32;
@@ -558,48 +572,48 @@ attn_simt_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __r
   const T* Vb = V + (long long)b * sb + (long long)g * sh;
   const uint32_t* ul = ulist + (size_t)gi * Lcap;
 
-  Row8 qv;
+  float qv[DPL];
   {
-    const TQ* qp = q + ((size_t)row * RBQ_D + c * 8);
+    const TQ* qp = q + ((size_t)row * D + c * DPL);
 #pragma unroll
-    for (int d = 0; d < 8; ++d) qv.v[d] = rbq_ld_elem(qp, d);
+    for (int d = 0; d < DPL; ++d) qv[d] = rbq_ld_elem(qp, d);
   }
   uint32_t my_ent = 0u;                                         // token | mask << 28 ; mask bit clear = not attended by this head
   if (lane < nw) {
     const int it = i0 + lane;
     my_ent = (it < usel) ? ul[it] : ((uint32_t)(nidx + (it - usel)) | (0xFu << 28));
   }
-  float m = -INFINITY, l = 0.0f, acc[8];
+  float m = -INFINITY, l = 0.0f, acc[DPL];
 #pragma unroll
-  for (int d = 0; d < 8; ++d) acc[d] = 0.0f;
+  for (int d = 0; d < DPL; ++d) acc[d] = 0.0f;
 
-  for (int base = 0; base < nw; base += 8) {
-    Row8 kr[4], vr[4];
-    bool ok[4];
+  for (int base = 0; base < nw; base += 2 * NJ) {
+    float kr[NJ][DPL], vr[NJ][DPL];
+    bool ok[NJ];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NJ; ++j) {
       const int item = base + 2 * j + half;
       const uint32_t ent = __shfl_sync(0xffffffffu, my_ent, item & 31);
       ok[j] = (item < nw) && ((ent >> (28 + hl)) & 1u);
-      const long long off = (long long)(ent & 0x0FFFFFFFu) * st + c * 8;
-      kr[j] = load8(Kb + off);                                  // masked items read a valid row: harmless
-      vr[j] = load8(Vb + off);
+      const long long off = (long long)(ent & 0x0FFFFFFFu) * st + c * DPL;
+      load_row<DPL>(Kb + off, kr[j]);                           // masked items read a valid row: harmless
+      load_row<DPL>(Vb + off, vr[j]);
     }
-    float s[4];
+    float s[NJ];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NJ; ++j) {
       float d0 = 0.0f;
 #pragma unroll
-      for (int d = 0; d < 8; ++d) d0 = fmaf(qv.v[d], kr[j].v[d], d0);
+      for (int d = 0; d < DPL; ++d) d0 = fmaf(qv[d], kr[j][d], d0);
       s[j] = d0;
     }
 #pragma unroll
     for (int o = 8; o > 0; o >>= 1)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) s[j] += __shfl_xor_sync(0xffffffffu, s[j], o);
+      for (int j = 0; j < NJ; ++j) s[j] += __shfl_xor_sync(0xffffffffu, s[j], o);
     float gmax = -INFINITY;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NJ; ++j) {
       s[j] = ok[j] ? s[j] * sm_scale : -INFINITY;
       gmax = fmaxf(gmax, s[j]);
     }
@@ -609,88 +623,118 @@ attn_simt_kernel(const TQ* __restrict__ q, const T* __restrict__ K, const T* __r
     const float resc = __expf(m - m_use);                       // m = -inf -> 0
     l *= resc;
 #pragma unroll
-    for (int d = 0; d < 8; ++d) acc[d] *= resc;
+    for (int d = 0; d < DPL; ++d) acc[d] *= resc;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < NJ; ++j) {
       const float p = __expf(s[j] - m_use);                     // masked: exp(-inf) = 0
       l += p;
 #pragma unroll
-      for (int d = 0; d < 8; ++d) acc[d] = fmaf(p, vr[j].v[d], acc[d]);
+      for (int d = 0; d < DPL; ++d) acc[d] = fmaf(p, vr[j][d], acc[d]);
     }
     m = m_new;
   }
   // merge the two half-warps (same m), then the warps of the CTA
   l += __shfl_xor_sync(0xffffffffu, l, 16);
 #pragma unroll
-  for (int d = 0; d < 8; ++d) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], 16);
+  for (int d = 0; d < DPL; ++d) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], 16);
   if (half == 0) {
 #pragma unroll
-    for (int d = 0; d < 8; ++d) s_part[warp][c * 8 + d] = acc[d];
-    if (c == 0) { s_part[warp][RBQ_D] = m; s_part[warp][RBQ_D + 1] = l; }
+    for (int d = 0; d < DPL; ++d) s_part[warp][c * DPL + d] = acc[d];
+    if (c == 0) { s_part[warp][D] = m; s_part[warp][D + 1] = l; }
   }
   __syncthreads();
-  if (tid < RBQ_D) {
+  for (int d = tid; d < D; d += AT_THREADS) {
     float mm = -INFINITY;
 #pragma unroll
-    for (int w = 0; w < AT_WARPS; ++w) mm = fmaxf(mm, s_part[w][RBQ_D]);
+    for (int w = 0; w < AT_WARPS; ++w) mm = fmaxf(mm, s_part[w][D]);
     float o = 0.0f, ll = 0.0f;
 #pragma unroll
     for (int w = 0; w < AT_WARPS; ++w) {
-      const float mw = s_part[w][RBQ_D];
+      const float mw = s_part[w][D];
       const float f = (mw == -INFINITY) ? 0.0f : __expf(mw - mm);
-      o = fmaf(f, s_part[w][tid], o);
-      ll = fmaf(f, s_part[w][RBQ_D + 1], ll);
+      o = fmaf(f, s_part[w][d], o);
+      ll = fmaf(f, s_part[w][D + 1], ll);
     }
-    dst[tid] = o;
-    if (tid == 0) { dst[RBQ_D] = mm; dst[RBQ_D + 1] = ll; }
+    dst[d] = o;
+    if (d == 0) { dst[D] = mm; dst[D + 1] = ll; }
   }
 }
 
-// grid = rows, 128 threads; natural-log units
+// grid = rows, D threads; natural-log units
 template <typename TO>
-__global__ void __launch_bounds__(RBQ_D)
-attn_simt_merge_kernel(const float* __restrict__ part, const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
-                       const int32_t* __restrict__ n_total, int Hq, int Hkv, int max_chunks, TO* __restrict__ out,
-                       float* __restrict__ lse) {
+__global__ void attn_simt_merge_kernel(const float* __restrict__ part, const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
+                                       const int32_t* __restrict__ n_total, int Hq, int Hkv, int D, int max_chunks, TO* __restrict__ out,
+                                       float* __restrict__ lse) {
+  const int AT_PART = D + 2;
   const int row = blockIdx.x, d = threadIdx.x, b = row / Hq, G = Hq / Hkv;
   const int gi = b * Hkv + (row % Hq) / G;
   const int na = ucount[gi] + max(0, n_total[b] - max(0, n_indexed[b]));
   const int nch = min(max_chunks, (na + AT_CHUNK - 1) / AT_CHUNK);
   const float* base = part + (size_t)row * max_chunks * AT_PART;
   float mm = -INFINITY;
-  for (int ch = 0; ch < nch; ++ch) mm = fmaxf(mm, base[(size_t)ch * AT_PART + RBQ_D]);
+  for (int ch = 0; ch < nch; ++ch) mm = fmaxf(mm, base[(size_t)ch * AT_PART + D]);
   float o = 0.0f, l = 0.0f;
   for (int ch = 0; ch < nch; ++ch) {
     const float* p = base + (size_t)ch * AT_PART;
-    const float f = (p[RBQ_D] == -INFINITY) ? 0.0f : __expf(p[RBQ_D] - mm);
+    const float f = (p[D] == -INFINITY) ? 0.0f : __expf(p[D] - mm);
     o = fmaf(f, p[d], o);
-    l = fmaf(f, p[RBQ_D + 1], l);
+    l = fmaf(f, p[D + 1], l);
   }
   const bool empty = !(l > 0.0f);
-  rbq_st_elem(out, (long long)row * RBQ_D + d, empty ? 0.0f : o / l);
+  rbq_st_elem(out, (long long)row * D + d, empty ? 0.0f : o / l);
   if (lse && d == 0) lse[row] = empty ? -INFINITY : mm + logf(l);
 }
 
+template <typename T, typename TQ, int D>
+int launch_simt_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* ulist, const int32_t* ucount,
+                  int max_chunks, float* part, cudaStream_t s) {
+  const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
+  dim3 grid(max_chunks, rows);
+  attn_simt_kernel<T, TQ, D><<<grid, AT_THREADS, 0, s>>>((const TQ*)q, (const T*)kv.k, (const T*)kv.v, kv.sb, kv.sh, kv.st, ulist,
+                                                         ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                         ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->sm_scale, max_chunks, part);
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
 template <typename T, typename TQ>
 int launch_simt(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* ulist, const int32_t* ucount,
                 int max_chunks, float* part, cudaStream_t s) {
-  const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
-  dim3 grid(max_chunks, rows);
-  attn_simt_kernel<T, TQ><<<grid, AT_THREADS, 0, s>>>((const TQ*)q, (const T*)kv.k, (const T*)kv.v, kv.sb, kv.sh, kv.st, ulist,
-                                                      ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
-                                                      ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->sm_scale, max_chunks, part);
-  RBQ_LAUNCH_OK(ctx);
-  return RBQ_OK;
+  switch (ctx->cfg.head_dim) {
+    case 64: return launch_simt_d<T, TQ, 64>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+    case 256: return launch_simt_d<T, TQ, 256>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+    default: return launch_simt_d<T, TQ, 128>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  }
 }
 
 }  // namespace
 
+// tensor-pipe gather: bf16 K/V and q, head_dim 64 or 128 (256: 128 accumulator registers per thread would not fit)
+static bool rbq_attention_uses_mma(const rbq_ctx* ctx) {
+  return ctx->cfg.kv_dtype == RBQ_BF16 && ctx->cfg.q_dtype == RBQ_BF16 && ctx->cfg.head_dim <= 128;
+}
+
+template <int D>
+static int launch_gather_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* ulist,
+                           const int32_t* ucount, int groups, float* part, int32_t* gdone, void* out, float* lse, cudaStream_t s) {
+  auto kern = attn_gather_kernel<D>;
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_GATHER + (D == 64 ? 0 : 1), kern, GaCfg<D>::SMEM);
+  const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the arrival count uses one thread per CTA
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, dim3(nc), dim3(GA_THREADS), (size_t)GaCfg<D>::SMEM, s, (const __nv_bfloat16*)q,
+                                  (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st,
+                                  (const uint32_t*)ulist, (const int32_t*)ucount, (const int32_t*)idx->n_indexed,
+                                  (const int32_t*)idx->n_total, groups, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
+                                  ctx->cfg.max_tokens, ctx->sm_scale * 1.4426950408889634f, part, gdone, out,
+                                  ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse));
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
+
 size_t rbq_attention_part_bytes(const rbq_ctx* ctx) {
   const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads, groups = (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads;
-  const bool mma = ctx->cfg.kv_dtype == RBQ_BF16 && ctx->cfg.q_dtype == RBQ_BF16;
-  if (mma) return ((size_t)ctx->sm_count + groups) * ctx->G * GA_PART * sizeof(float);
+  const size_t D = ctx->cfg.head_dim;
+  if (rbq_attention_uses_mma(ctx)) return ((size_t)ctx->sm_count + groups) * ctx->G * (D + 4) * sizeof(float);
   const size_t max_chunks = ((size_t)ctx->cfg.max_tokens + AT_CHUNK - 1) / AT_CHUNK;
-  return rows * max_chunks * AT_PART * sizeof(float);
+  return rows * max_chunks * (D + 2) * sizeof(float);
 }
 
 int rbq_launch_bits_from_lists(rbq_ctx* ctx, const rbq_index* idx, const int32_t* sel_idx, const int32_t* sel_cnt, uint32_t* bits,
@@ -732,30 +776,23 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   RBQ_LAUNCH_OK(ctx);
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
-  if (kbf && qbf) {
-    RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_GATHER, attn_gather_kernel, GA_SMEM);
-    const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the arrival count uses one thread per CTA
-    RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_gather_kernel, dim3(nc), dim3(GA_THREADS), (size_t)GA_SMEM, s, (const __nv_bfloat16*)q,
-                                    (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st,
-                                    (const uint32_t*)ulist, (const int32_t*)ucount, (const int32_t*)idx->n_indexed,
-                                    (const int32_t*)idx->n_total, groups, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
-                                    ctx->cfg.max_tokens, ctx->sm_scale * 1.4426950408889634f, part, gdone, out,
-                                    ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse));
-    RBQ_LAUNCH_OK(ctx);
-    return RBQ_OK;
+  if (rbq_attention_uses_mma(ctx)) {
+    if (ctx->cfg.head_dim == 64) return launch_gather_d<64>(ctx, q, kv, idx, ulist, ucount, groups, part, gdone, out, lse, s);
+    return launch_gather_d<128>(ctx, q, kv, idx, ulist, ucount, groups, part, gdone, out, lse, s);
   }
   const int max_chunks = (ctx->cfg.max_tokens + AT_CHUNK - 1) / AT_CHUNK;
   int rc;
-  if (kbf) rc = launch_simt<__nv_bfloat16, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  if (kbf && qbf) rc = launch_simt<__nv_bfloat16, __nv_bfloat16>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
+  else if (kbf) rc = launch_simt<__nv_bfloat16, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
   else if (qbf) rc = launch_simt<float, __nv_bfloat16>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
   else rc = launch_simt<float, float>(ctx, q, kv, idx, ulist, ucount, max_chunks, part, s);
   if (rc != RBQ_OK) return rc;
   if (ctx->cfg.out_dtype == RBQ_BF16)
-    attn_simt_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
-                                                  ctx->cfg.n_kv_heads, max_chunks, (__nv_bfloat16*)out, lse);
+    attn_simt_merge_kernel<<<rows, ctx->cfg.head_dim, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                              ctx->cfg.n_kv_heads, ctx->cfg.head_dim, max_chunks, (__nv_bfloat16*)out, lse);
   else
-    attn_simt_merge_kernel<<<rows, RBQ_D, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
-                                                  ctx->cfg.n_kv_heads, max_chunks, (float*)out, lse);
+    attn_simt_merge_kernel<<<rows, ctx->cfg.head_dim, 0, s>>>(part, ucount, idx->n_indexed, idx->n_total, ctx->cfg.n_q_heads,
+                                                              ctx->cfg.n_kv_heads, ctx->cfg.head_dim, max_chunks, (float*)out, lse);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

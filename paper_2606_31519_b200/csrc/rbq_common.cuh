@@ -2,6 +2,7 @@
 // CUDA path only: nothing here is shared with oracle/.
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -64,8 +65,8 @@ struct rbq_ctx {
 
 // per-context "function attribute set" slots (the attribute is per device; a context lives on one device): base ids, each
 // kernel family adds the index of its instantiation
-enum { RBQ_ATTR_QUERY = 0 /* +6 */, RBQ_ATTR_EST = 8 /* +36 */, RBQ_ATTR_TOPP = 48 /* +9 */, RBQ_ATTR_ENC_EXACT = 60 /* +4 */,
-       RBQ_ATTR_FBIAS = 66 /* +2 */, RBQ_ATTR_ENC_FAST = 70, RBQ_ATTR_GATHER = 72 /* +8 */, RBQ_ATTR_ALG3 = 82, RBQ_ATTR_MISC = 84 };
+enum { RBQ_ATTR_QUERY = 0 /* +6 */, RBQ_ATTR_EST = 8 /* +36 */, RBQ_ATTR_TOPP = 48 /* +9 */, RBQ_ATTR_ENC_EXACT = 60 /* +12 */,
+       RBQ_ATTR_FBIAS = 74 /* +6 */, RBQ_ATTR_ENC_FAST = 82, RBQ_ATTR_GATHER = 84 /* +8 */, RBQ_ATTR_ALG3 = 94, RBQ_ATTR_MISC = 96 };
 
 #define RBQ_FAIL(ctx, code, ...)                                   \
   do {                                                             \
@@ -94,6 +95,11 @@ __device__ __forceinline__ float rbq_ld_elem(const __nv_bfloat16* p, long long i
 __device__ __forceinline__ void rbq_st_elem(float* p, long long i, float v) { p[i] = v; }
 __device__ __forceinline__ void rbq_st_elem(__nv_bfloat16* p, long long i, float v) {
   p[i] = __float2bfloat16_rn(v);
+}
+// the per-token factor as stored: fp32, or binary16 (RNE) when rbq_config.factor_dtype = RBQ_F16
+__device__ __forceinline__ void rbq_store_factor(void* f_scale, int f16, size_t i, float v) {
+  if (f16) reinterpret_cast<__half*>(f_scale)[i] = __float2half_rn(v);
+  else reinterpret_cast<float*>(f_scale)[i] = v;
 }
 __device__ __forceinline__ float rbq_bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
 __device__ __forceinline__ float rbq_bf16hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }

@@ -14,7 +14,8 @@ namespace {
 
 constexpr int ENC_TOK = 64;        // tokens per CTA tile
 constexpr int ENC_THREADS = 256;
-constexpr int XS = RBQ_D + 1;      // padded row stride of the x / y tile (bank-conflict-free per-token access)
+// head_dim D is a template parameter (64, 128, 256).  XS = D + 1: padded row stride of the x / y tile (bank-conflict-free
+// per-token access).  The dense P is staged in chunks of KC = min(D, 128) rows (D = 256: two chunks of 128 KB).
 
 // ---- centroid: c_k = mean over t < n of K[b][g][t][:] , fp64 accumulation ------------------------
 // Partial sums over CEN_SPLIT contiguous token ranges, then a fixed-order final sum.  fp64 sums of
@@ -53,13 +54,14 @@ __device__ __forceinline__ void rbq_raw_to_f(const RbqRaw8F& u, float (&v)[8]) {
 // 16-byte pieces) in flight per thread; 4 CTAs per SM keep ~19 MB in flight over the chip.
 constexpr int CEN_THREADS = 256;
 
-template <typename T>
-__global__ void __launch_bounds__(CEN_THREADS, 4)
+template <typename T, int D>
+__global__ void __launch_bounds__(CEN_THREADS, D == 256 ? 2 : 4)
 centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
                         const int32_t* __restrict__ seq_lens, int Hkv, double* __restrict__ part) {
-  __shared__ double s_acc[CEN_THREADS / 16][RBQ_D];
+  constexpr int TPR = D / 8, RPR = CEN_THREADS / TPR;          // threads per row (8 dims each), rows per round
+  __shared__ double s_acc[RPR][D];
   const int bg = blockIdx.x, b = bg / Hkv, g = bg % Hkv, s = blockIdx.y;
-  const int c8 = (threadIdx.x & 15) * 8, r = threadIdx.x >> 4;
+  const int c8 = (threadIdx.x % TPR) * 8, r = threadIdx.x / TPR;
   const int n = seq_lens[b];
   const int per = (n + CEN_SPLIT - 1) / CEN_SPLIT;
   const int t0 = s * per, t1 = min(n, t0 + per);
@@ -68,11 +70,11 @@ centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, lon
   double acc[8];
 #pragma unroll
   for (int d = 0; d < 8; ++d) acc[d] = 0.0;
-  for (int t = t0 + r; t < t1; t += CEN_FLIGHT * (CEN_THREADS / 16)) {
+  for (int t = t0 + r; t < t1; t += CEN_FLIGHT * RPR) {
     decltype(rbq_ldraw8(base)) raw[CEN_FLIGHT];
 #pragma unroll
     for (int u = 0; u < CEN_FLIGHT; ++u) {
-      const int tt = t + u * (CEN_THREADS / 16);
+      const int tt = t + u * RPR;
       raw[u] = (tt < t1) ? rbq_ldraw8(base + (long long)tt * st) : rbq_zero_raw(base);
     }
 #pragma unroll
@@ -86,36 +88,37 @@ centroid_partial_kernel(const T* __restrict__ K, long long sb, long long sh, lon
 #pragma unroll
   for (int d = 0; d < 8; ++d) s_acc[r][c8 + d] = acc[d];
   __syncthreads();
-  if (threadIdx.x < RBQ_D) {
+  if (threadIdx.x < D) {
     double a = 0.0;
 #pragma unroll
-    for (int k = 0; k < CEN_THREADS / 16; ++k) a += s_acc[k][threadIdx.x];
-    part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + threadIdx.x] = a;
+    for (int k = 0; k < RPR; ++k) a += s_acc[k][threadIdx.x];
+    part[((size_t)bg * CEN_SPLIT + s) * D + threadIdx.x] = a;
   }
 }
 
 __global__ void centroid_final_kernel(const double* __restrict__ part, const int32_t* __restrict__ seq_lens,
-                                      int Hkv, float* __restrict__ c_k) {
+                                      int Hkv, int D, float* __restrict__ c_k) {      // D threads
   const int bg = blockIdx.x, b = bg / Hkv, d = threadIdx.x;
   const int n = seq_lens[b];
   double acc = 0.0;
-  for (int s = 0; s < CEN_SPLIT; ++s) acc += part[((size_t)bg * CEN_SPLIT + s) * RBQ_D + d];
-  c_k[(size_t)bg * RBQ_D + d] = (n > 0) ? (float)(acc / (double)n) : 0.0f;
+  for (int s = 0; s < CEN_SPLIT; ++s) acc += part[((size_t)bg * CEN_SPLIT + s) * D + d];
+  c_k[(size_t)bg * D + d] = (n > 0) ? (float)(acc / (double)n) : 0.0f;
 }
 
 // ---- Alg.1 tile kernel --------------------------------------------------------------------------
 // grid = (ceil(max_count / ENC_TOK), B*Hkv).  Tokens [t_begin[b], t_begin[b]+count[b]).
-// smem: x tile [ENC_TOK][XS] fp32 (becomes the y tile), P [D][D] fp32 (dense only), n2[ENC_TOK].
-template <typename T, int ROT>
+// smem: x tile [ENC_TOK][XS] fp32 (becomes the y tile), n2[ENC_TOK], P chunk [KC][D] fp32 (dense) or the D signs (WH).
+template <typename T, int ROT, int D>
 __global__ void __launch_bounds__(ENC_THREADS)
 encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
               const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count, int fixed_count,
               int Hkv, int Lcap, const float* __restrict__ rot, const float* __restrict__ c_k,
-              uint32_t* __restrict__ codes, float* __restrict__ f_scale) {
+              uint32_t* __restrict__ codes, void* __restrict__ f_scale, int fs_f16) {
+  constexpr int XS = D + 1, W = D / 32, KC = D < 128 ? D : 128, NG = D / 64;   // NG: float4 output groups per thread
   extern __shared__ __align__(16) float smem[];
   float* xs = smem;                                 // [ENC_TOK][XS]
   float* n2s = xs + ENC_TOK * XS;                   // [ENC_TOK]
-  float* rs = n2s + ENC_TOK;                        // dense: [D][D]; WH: [D] signs
+  float* rs = n2s + ENC_TOK;                        // dense: [KC][D]; WH: [D] signs
 
   const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
   const int tb = t_begin ? t_begin[b] : 0;
@@ -125,25 +128,20 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
   const int ntok = min(ENC_TOK, cnt - tile0);
   const int tid = threadIdx.x;
   const T* base = K + (long long)b * sb + (long long)g * sh + (long long)(tb + tile0) * st;
-  const float* ck = c_k + (size_t)bg * RBQ_D;
+  const float* ck = c_k + (size_t)bg * D;
 
   // x = fl32(k) - c_k
   // 16-byte loads; a warp covers 8 rows x 4 chunks of 8 elements so that its shared-memory stores are conflict-free
   // with the padded row stride (bank = row + 8 * chunk + k)
-  for (int e = tid; e < ENC_TOK * RBQ_D / 8; e += ENC_THREADS) {
+  for (int e = tid; e < ENC_TOK * D / 8; e += ENC_THREADS) {
     const int wv = e >> 5, ln = e & 31;
-    const int r = (wv >> 2) * 8 + (ln >> 2), d = ((wv & 3) * 4 + (ln & 3)) * 8;
+    const int r = (wv / (D / 32)) * 8 + (ln >> 2), d = ((wv % (D / 32)) * 4 + (ln & 3)) * 8;
     float v[8];
     if (r < ntok) rbq_ld8(base + (long long)r * st + d, v);
 #pragma unroll
     for (int k = 0; k < 8; ++k) xs[r * XS + d + k] = (r < ntok) ? __fsub_rn(v[k], ck[d + k]) : 0.0f;
   }
-  if (ROT == RBQ_ROT_DENSE) {
-    for (int e = tid; e < RBQ_D * RBQ_D / 4; e += ENC_THREADS)
-      reinterpret_cast<float4*>(rs)[e] = reinterpret_cast<const float4*>(rot)[e];
-  } else {
-    if (tid < RBQ_D) rs[tid] = rot[tid];
-  }
+  if (ROT == RBQ_ROT_WH && tid < D) rs[tid] = rot[tid];
   __syncthreads();
 
   // n2: one thread per token, sequential fma chain (i ascending)
@@ -151,64 +149,82 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
     float n2 = 0.0f;
     const float* xr = xs + tid * XS;
 #pragma unroll 8
-    for (int i = 0; i < RBQ_D; ++i) n2 = fmaf(xr[i], xr[i], n2);
+    for (int i = 0; i < D; ++i) n2 = fmaf(xr[i], xr[i], n2);
     n2s[tid] = n2;
   }
 
   if (ROT == RBQ_ROT_DENSE) {
-    // thread -> 4 tokens (tt*4..+3) x 8 outputs (tj*4..+3 and 64+tj*4..+3)
+    // thread -> 4 tokens (tt*4..+3) x 4*NG outputs (columns 64 q + tj*4 .. +3, q < NG); P staged KC rows at a time, the
+    // chains run on across the chunks (i ascending: the canonical order)
     const int tj = tid & 15, tt = tid >> 4;
-    float acc[4][8];
+    float acc[4][4 * NG];
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
-      for (int n = 0; n < 8; ++n) acc[m][n] = 0.0f;
+      for (int n = 0; n < 4 * NG; ++n) acc[m][n] = 0.0f;
     const float* x0 = xs + (tt * 4) * XS;
+    for (int ic = 0; ic < D; ic += KC) {
+      if (ic > 0) __syncthreads();                  // everyone done with the previous chunk of P
+      for (int e = tid; e < KC * D / 4; e += ENC_THREADS)
+        reinterpret_cast<float4*>(rs)[e] = reinterpret_cast<const float4*>(rot + (size_t)ic * D)[e];
+      __syncthreads();
 #pragma unroll 4
-    for (int i = 0; i < RBQ_D; ++i) {
-      const float4 r0 = *reinterpret_cast<const float4*>(rs + i * RBQ_D + tj * 4);
-      const float4 r1 = *reinterpret_cast<const float4*>(rs + i * RBQ_D + 64 + tj * 4);
-      const float rr[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+      for (int i = 0; i < KC; ++i) {
+        float rr[4 * NG];
 #pragma unroll
-      for (int m = 0; m < 4; ++m) {
-        const float xv = x0[m * XS + i];
+        for (int q = 0; q < NG; ++q) {
+          const float4 r4 = *reinterpret_cast<const float4*>(rs + i * D + 64 * q + tj * 4);
+          rr[4 * q] = r4.x; rr[4 * q + 1] = r4.y; rr[4 * q + 2] = r4.z; rr[4 * q + 3] = r4.w;
+        }
 #pragma unroll
-        for (int n = 0; n < 8; ++n) acc[m][n] = fmaf(xv, rr[n], acc[m][n]);
+        for (int m = 0; m < 4; ++m) {
+          const float xv = x0[m * XS + ic + i];
+#pragma unroll
+          for (int n = 0; n < 4 * NG; ++n) acc[m][n] = fmaf(xv, rr[n], acc[m][n]);
+        }
       }
     }
     __syncthreads();                                 // everyone done reading x (n2 included)
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
-      for (int n = 0; n < 8; ++n)
-        xs[(tt * 4 + m) * XS + (n < 4 ? tj * 4 + n : 64 + tj * 4 + (n - 4))] = acc[m][n];
+      for (int n = 0; n < 4 * NG; ++n)
+        xs[(tt * 4 + m) * XS + 64 * (n >> 2) + tj * 4 + (n & 3)] = acc[m][n];
   } else {
     __syncthreads();
-    // WH: warp w handles tokens w, w+8, ...; lane holds elements 4*lane..4*lane+3
+    // WH: warp w handles tokens w, w+8, ...; lane holds elements W*lane .. W*lane + W-1: levels h < W inside the lane, the
+    // others by shuffles
     const int warp = tid >> 5, lane = tid & 31;
     for (int r = warp; r < ENC_TOK; r += ENC_THREADS / 32) {
-      float* xr = xs + r * XS + lane * 4;
-      float u0 = __fmul_rn(rs[lane * 4 + 0], xr[0]), u1 = __fmul_rn(rs[lane * 4 + 1], xr[1]);
-      float u2 = __fmul_rn(rs[lane * 4 + 2], xr[2]), u3 = __fmul_rn(rs[lane * 4 + 3], xr[3]);
-      float a, c;
-      a = __fadd_rn(u0, u1); c = __fsub_rn(u0, u1); u0 = a; u1 = c;          // h = 1
-      a = __fadd_rn(u2, u3); c = __fsub_rn(u2, u3); u2 = a; u3 = c;
-      a = __fadd_rn(u0, u2); c = __fsub_rn(u0, u2); u0 = a; u2 = c;          // h = 2
-      a = __fadd_rn(u1, u3); c = __fsub_rn(u1, u3); u1 = a; u3 = c;
+      float* xr = xs + r * XS + lane * W;
+      float u[W];
 #pragma unroll
-      for (int m = 1; m < 32; m <<= 1) {                                      // h = 4*m
+      for (int e = 0; e < W; ++e) u[e] = __fmul_rn(rs[lane * W + e], xr[e]);
+#pragma unroll
+      for (int hh = 1; hh < W; hh <<= 1) {
+#pragma unroll
+        for (int e = 0; e < W; ++e) {
+          if ((e & hh) == 0) {
+            const float a = u[e], c = u[e | hh];
+            u[e] = __fadd_rn(a, c);
+            u[e | hh] = __fsub_rn(a, c);
+          }
+        }
+      }
+#pragma unroll
+      for (int m = 1; m < 32; m <<= 1) {                                      // h = W*m
         // (a, b) -> (a + b, a - b): the upper lane computes p - u, the lower one u + p; both are fmaf(u, +-1, p),
         // bit-identical to the add / subtract (the product with +-1 is exact, one rounding)
         const float sg = (lane & m) ? -1.0f : 1.0f;
-        float p0 = __shfl_xor_sync(0xffffffffu, u0, m), p1 = __shfl_xor_sync(0xffffffffu, u1, m);
-        float p2 = __shfl_xor_sync(0xffffffffu, u2, m), p3 = __shfl_xor_sync(0xffffffffu, u3, m);
-        u0 = fmaf(u0, sg, p0);
-        u1 = fmaf(u1, sg, p1);
-        u2 = fmaf(u2, sg, p2);
-        u3 = fmaf(u3, sg, p3);
+#pragma unroll
+        for (int e = 0; e < W; ++e) {
+          const float pp = __shfl_xor_sync(0xffffffffu, u[e], m);
+          u[e] = fmaf(u[e], sg, pp);
+        }
       }
       __syncwarp();
-      xr[0] = u0; xr[1] = u1; xr[2] = u2; xr[3] = u3;                         // unscaled u
+#pragma unroll
+      for (int e = 0; e < W; ++e) xr[e] = u[e];                              // unscaled u
     }
   }
   __syncthreads();
@@ -217,10 +233,10 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
   if (tid < ntok) {
     const float* yr = xs + tid * XS;
     float l1 = 0.0f;
-    uint32_t w[RBQ_WORDS];
-    const float c = (float)(1.0 / sqrt((double)RBQ_D));
+    uint32_t w[W];
+    const float c = (float)(1.0 / sqrt((double)D));
 #pragma unroll
-    for (int ww = 0; ww < RBQ_WORDS; ++ww) {
+    for (int ww = 0; ww < W; ++ww) {
       uint32_t word = 0;
 #pragma unroll 8
       for (int j = 0; j < 32; ++j) {
@@ -233,8 +249,14 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
     }
     if (ROT == RBQ_ROT_WH) l1 = __fmul_rn(l1, c);
     const size_t tok = (size_t)bg * Lcap + tb + tile0 + tid;
-    reinterpret_cast<uint4*>(codes)[tok] = make_uint4(w[0], w[1], w[2], w[3]);
-    f_scale[tok] = (l1 == 0.0f) ? 0.0f : __fdiv_rn(n2s[tid], l1);
+    if (W == 2) {
+      reinterpret_cast<uint2*>(codes)[tok] = make_uint2(w[0], w[1]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < W / 4; ++q)
+        reinterpret_cast<uint4*>(codes)[tok * (W / 4) + q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
+    }
+    rbq_store_factor(f_scale, fs_f16, tok, (l1 == 0.0f) ? 0.0f : __fdiv_rn(n2s[tid], l1));
   }
 }
 
@@ -244,13 +266,13 @@ encode_kernel(const T* __restrict__ K, long long sb, long long sh, long long st,
 // coalesced 16-byte loads (padded rows: conflict-free per-token reads), c_q of the group's G heads next to them; a
 // thread owns one token and runs the G chains side by side (each staged k_i feeds G independent FMAs).
 constexpr int FB_TOK = 128;
-constexpr int FB_XS = RBQ_D + 1;
 
-template <typename T>
+template <typename T, int D>
 __global__ void __launch_bounds__(FB_TOK)
 fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st, const int32_t* __restrict__ t_begin,
              const int32_t* __restrict__ t_count, int fixed_count, int Hq, int Hkv, int Lcap, const float* __restrict__ c_q,
              float* __restrict__ f_bias) {
+  constexpr int FB_XS = D + 1;
   extern __shared__ __align__(16) float fb_smem[];
   float* ks = fb_smem;                              // [FB_TOK][FB_XS]
   float* cq = ks + FB_TOK * FB_XS;                  // [G][D]
@@ -263,15 +285,15 @@ fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st, 
   const int ntok = min(FB_TOK, cnt - tile0);
   const int tid = threadIdx.x;
   const T* base = K + (long long)b * sb + (long long)g * sh + (long long)(tb + tile0) * st;
-  for (int e = tid; e < FB_TOK * RBQ_D / 8; e += FB_TOK) {
+  for (int e = tid; e < FB_TOK * D / 8; e += FB_TOK) {
     const int wv = e >> 5, ln = e & 31;
-    const int r = (wv >> 2) * 8 + (ln >> 2), d = ((wv & 3) * 4 + (ln & 3)) * 8;
+    const int r = (wv / (D / 32)) * 8 + (ln >> 2), d = ((wv % (D / 32)) * 4 + (ln & 3)) * 8;
     float v[8];
     if (r < ntok) rbq_ld8(base + (long long)r * st + d, v);
 #pragma unroll
     for (int k = 0; k < 8; ++k) ks[r * FB_XS + d + k] = (r < ntok) ? v[k] : 0.0f;
   }
-  for (int e = tid; e < G * RBQ_D; e += FB_TOK) cq[e] = c_q[((size_t)b * Hq + (size_t)g * G) * RBQ_D + e];
+  for (int e = tid; e < G * D; e += FB_TOK) cq[e] = c_q[((size_t)b * Hq + (size_t)g * G) * D + e];
   __syncthreads();
   if (tid >= ntok) return;
   const float* kr = ks + tid * FB_XS;
@@ -279,11 +301,11 @@ fbias_kernel(const T* __restrict__ K, long long sb, long long sh, long long st, 
 #pragma unroll
   for (int h = 0; h < RBQ_MAX_G; ++h) acc[h] = 0.0f;
 #pragma unroll 8
-  for (int i = 0; i < RBQ_D; ++i) {
+  for (int i = 0; i < D; ++i) {
     const float kv = kr[i];
 #pragma unroll
     for (int h = 0; h < RBQ_MAX_G; ++h)
-      if (h < G) acc[h] = fmaf(cq[h * RBQ_D + i], kv, acc[h]);
+      if (h < G) acc[h] = fmaf(cq[h * D + i], kv, acc[h]);
   }
 #pragma unroll
   for (int h = 0; h < RBQ_MAX_G; ++h)
@@ -328,43 +350,62 @@ __global__ void append_bump_kernel(int32_t* n_indexed, int32_t* n_total, int B, 
 
 }  // namespace
 
-int rbq_launch_centroid(rbq_ctx* ctx, const RbqKV& kv, const int32_t* seq_lens, float* c_k, cudaStream_t s) {
+template <typename T, int D>
+static int launch_centroid_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* seq_lens, float* c_k, cudaStream_t s) {
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   double* part = reinterpret_cast<double*>(static_cast<char*>(ctx->ws) + ctx->off_centroid);
-  dim3 grid(BG, CEN_SPLIT);
-  if (ctx->cfg.kv_dtype == RBQ_BF16)
-    centroid_partial_kernel<<<grid, CEN_THREADS, 0, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
-                                                    ctx->cfg.n_kv_heads, part);
-  else
-    centroid_partial_kernel<<<grid, CEN_THREADS, 0, s>>>((const float*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
-                                                    ctx->cfg.n_kv_heads, part);
+  centroid_partial_kernel<T, D><<<dim3(BG, CEN_SPLIT), CEN_THREADS, 0, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, seq_lens,
+                                                                           ctx->cfg.n_kv_heads, part);
   RBQ_LAUNCH_OK(ctx);
-  centroid_final_kernel<<<BG, RBQ_D, 0, s>>>(part, seq_lens, ctx->cfg.n_kv_heads, c_k);
+  centroid_final_kernel<<<BG, D, 0, s>>>(part, seq_lens, ctx->cfg.n_kv_heads, D, c_k);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
-template <typename T, int ROT>
-static int launch_encode_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
+// dispatch on (K/V dtype, head_dim): F<T, D>(args...)
+#define RBQ_DISPATCH_TD(ctx, F, ...)                                                              \
+  do {                                                                                            \
+    const bool bf_ = (ctx)->cfg.kv_dtype == RBQ_BF16;                                             \
+    switch ((ctx)->cfg.head_dim) {                                                                \
+      case 64: return bf_ ? F<__nv_bfloat16, 64>(__VA_ARGS__) : F<float, 64>(__VA_ARGS__);         \
+      case 256: return bf_ ? F<__nv_bfloat16, 256>(__VA_ARGS__) : F<float, 256>(__VA_ARGS__);      \
+      default: return bf_ ? F<__nv_bfloat16, 128>(__VA_ARGS__) : F<float, 128>(__VA_ARGS__);       \
+    }                                                                                             \
+  } while (0)
+
+int rbq_launch_centroid(rbq_ctx* ctx, const RbqKV& kv, const int32_t* seq_lens, float* c_k, cudaStream_t s) {
+  RBQ_DISPATCH_TD(ctx, launch_centroid_t, ctx, kv, seq_lens, c_k, s);
+}
+
+template <typename T, int D, int ROT>
+static int launch_encode_r(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
                            int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
-  const size_t smem = (size_t)(ENC_TOK * XS + ENC_TOK + (ROT == RBQ_ROT_DENSE ? RBQ_D * RBQ_D : RBQ_D)) * sizeof(float);
-  auto kern = encode_kernel<T, ROT>;
-  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_EXACT + (sizeof(T) == 2 ? 0 : 2) + (ROT == RBQ_ROT_DENSE ? 0 : 1), kern, smem);
+  constexpr int KC = D < 128 ? D : 128;
+  const size_t smem = (size_t)(ENC_TOK * (D + 1) + ENC_TOK + (ROT == RBQ_ROT_DENSE ? KC * D : D)) * sizeof(float);
+  auto kern = encode_kernel<T, ROT, D>;
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_ENC_EXACT + (D == 64 ? 0 : D == 128 ? 4 : 8) + (sizeof(T) == 2 ? 0 : 2) + (ROT == RBQ_ROT_DENSE ? 0 : 1), kern, smem);
   dim3 grid((max_count + ENC_TOK - 1) / ENC_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
   kern<<<grid, ENC_THREADS, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count,
                                        ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, ctx->cfg.rot, idx->c_k,
-                                       idx->codes, idx->f_scale);
+                                       idx->codes, idx->f_scale, ctx->cfg.factor_dtype == RBQ_F16 ? 1 : 0);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
+template <typename T, int D>
+static int launch_encode_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
+                           int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
+  if (ctx->cfg.rot_kind == RBQ_ROT_WH) return launch_encode_r<T, D, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  return launch_encode_r<T, D, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+}
+
 // f_bias = <c_q, k> for the same token ranges (either encode mode)
-template <typename T>
+template <typename T, int D>
 static int launch_fbias_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count, int fixed_count,
                           int max_count, const rbq_index* idx, cudaStream_t s) {
-  const size_t smem = (size_t)(FB_TOK * FB_XS + ctx->G * RBQ_D) * sizeof(float);
-  auto kern = fbias_kernel<T>;
-  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_FBIAS + (sizeof(T) == 2 ? 0 : 1), kern, smem);
+  const size_t smem = (size_t)(FB_TOK * (D + 1) + ctx->G * D) * sizeof(float);
+  auto kern = fbias_kernel<T, D>;
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_FBIAS + (D == 64 ? 0 : D == 128 ? 2 : 4) + (sizeof(T) == 2 ? 0 : 1), kern, smem);
   dim3 grid((max_count + FB_TOK - 1) / FB_TOK, ctx->cfg.batch * ctx->cfg.n_kv_heads);
   kern<<<grid, FB_TOK, smem, s>>>((const T*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count, fixed_count, ctx->cfg.n_q_heads,
                                   ctx->cfg.n_kv_heads, ctx->cfg.max_tokens, idx->c_q, idx->f_bias);
@@ -372,19 +413,22 @@ static int launch_fbias_t(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin,
   return RBQ_OK;
 }
 
+static int launch_encode_exact(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count, int fixed_count,
+                               int max_count, const rbq_index* idx, cudaStream_t s) {
+  RBQ_DISPATCH_TD(ctx, launch_encode_t, ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+}
+static int launch_fbias(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count, int fixed_count,
+                        int max_count, const rbq_index* idx, cudaStream_t s) {
+  RBQ_DISPATCH_TD(ctx, launch_fbias_t, ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+}
+
 int rbq_launch_encode(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin, const int32_t* t_count,
                       int fixed_count, int max_count, const rbq_index* idx, cudaStream_t s) {
   if (max_count <= 0) return RBQ_OK;
-  const bool bf = ctx->cfg.kv_dtype == RBQ_BF16, wh = ctx->cfg.rot_kind == RBQ_ROT_WH;
-  int rc;
-  if (ctx->cfg.enc_mode == RBQ_ENC_FAST) rc = rbq_launch_encode_fast(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  else if (bf && !wh) rc = launch_encode_t<__nv_bfloat16, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  else if (bf && wh) rc = launch_encode_t<__nv_bfloat16, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  else if (!bf && !wh) rc = launch_encode_t<float, RBQ_ROT_DENSE>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
-  else rc = launch_encode_t<float, RBQ_ROT_WH>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  const int rc = ctx->cfg.enc_mode == RBQ_ENC_FAST ? rbq_launch_encode_fast(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s)
+                                                   : launch_encode_exact(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
   if (rc != RBQ_OK || !idx->c_q) return rc;
-  return bf ? launch_fbias_t<__nv_bfloat16>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s)
-            : launch_fbias_t<float>(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
+  return launch_fbias(ctx, kv, t_begin, t_count, fixed_count, max_count, idx, s);
 }
 
 int rbq_launch_set_counts(rbq_ctx* ctx, const int32_t* seq_lens, int32_t* n_indexed, int32_t* n_total, cudaStream_t s) {
@@ -396,7 +440,7 @@ int rbq_launch_set_counts(rbq_ctx* ctx, const int32_t* seq_lens, int32_t* n_inde
 int rbq_launch_append_copy(rbq_ctx* ctx, const void* k_new, const void* v_new, int n_new, const RbqKV& kv,
                            int32_t* n_indexed, int32_t* n_total, int commit, cudaStream_t s) {
   const int esz = ctx->cfg.kv_dtype == RBQ_BF16 ? 2 : 4;
-  const int row_vec = RBQ_D * esz / 16;
+  const int row_vec = ctx->cfg.head_dim * esz / 16;
   if (n_new > 0) {
     dim3 grid((n_new * row_vec + 127) / 128, ctx->cfg.batch * ctx->cfg.n_kv_heads);
     append_copy_kernel<<<grid, 128, 0, s>>>((const uint4*)k_new, (const uint4*)v_new, n_new, row_vec,

@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(T5_THREADS, 1)
 encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long sh, long long st,
                   const int32_t* __restrict__ t_begin, const int32_t* __restrict__ t_count, int fixed_count, int Hkv,
                   int Lcap, const float* __restrict__ rot, int wh, const float* __restrict__ c_k, uint32_t* __restrict__ codes,
-                  float* __restrict__ f_scale) {
+                  void* __restrict__ f_scale, int fs_f16) {
   extern __shared__ __align__(128) unsigned char t5_smem[];
   const bool issuer = threadIdx.x >= T5_GROUPS * T5_GTHREADS;  // the last T5_GROUPS warps only issue MMAs
   const int grp = issuer ? ((int)threadIdx.x - T5_GROUPS * T5_GTHREADS) >> 5 : (int)threadIdx.x / T5_GTHREADS;   // pipeline group
@@ -229,7 +229,7 @@ encode_tc5_kernel(const __nv_bfloat16* __restrict__ K, long long sb, long long s
       const size_t tok = (size_t)bg * Lcap + tb + tile0 + r;
       const bool zero = l1t == 0.0f;
       reinterpret_cast<uint4*>(codes)[tok] = zero ? make_uint4(0u, 0u, 0u, 0u) : make_uint4(w0, w1, ex.y, ex.z);
-      f_scale[tok] = zero ? 0.0f : n2buf[r] / l1t;
+      rbq_store_factor(f_scale, fs_f16, tok, zero ? 0.0f : n2buf[r] / l1t);
     }
   };
 
@@ -291,7 +291,7 @@ int rbq_launch_encode_fast(rbq_ctx* ctx, const RbqKV& kv, const int32_t* t_begin
   encode_tc5_kernel<<<dim3(gx, BG), T5_THREADS, T5_SMEM, s>>>((const __nv_bfloat16*)kv.k, kv.sb, kv.sh, kv.st, t_begin, t_count,
                                                              fixed_count, ctx->cfg.n_kv_heads, ctx->cfg.max_tokens,
                                                              ctx->cfg.rot, ctx->cfg.rot_kind == RBQ_ROT_WH ? 1 : 0, idx->c_k,
-                                                             idx->codes, idx->f_scale);
+                                                             idx->codes, idx->f_scale, ctx->cfg.factor_dtype == RBQ_F16 ? 1 : 0);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }

@@ -97,9 +97,10 @@ template <int W> struct GroupLoad {   // what lane (g, t) needs of one 32-token 
 };
 
 // grid = k * SMs CTAs of EST_WARPS warps.  Flat group index -> (sequence b, KV head, 32-token group).
-template <int W, bool INT_OUT, bool HAS_BIAS>
+// F16: the factors are stored as binary16 (rbq_config.factor_dtype; 2 + D/8 bytes per unit instead of 4 + D/8)
+template <int W, bool INT_OUT, bool HAS_BIAS, bool F16>
 __global__ void __launch_bounds__(EST_THREADS, W == 8 ? 2 : 3)
-estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_scale,
+estimate_kernel(const uint32_t* __restrict__ codes, const void* __restrict__ f_scale,
                 const float* __restrict__ f_bias, const int32_t* __restrict__ n_indexed,
                 const RbqQConst* __restrict__ qconst, int B, int Hq, int Hkv, int Lcap, float sm_scale,
                 float* __restrict__ scores, int32_t* __restrict__ dot_out, int32_t* __restrict__ pop_out,
@@ -142,7 +143,8 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
     // lane (g, t): word t of tokens 4g..4g+3 of a group and their factors.  A token run beyond the allocation
     // (Lcap % 32 != 0) is clamped to its last 4 tokens (never stored); groups beyond the segment are not loaded.
     const uint32_t* cbase = codes + prow * W;
-    const float* fbase = f_scale + prow;
+    const float* fbase = reinterpret_cast<const float*>(f_scale) + prow;          // F16: see load_at
+    const __half* hbase = reinterpret_cast<const __half*>(f_scale) + prow;
     const int tok_clamp = Lcap - 4;
     auto load_at = [&](int gi) -> GroupLoad<W> {
       const int tk = min(gi * 32 + 4 * g, tok_clamp);
@@ -150,7 +152,13 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
       GroupLoad<W> r;
 #pragma unroll
       for (int k = 0; k < 4; ++k) r.w[k] = load_tok<W>(p + k * W, t);
-      r.fs = __ldg(reinterpret_cast<const float4*>(fbase + tk));
+      if (F16) {
+        const uint2 hv = __ldg(reinterpret_cast<const uint2*>(hbase + tk));
+        const float2 f01 = __half22float2(*reinterpret_cast<const __half2*>(&hv.x)), f23 = __half22float2(*reinterpret_cast<const __half2*>(&hv.y));
+        r.fs = make_float4(f01.x, f01.y, f23.x, f23.y);
+      } else {
+        r.fs = __ldg(reinterpret_cast<const float4*>(fbase + tk));
+      }
       return r;
     };
     // three groups of loads in flight per warp; codes and factors do not depend on S3, its constants do
@@ -230,8 +238,8 @@ estimate_kernel(const uint32_t* __restrict__ codes, const float* __restrict__ f_
   }
 }
 
-template <int W, bool INT_OUT, bool HAS_BIAS>
-int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t s) {
+template <int W, bool INT_OUT, bool HAS_BIAS, bool F16>
+int launch_f(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t s) {
   if (ctx->cfg.batch > EST_MAX_B) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch %d > %d", ctx->cfg.batch, EST_MAX_B);
   // upper bound of the work: every sequence full; 3 CTAs (24 warps) per SM, fewer when there is little work
   const long long max_groups = (long long)ctx->cfg.batch * ctx->cfg.n_kv_heads * ((ctx->cfg.max_tokens + 31) / 32);
@@ -240,12 +248,18 @@ int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, in
   if (ctas > cap) ctas = cap;
   if (ctas < 1) ctas = 1;
   const RbqQConst* qc = reinterpret_cast<const RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
-  RBQ_CUDA_OK(ctx, rbq_launch_pdl(estimate_kernel<W, INT_OUT, HAS_BIAS>, dim3((unsigned)ctas), dim3(EST_THREADS), 0, s,
-                                  (const uint32_t*)idx->codes, (const float*)idx->f_scale, (const float*)idx->f_bias,
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(estimate_kernel<W, INT_OUT, HAS_BIAS, F16>, dim3((unsigned)ctas), dim3(EST_THREADS), 0, s,
+                                  (const uint32_t*)idx->codes, (const void*)idx->f_scale, (const float*)idx->f_bias,
                                   (const int32_t*)idx->n_indexed, qc, ctx->cfg.batch, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads,
                                   ctx->cfg.max_tokens, ctx->sm_scale, scores, dot, pop, rowmax_key));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
+}
+
+template <int W, bool INT_OUT, bool HAS_BIAS>
+int launch_t(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t s) {
+  if (ctx->cfg.factor_dtype == RBQ_F16) return launch_f<W, INT_OUT, HAS_BIAS, true>(ctx, idx, scores, dot, pop, rowmax_key, s);
+  return launch_f<W, INT_OUT, HAS_BIAS, false>(ctx, idx, scores, dot, pop, rowmax_key, s);
 }
 
 template <int W>

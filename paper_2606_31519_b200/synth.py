@@ -95,10 +95,9 @@ def config_seq_lens(cfg: int, B: int | None = None, L: int | None = None) -> np.
     return np.full(B, l0, np.int32)
 
 
-def _draw_group(cfg, b, g, L, G, n_heavy, knob, variant, dtype):
+def _draw_group(cfg, b, g, L, G, n_heavy, knob, variant, dtype, D=D_HEAD):
     """One (sequence, KV head): keys, values and the G queries that read them."""
-    D = D_HEAD
-    rng = np.random.default_rng([SEED, cfg, b, g])
+    rng = np.random.default_rng([SEED, cfg, b, g] if D == D_HEAD else [SEED, cfg, b, g, D])
     K = rng.standard_normal((L, D), dtype=np.float32)
     K[:, 0:4] *= 10.0
     V = rng.standard_normal((L, D), dtype=np.float32)
@@ -149,18 +148,19 @@ def _draw_group(cfg, b, g, L, G, n_heavy, knob, variant, dtype):
 
 def make_workload(cfg: int, *, L: int | None = None, B: int | None = None, variant: str = "C",
                   with_cq: bool = False, p: float | None = None, extra_cap: int = 0,
-                  n_heavy: int | None = None) -> Workload:
+                  n_heavy: int | None = None, D: int = D_HEAD, Hq: int | None = None, Hkv: int | None = None) -> Workload:
     """Build configuration `cfg` of BASELINE.json (optionally scaled down via L / B).
 
     variant "C" = calibrated (temperature beta, sink gain gamma), "L" = literal wording
     (beta = 1, sink keys = 2 x query; degenerate, parity-only).  `extra_cap` adds room at
     the tail of every sequence for appended tokens.
     """
-    b0, Hq, Hkv, _, dtype, nh0, knob, p0, W = _CFG[cfg]
+    b0, Hq0, Hkv0, _, dtype, nh0, knob, p0, W = _CFG[cfg]
+    Hq, Hkv = Hq0 if Hq is None else Hq, Hkv0 if Hkv is None else Hkv     # head counts / head_dim other than the config's: SURVEY 8(f1)
     n_heavy = nh0 if n_heavy is None else n_heavy
     seq_lens = config_seq_lens(cfg, B, L)
     B = len(seq_lens)
-    D, G = D_HEAD, Hq // Hkv
+    G = Hq // Hkv
     Lcap = int(seq_lens.max()) + int(extra_cap)
     Lcap = (Lcap + 63) // 64 * 64
     K = np.zeros((B, Hkv, Lcap, D), np.float32)
@@ -170,7 +170,7 @@ def make_workload(cfg: int, *, L: int | None = None, B: int | None = None, varia
     for b in range(B):
         Lb = int(seq_lens[b])
         for g in range(Hkv):
-            k_, v_, q_, s_ = _draw_group(cfg, b, g, Lb, G, n_heavy, knob, variant, dtype)
+            k_, v_, q_, s_ = _draw_group(cfg, b, g, Lb, G, n_heavy, knob, variant, dtype, D)
             K[b, g, :Lb], V[b, g, :Lb] = k_, v_
             q[b, g * G:(g + 1) * G] = q_
             sigma[b, g * G:(g + 1) * G] = s_
@@ -182,12 +182,12 @@ def make_workload(cfg: int, *, L: int | None = None, B: int | None = None, varia
                     rot_gauss=rotation_gaussian(D), wh_signs=wh_sign_vector(D), sigma=sigma)
 
 
-def append_rows(cfg: int, step: int, B: int, Hkv: int, n_new: int, dtype: str = "bf16"):
+def append_rows(cfg: int, step: int, B: int, Hkv: int, n_new: int, dtype: str = "bf16", D: int = D_HEAD):
     """Plain K, V rows for tokens appended at decode step `step` (drawn as recipe step 1)."""
     rng = np.random.default_rng([SEED, cfg, 1000 + step])
-    K = rng.standard_normal((B, Hkv, n_new, D_HEAD), dtype=np.float32)
+    K = rng.standard_normal((B, Hkv, n_new, D), dtype=np.float32)
     K[..., 0:4] *= 10.0
-    V = rng.standard_normal((B, Hkv, n_new, D_HEAD), dtype=np.float32)
+    V = rng.standard_normal((B, Hkv, n_new, D), dtype=np.float32)
     V[..., 0:4] *= 10.0
     if dtype == "bf16":
         K, V = bf16_round(K), bf16_round(V)

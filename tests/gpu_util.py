@@ -18,6 +18,10 @@ D = 128
 SM_SCALE = 1.0 / math.sqrt(D)
 
 
+def sm_scale(w):
+    return 1.0 / math.sqrt(w.D)
+
+
 def torch_dtype(w):
     import torch
     return torch.float32 if w.kv_dtype == "f32" else torch.bfloat16
@@ -31,14 +35,14 @@ def to_dev(a, dtype=None):
     return t.cuda()
 
 
-def make_cache(w, rot, *, rot_kind=0, with_cq=False, flush_tokens=0, out_dtype=None, upload_kv=True):
+def make_cache(w, rot, *, rot_kind=0, with_cq=False, flush_tokens=0, out_dtype=None, upload_kv=True, **kw):
     """RaBitQCache for workload `w` with K/V (and c_q) uploaded; nothing encoded yet."""
     import torch
     from paper_2606_31519_b200 import binding as rb
     dt = torch_dtype(w)
     c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(np.ascontiguousarray(rot, dtype=np.float32)),
                        flush_tokens=flush_tokens, kv_dtype=dt, q_dtype=dt, out_dtype=out_dtype or torch.float32,
-                       rot_kind=rot_kind, with_cq=with_cq)
+                       rot_kind=rot_kind, with_cq=with_cq, head_dim=w.D, **kw)
     if upload_kv:
         c.K.copy_(to_dev(w.K, dt))
         c.V.copy_(to_dev(w.V, dt))
@@ -58,32 +62,43 @@ def load_index(c, o):
     c.n_total.copy_(to_dev(o["n_total"]))
 
 
-def oracle_index(orc, w, rot, rot_kind=0, with_cq=False):
-    """O2: centroid + Alg.1 over tokens [0, seq_lens) with the oracle."""
+def oracle_index(orc, w, rot, rot_kind=0, with_cq=False, factor_f16=False):
+    """O2: centroid + Alg.1 over tokens [0, seq_lens) with the oracle (factor_f16: O2c, factors rounded to binary16)."""
     c_k = orc.centroid(w.K, w.seq_lens)
     codes, f_scale, f_bias = orc.encode(w.K, np.zeros_like(w.seq_lens), w.seq_lens, rot_kind, rot, c_k,
                                         w.c_q if with_cq else None)
+    if factor_f16:
+        f_scale = orc.round_factors_f16(f_scale)
     return dict(c_k=c_k, codes=codes, f_scale=f_scale, f_bias=f_bias, n_indexed=w.seq_lens.copy(),
                 n_total=w.seq_lens.copy())
 
 
-def oracle_full(orc, w, rot, rot_kind=0, with_cq=False, p=None):
-    o = oracle_index(orc, w, rot, rot_kind, with_cq)
+def oracle_full(orc, w, rot, rot_kind=0, with_cq=False, p=None, factor_f16=False):
+    o = oracle_index(orc, w, rot, rot_kind, with_cq, factor_f16)
     scores, qp, dot, pop = orc.estimate_scores(w.q, o["codes"], o["f_scale"], o["f_bias"], o["c_k"],
-                                               w.c_q if with_cq else None, o["n_indexed"], rot_kind, rot, SM_SCALE)
+                                               w.c_q if with_cq else None, o["n_indexed"], rot_kind, rot, sm_scale(w))
     o.update(scores=scores, qp=qp, dot=dot, pop=pop)
     p = w.p if p is None else p
     n_rows = np.repeat(o["n_indexed"], w.Hq)
     sel_idx, sel_cnt = orc.topp(scores.reshape(w.B * w.Hq, w.Lcap), n_rows, p)
     o.update(sel_idx=sel_idx.reshape(w.B, w.Hq, w.Lcap), sel_cnt=sel_cnt.reshape(w.B, w.Hq), p=p)
-    out, lse = orc.attention(w.q, w.K, w.V, o["sel_idx"], o["sel_cnt"], o["n_indexed"], o["n_total"], SM_SCALE)
+    out, lse = orc.attention(w.q, w.K, w.V, o["sel_idx"], o["sel_cnt"], o["n_indexed"], o["n_total"], sm_scale(w))
     o.update(out=out, lse=lse)
     return o
 
 
 @functools.lru_cache(maxsize=None)
-def workload(cfg, L=None, B=None, variant="C", with_cq=False, extra_cap=0, n_heavy=None):
-    return synth.make_workload(cfg, L=L, B=B, variant=variant, with_cq=with_cq, extra_cap=extra_cap, n_heavy=n_heavy)
+def workload(cfg, L=None, B=None, variant="C", with_cq=False, extra_cap=0, n_heavy=None, D=128, Hq=None, Hkv=None):
+    return synth.make_workload(cfg, L=L, B=B, variant=variant, with_cq=with_cq, extra_cap=extra_cap, n_heavy=n_heavy, D=D,
+                               Hq=Hq, Hkv=Hkv)
+
+
+@functools.lru_cache(maxsize=None)
+def rotation(orc_mod, D, kind=0):
+    """Rotation input of the recipe for head_dim D: dense QR matrix (kind 0, by the oracle) or WH sign vector (kind 1)."""
+    if kind == 1:
+        return synth.wh_sign_vector(D)
+    return orc_mod.rotation_from_gaussian(synth.rotation_gaussian(D))[0]
 
 
 # ---- comparison rules -------------------------------------------------------------------------------

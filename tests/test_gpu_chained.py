@@ -16,10 +16,10 @@ pytestmark = pytest.mark.gpu
 ROT_DENSE, ROT_WH = 0, 1
 
 
-def _chained(orc, w, rot, kind, p, with_cq=False):
+def _chained(orc, w, rot, kind, p, with_cq=False, factor_f16=False):
     import torch
-    o = U.oracle_full(orc, w, rot, kind, with_cq, p=p)
-    c = U.make_cache(w, rot, rot_kind=kind, with_cq=with_cq)
+    o = U.oracle_full(orc, w, rot, kind, with_cq, p=p, factor_f16=factor_f16)
+    c = U.make_cache(w, rot, rot_kind=kind, with_cq=with_cq, **(dict(factor_dtype=torch.float16) if factor_f16 else {}))
     c.encode_keys(U.to_dev(w.seq_lens))
     q = U.to_dev(w.q, U.torch_dtype(w))
     # staged calls
@@ -67,6 +67,29 @@ def test_decode_step_chained(orc, rot128, cfg, kw, p, kind):
     from paper_2606_31519_b200 import synth
     rot = rot128[0] if kind == ROT_DENSE else synth.wh_sign_vector(128)
     _chained(orc, U.workload(cfg, **kw), rot, kind, p)
+
+
+@pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
+@pytest.mark.parametrize("cfg,kw,D", [(1, dict(L=5003), 128), (3, dict(L=3001, B=3), 128), (1, dict(L=3001), 64), (2, dict(L=4100, n_heavy=32), 256)])
+def test_decode_step_chained_f16_factors(orc, cfg, kw, D, kind):
+    """2-byte correction factors: rbq_config.factor_dtype = RBQ_F16.  The stored
+    factors are the oracle's fp32 factors rounded to binary16 bit for bit; logits, Top-p sets and outputs then match the
+    oracle run on those rounded factors at the usual tolerances (the rounding itself moves a logit by <= 2^-11 of its
+    estimated part: tests/test_oracle_rotation_encode.py::test_factors_f16_rounding_and_logit_bound)."""
+    import torch
+    w = U.workload(cfg, D=D, **kw)
+    rot = U.rotation(orc, D, kind)
+    o = _chained(orc, w, rot, kind, 0.9, factor_f16=True)
+    c = U.make_cache(w, rot, rot_kind=kind, factor_dtype=torch.float16)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    torch.cuda.synchronize()
+    fs = c.f_scale.cpu().numpy()
+    assert fs.dtype == np.float16
+    for b in range(w.B):
+        n = int(w.seq_lens[b])
+        assert (fs[b, :, :n].view(np.uint16) == o["f_scale"][b, :, :n].astype(np.float16).view(np.uint16)).all(), "fp16 factors differ"
+        assert (c.codes.cpu().numpy().view(np.uint32)[b, :, :n] == o["codes"][b, :, :n]).all()
+    c.close()
 
 
 def test_decode_step_chained_with_cq(orc, rot128):
@@ -345,7 +368,9 @@ def test_error_codes(rot128):
         h = C.c_void_p()
         return lib.rbq_create(C.byref(cfg), C.byref(h)), h
 
-    assert create(head_dim=64)[0] == -2 and create(head_dim=256)[0] == -2          # RBQ_ERR_UNSUPPORTED
+    assert create(head_dim=96)[0] == -2 and create(head_dim=512)[0] == -2          # RBQ_ERR_UNSUPPORTED (64 / 128 / 256 are built)
+    assert create(head_dim=64, enc_mode=1)[0] == -2 and create(head_dim=256, enc_mode=1)[0] == -2   # RBQ_ENC_FAST: head_dim 128 only
+    assert create(n_q_heads=8, n_kv_heads=1)[0] == -2                               # G = 8
     assert create(head_dim=100)[0] == -1 and create(n_q_heads=3, n_kv_heads=2)[0] == -1
     assert create(max_tokens=0)[0] == -1 and create(rot=None)[0] == -1
     rc, h = create()
