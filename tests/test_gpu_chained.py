@@ -278,6 +278,64 @@ def test_append_beyond_capacity_is_dropped_and_flagged(orc, rot128):
     c.close()
 
 
+@pytest.mark.parametrize("fast", [False, True])
+def test_pipelined_prefill_side_stream(orc, rot128, fast):
+    """Asynchronous pipelined prefill ("a secondary, low-priority CUDA stream ... the quantization process
+    proceeds in parallel with the heavy attention computation", L341 "<10 % TTFT overhead"): rbq_encode_keys
+    (centroid + Alg.1) runs on a low-priority stream while a dense causal attention of the same layer (torch SDPA, a
+    library call standing in for the model) occupies the main stream; the two are joined by an event before the first
+    decode step.  The index built under that contention must be the oracle's (bit for bit in RBQ_ENC_EXACT, inside the
+    guard band in RBQ_ENC_FAST), and the decode step that follows must see it."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb
+    w = U.workload(1, L=16384)
+    rot = rot128[0]
+    o = U.oracle_full(orc, w, rot)
+    c = rb.RaBitQCache(w.B, w.Hq, w.Hkv, w.Lcap, torch.from_numpy(rot), enc_mode=rb.RBQ_ENC_FAST if fast else rb.RBQ_ENC_EXACT)
+    c.K.copy_(U.to_dev(w.K, torch.bfloat16))
+    c.V.copy_(U.to_dev(w.V, torch.bfloat16))
+    seq = U.to_dev(w.seq_lens)
+    n = int(w.seq_lens[0])
+    G = w.Hq // w.Hkv
+    qs = torch.randn(1, w.Hq, n, 128, device="cuda", dtype=torch.bfloat16)          # the prefill's own queries
+    kk = c.K[:, :, :n].repeat_interleave(G, dim=1).contiguous()
+    vv = c.V[:, :, :n].repeat_interleave(G, dim=1).contiguous()
+    lo, hi = torch.cuda.Stream.priority_range()
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream(priority=lo)
+    torch.cuda.synchronize()
+    side.wait_stream(main)
+    for _ in range(2):                                                               # attention in flight on the main stream ...
+        att = torch.nn.functional.scaled_dot_product_attention(qs, kk, vv, is_causal=True)
+    c.encode_keys(seq, stream=side)                                                  # ... index build beside it
+    done = torch.cuda.Event()
+    done.record(side)
+    main.wait_event(done)                                                            # "until the first decoding step of that layer"
+    out = c.new_out()
+    sel_cnt = c.new_sel()[1]
+    c.decode_step(U.to_dev(w.q, torch.bfloat16), w.p, out, None, sel_cnt)
+    torch.cuda.synchronize()
+    assert torch.isfinite(att).all()
+    codes = c.codes.cpu().numpy().view(np.uint32)
+    fs = c.f_scale.cpu().numpy()
+    if not fast:
+        assert (codes[0, :, :n] == o["codes"][0, :, :n]).all() and (fs[0, :, :n].view(np.uint32) == o["f_scale"][0, :, :n].view(np.uint32)).all()
+        U.assert_attention_close(out.cpu().numpy(), o["out"], "bf16")
+        assert np.abs(sel_cnt.cpu().numpy().astype(np.int64) - o["sel_cnt"]).max() <= max(2, int(0.002 * o["sel_cnt"].max()))
+    else:
+        P = rot.astype(np.float64)
+        for g in range(w.Hkv):
+            x = w.K[0, g, :n].astype(np.float64) - o["c_k"][0, g].astype(np.float64)
+            y = x @ P
+            xn = np.linalg.norm(x, axis=1, keepdims=True)
+            diff = codes[0, g, :n] ^ o["codes"][0, g, :n]
+            bits = ((diff[:, :, None] >> np.arange(32, dtype=np.uint32)) & 1).reshape(n, 128).astype(bool)
+            assert (np.abs(y)[bits] <= 1e-5 * np.broadcast_to(xn, y.shape)[bits]).all()
+            ref = o["f_scale"][0, g, :n].astype(np.float64)
+            assert (np.abs(fs[0, g, :n] - ref) <= 1e-5 * np.abs(ref)).all()
+        U.assert_attention_close(out.cpu().numpy(), o["out"], "bf16")
+    c.close()
+
+
 def test_append_many_tokens_per_call(orc, rot128):
     """n_new = 5 per call with W = 8 (flush of whole windows only), and n_new >= W in one call."""
     import torch
