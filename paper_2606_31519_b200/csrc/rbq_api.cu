@@ -292,7 +292,7 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
   RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
-  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4], ev[5] between its kernels
+  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4] after the plan
   ctx->stage_ev = nullptr;
   if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[RBQ_N_STAGES], s));
   return rc;

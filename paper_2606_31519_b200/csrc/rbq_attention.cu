@@ -772,8 +772,8 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
     case 2: RBQ_PLAN_LAUNCH(2); break;
     default: RBQ_PLAN_LAUNCH(1); break;
   }
-#undef RBQ_PLAN_LAUNCH
   RBQ_LAUNCH_OK(ctx);
+#undef RBQ_PLAN_LAUNCH
   if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));
   const bool kbf = ctx->cfg.kv_dtype == RBQ_BF16, qbf = ctx->cfg.q_dtype == RBQ_BF16;
   if (rbq_attention_uses_mma(ctx)) {

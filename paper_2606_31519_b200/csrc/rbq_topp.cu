@@ -13,14 +13,17 @@
 //             2^-22 fixed point, so the bin mass is exp(-j/64) * sum(r): integer sums => order-independent, deterministic.
 //             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin travel
 //             through distributed shared memory (DSMEM is ~20 B/clk per SM).
-//   pass 2  : the tokens of the crossing bin (a few hundred at 128 K context) are gathered from all CTAs in one
-//             DSMEM round; every CTA ranks its share of them against all of them with integer prefix masses
-//             (8 threads per candidate) and the one thread that finds the cut C* writes it into every CTA of the
-//             cluster.  If the crossing bin holds more than TP_CAND tokens (heavy ties), it is first narrowed by
-//             cluster-wide 11-bit radix levels on C.
-//   pass 3  : token t is selected  <=>  C(t) >= C*.  Written as a per-row BITMAP (the representation
-//             the gather attention consumes), the count, and -- only when the caller asks for it --
-//             the ascending index list.
+//   pass 2  : ONE more pass over the resident slice classifies every token: bins above the crossing bin are selected (their
+//             bitmap words are assembled right away), the tokens of the crossing bin (a few hundred at 128 K context) become
+//             candidates; these are gathered from all CTAs in one DSMEM round; every CTA ranks its share of them against all
+//             of them with integer prefix masses (8 threads per candidate) and the one thread that finds the cut C*
+//             writes it into every CTA of the cluster.  If the crossing bin holds more than TP_CAND tokens (heavy ties),
+//             it is first narrowed by cluster-wide 11-bit radix levels on C.
+//   (A variant in which the last of a KV group's row clusters also built the group's union list for S7 in its tail was
+//   measured and dropped: on 8 x 4 CTAs the expansion took 32 K cycles, the stand-alone plan kernel on 128 CTAs 8 us.)
+//   pass 3  : only the CANDIDATES are revisited: candidate t is selected  <=>  C(t) >= C*; its bit is OR-ed into the words.
+//             Output: a per-row BITMAP (the representation the gather attention consumes), the count, and -- only when
+//             the caller asks for it -- the ascending index list.
 #include <cooperative_groups.h>
 
 #include "rbq_common.cuh"
@@ -28,6 +31,19 @@
 RBQ_PROBE_DECL(topp_probe);
 
 namespace cg = cooperative_groups;
+
+#ifdef RBQ_PROBE
+#define TP_STAMP(slot)                                                                                          \
+  do {                                                                                                          \
+    const unsigned cta_ = blockIdx.y * gridDim.x + blockIdx.x;                                                   \
+    if (threadIdx.x == 0 && cta_ < RBQ_PROBE_CTAS) {                                                             \
+      topp_probe[cta_ * RBQ_PROBE_SLOTS + (slot)] = (unsigned long long)clock64();                               \
+      if ((slot) == 0) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); topp_probe[cta_ * RBQ_PROBE_SLOTS + 15] = gt_; } \
+    }                                                                                                           \
+  } while (0)
+#else
+#define TP_STAMP(slot) do {} while (0)
+#endif
 
 namespace {
 
@@ -60,7 +76,8 @@ struct TpSmall {
 constexpr size_t TP_OFF_HIST = (sizeof(TpSmall) + 127) & ~size_t(127);
 constexpr size_t TP_OFF_A = TP_OFF_HIST + TP_NB * sizeof(uint2);                 // 24 KB: cand_all | cand_loc
 constexpr size_t TP_A_HALF = TP_CAND * 12;                                       // comp u64 + rfix u32
-constexpr size_t TP_OFF_SC = TP_OFF_A + 2 * TP_A_HALF;
+constexpr size_t TP_OFF_SELW = TP_OFF_A + 2 * TP_A_HALF;                          // 8 KB: selection words of the slice (<= 2048)
+constexpr size_t TP_OFF_SC = TP_OFF_SELW + 2048 * sizeof(uint32_t);
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -181,12 +198,13 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
   rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
+  TP_STAMP(0);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
   uint32_t* hist = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);
   uint32_t hist_sa = (uint32_t)__cvta_generic_to_shared(hist);   // 32-bit shared address for the histogram atomics,
   asm volatile("mov.u32 %0, %0;" : "+r"(hist_sa));               // opaque: kept in a register, not rebuilt from SR_CgaCtaId per atomic
-  uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_HIST);          // aliases hist once the cut is known
+  uint32_t* selw = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_SELW);          // own area: written while peers may still read hist
   u64* all_comp = reinterpret_cast<u64*>(smem_raw + TP_OFF_A);
   uint32_t* all_rfix = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A + TP_CAND * 8);
   uint32_t* woff = reinterpret_cast<uint32_t*>(smem_raw + TP_OFF_A);             // aliases cand_all after the cut is known
@@ -229,6 +247,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   rbq_pdl_wait();                                             // scores and row maxima of S5
+  TP_STAMP(1);
   const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
   __syncthreads();
   {
@@ -304,7 +323,9 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     for (int o = 1; o < 8; o <<= 1) { ms += __shfl_xor_sync(FULL, ms, o); cs += __shfl_xor_sync(FULL, cs, o); }
     if ((tid & 7) == 0) { sh.xc_mass[tid >> 3] = ms * sh.tabA[tid >> 3]; sh.xc_cnt[tid >> 3] = cs; }
   }
+  TP_STAMP(2);
   csync();                                                    // S1: histograms and coarse summaries complete
+  TP_STAMP(3);
   if (rank == 0 && tid == 0) rowmax_key[row] = 0u;            // every CTA of the row has read its maximum: clear the key for the next step
   if (warp == 0) {
     // coarse crossing: lane l owns coarse bins 2l, 2l+1 (totals over the cluster in rank order), warp scan in fp64;
@@ -378,6 +399,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     }
   }
   __syncthreads();
+  TP_STAMP(4);
   const int bx = (int)sh.bx;
   uint32_t cntx = sh.cntx;
   const float u_lo = (float)bx * 0.015625f, u_hi = (bx == TP_NB - 1) ? INFINITY : (float)(bx + 1) * 0.015625f;
@@ -443,31 +465,47 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     }
   }
 
-  // ---- pass 2: candidates of this CTA -> local list; gather all ---------------------------------------------
+  // ---- pass 2: every token classified once: above the crossing bin -> its bit (8 lanes assemble one 32-token word);
+  //      in the crossing bin (and, after a radix narrowing, inside the candidate range) -> local candidate list ----------
   {
     u64 lo64 = 0, hi64 = 0;
     if (use_range) { lo64 = sh.lo64; hi64 = sh.hi64; }
-    const int n4 = (len + 3) >> 2;
-    for (int i4 = tid; i4 < n4; i4 += TP_THREADS) {
-      const float4 v4 = reinterpret_cast<const float4*>(sc)[i4];
+    const int n4r = nwords * 8;                               // float4 groups, rounded up to whole words
+#pragma unroll 2
+    for (int base = warp * 32; base < n4r; base += TP_THREADS) {
+      const int i4 = base + lane;
+      const float4 v4 = (i4 < n4r) ? reinterpret_cast<const float4*>(sc)[i4] : make_float4(0.f, 0.f, 0.f, 0.f);
       const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+      uint32_t nib = 0;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
+        const int i = 4 * i4 + k;
         const float u = __fsub_rn(m, v[k]);
-        if (u >= u_lo && u < u_hi && 4 * i4 + k < len) {
-          const u64 c = composite(v[k], lo + 4 * i4 + k);
+        bool sel = (i < len) && (u < u_lo);
+        if (i < len && u >= u_lo && u < u_hi) {
+          const u64 c = composite(v[k], lo + i);
           if (!use_range || (c >= lo64 && c <= hi64)) {
             int j_unused;
             uint32_t rfix;
             bin0(m, v[k], j_unused, rfix);
             const uint32_t slot = atomicAdd(&sh.lcount, 1u);
             if (slot < TP_CAND) { loc_comp[slot] = c; loc_rfix[slot] = rfix; }
+          } else if (c > hi64) {
+            sel = true;                                       // narrowed range: above it = selected for sure
           }
         }
+        nib |= sel ? (1u << k) : 0u;
       }
+      uint32_t word = nib << (4 * (lane & 7));
+      word |= __shfl_xor_sync(FULL, word, 1);
+      word |= __shfl_xor_sync(FULL, word, 2);
+      word |= __shfl_xor_sync(FULL, word, 4);
+      if ((lane & 7) == 0 && i4 < n4r) selw[i4 >> 3] = word;
     }
   }
+  TP_STAMP(5);
   csync();                                                    // S2: candidate lists complete; histograms free
+  TP_STAMP(6);
   int ncand = 0;
   {
     int off[CS + 1];                                          // all peer counts first, then one round of independent remote loads
@@ -519,7 +557,9 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
       }
     }
   }
+  TP_STAMP(7);
   csync();                                                    // S3: the cut is visible in every CTA
+  TP_STAMP(8);
   if (!sh.found) {                                            // zero-weight candidates / rounding at the last ulp: take all of them
     if (tid == 0) {
       u64 mn = ~0ull;
@@ -531,30 +571,19 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   const u64 cstar = sh.cstar;
   const uint32_t total_sel = sh.ksel;
 
-  // ---- pass 3: bitmap words (always), ascending index list (on request).  A lane classifies 4 consecutive tokens,
-  //      8 lanes assemble one 32-token word ---------------------------------------------------------------------
+  // ---- pass 3: the candidates at or above the cut join the selection; bitmap words out (always), ascending index list
+  //      (on request) ------------------------------------------------------------------------------------------------
   {
-    const float sstar = rbq_fkey_inv((uint32_t)(cstar >> 32));
-    const int tstar = (int)(~(uint32_t)cstar);                // equal scores: indices <= tstar are selected
-    const int n4r = nwords * 8;                               // float4 groups, rounded up to whole words
-#pragma unroll 2
-    for (int base = warp * 32; base < n4r; base += TP_THREADS) {
-      const int i4 = base + lane;
-      const float4 v4 = (i4 < n4r) ? reinterpret_cast<const float4*>(sc)[i4] : make_float4(0.f, 0.f, 0.f, 0.f);
-      const float v[4] = {v4.x, v4.y, v4.z, v4.w};
-      uint32_t nib = 0;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int i = 4 * i4 + k;
-        const bool sel = (i < len) && ((v[k] > sstar) || (v[k] == sstar && lo + i <= tstar));
-        nib |= sel ? (1u << k) : 0u;
+    const int nloc = min((int)sh.lcount, TP_CAND);
+    for (int k = tid; k < nloc; k += TP_THREADS) {
+      const u64 c = loc_comp[k];
+      if (c >= cstar) {
+        const int i = (int)(~(uint32_t)c) - lo;               // slice-local token index
+        atomicOr(&selw[i >> 5], 1u << (i & 31));
       }
-      uint32_t word = nib << (4 * (lane & 7));
-      word |= __shfl_xor_sync(FULL, word, 1);
-      word |= __shfl_xor_sync(FULL, word, 2);
-      word |= __shfl_xor_sync(FULL, word, 4);
-      if ((lane & 7) == 0 && i4 < n4r) { const int w = i4 >> 3; bits_row[(lo >> 5) + w] = word; selw[w] = word; }
     }
+    __syncthreads();
+    for (int w = tid; w < nwords; w += TP_THREADS) bits_row[(lo >> 5) + w] = selw[w];
   }
   if (rank == 0 && tid == 0) sel_cnt[row] = (int32_t)total_sel;
   if (sel_idx) {
@@ -595,7 +624,10 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
       if ((bal >> lane) & 1u) sel_idx[rbase + obase + woff[w] + __popc(bal & lt)] = lo + w * 32 + lane;
     }
   }
+  TP_STAMP(9);
+  TP_STAMP(13);
   csync();                                                    // keep shared memory alive until every peer has read it
+  TP_STAMP(14);
 }
 
 // order-preserving key of the row maximum, for caller-provided scores (rbq_topp_select); rowmax_key pre-zeroed
