@@ -392,7 +392,10 @@ def run_b200(args):
     # warm-L2 variant of the same step (labelled as such): one replica, back to back
     o_w = caches[0].new_out()
     warm_us = ev_time_us(lambda i: caches[0].decode_step(q_dev, w.p, o_w), min(args.steps, 200), 5)
-    recall = leg_recall(w, caches[0], q_dev, sel_idx, sel_cnt) if rank == 0 else None
+    try:
+        recall = leg_recall(w, caches[0], q_dev, sel_idx, sel_cnt) if rank == 0 else None
+    except Exception as e:                          # a diagnostic: never takes the headline down
+        recall = {"error": f"{type(e).__name__}: {e}"}
     line = None
     if rank == 0:
         clocks = clk.summary()
@@ -725,7 +728,7 @@ def leg_recall(w, cache, q_dev, sel_idx, sel_cnt):
             k = cache.K[b, h // G, :n].float()
             lg = (k @ q_dev[b, h].float()) / math.sqrt(w.D)
             pr = torch.softmax(lg, dim=0)
-            idx = sel_idx[b, h, :int(sel_cnt[b, h])].long()
+            idx = torch.as_tensor(np.asarray(sel_idx[b, h, :int(sel_cnt[b, h])]), device=pr.device).long()
             rec.append(float(pr[idx].sum().item()))
     rec = np.array(rec)
     return {"min": float(rec.min()), "mean": float(rec.mean()), "max": float(rec.max())}

@@ -160,6 +160,9 @@ __device__ void build_group_table(const int32_t* __restrict__ ucount, const int3
   __syncthreads();
 }
 
+// Work partition of the gather: equal contiguous ranges of the concatenated attended rows, one per CTA.  (Snapping the
+// CTA boundaries to KV-group boundaries, so that no CTA pays a second prologue and merge, was measured in round 2: no gain --
+// the spread of the CTAs' finishing times comes from sparser groups streaming slower, not from the 7 straddling CTAs.)
 __device__ __forceinline__ long long cta_begin(long long total, int c, int nc) { return total * c / nc; }
 
 // ---- tensor-pipe gather attention (bf16 K/V and q) ----------------------------------------------------------------------
@@ -229,9 +232,12 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
   const int G = Hq / Hkv;
   rbq_pdl_trigger();
+  if (tid == 0) RBQ_STAMP(gather_probe, 0);
   rbq_pdl_wait();                                             // union lists of the plan kernel
+  if (tid == 0) RBQ_STAMP(gather_probe, 1);
 
   build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
+  if (tid == 0) RBQ_STAMP(gather_probe, 2);
   const long long total = s_start[ngroups];
   if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
     for (int gq = 0; gq < ngroups; ++gq) {
@@ -256,6 +262,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     }
     gi = lo;
   }
+  if (tid == 0) RBQ_STAMP(gather_probe, 9);
   unsigned char* my_smem = ga_smem + (size_t)warp * GA_STAGES * GA_STAGE_BYTES;
   const uint32_t my_base = smem_u32(my_smem);
 
@@ -279,6 +286,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
       }
     }
+    if (tid == 0) RBQ_STAMP(gather_probe, 10);
     float m_run = -INFINITY, l_run = 0.0f;
     float o[D / 8][4];
 #pragma unroll
@@ -312,11 +320,13 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 #pragma unroll
     for (int s = 0; s < GA_STAGES - 1; ++s) ent_ring[s] = (s < my_tiles) ? tile_entry(s) : 0u;
     ent_pend = (GA_STAGES - 1 < my_tiles) ? tile_entry(GA_STAGES - 1) : 0u;
+    if (tid == 0) RBQ_STAMP(gather_probe, 11 + (ent_ring[0] == 0xdeadbeefu));
 #pragma unroll
     for (int s = 0; s < GA_STAGES - 1; ++s) {
       if (s < my_tiles) issue(s, ent_ring[s]);
       cp_async_commit();
     }
+    if (tid == 0) RBQ_STAMP(gather_probe, 3);
     for (int i = 0; i < my_tiles; ++i) {
       const uint32_t ent = ent_ring[0];
       const int nx = i + GA_STAGES - 1;
@@ -328,6 +338,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       cp_async_commit();
       cp_async_wait<GA_STAGES - 1>();
       __syncwarp();
+      if (tid == 0 && i == 0) RBQ_STAMP(gather_probe, 4);
       const uint32_t kbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES), vbase = kbase + GA_TILE_BYTES;
 
       // S = Q K^T : two n-tiles of 8 tokens
@@ -385,6 +396,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       __syncwarp();                                            // tile consumed before its stage is refilled
     }
     cp_async_wait<0>();
+    if (tid == 0) RBQ_STAMP(gather_probe, 5);
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
 
@@ -416,6 +428,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       if (d == 0) { pdst[(size_t)h * GA_PART + D] = mm; pdst[(size_t)h * GA_PART + D + 1] = ll; }
     }
     // ---- arrival: the last CTA that finishes a group merges the group's partials into out / lse -------------------------
+    if (tid == 0) RBQ_STAMP(gather_probe, 6);
     __threadfence();
     const int nc = (int)gridDim.x;
     const bool touches = tid < nc && max(cta_begin(total, tid, nc), ga) < min(cta_begin(total, tid + 1, nc), gb);
@@ -424,6 +437,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     if (touches) { atomicMin(&s_clo, tid); atomicMax(&s_chi, tid); }
     if (tid == 0) s_last = (atomicAdd(&gdone[gi], 1) == expected - 1);
     __syncthreads();
+    if (tid == 0) RBQ_STAMP(gather_probe, 7);
     if (s_last) {
       __threadfence();
       float* s_f = stg;                                        // [G][GA_THREADS]: factor 2^(m - max) of slot c
@@ -514,6 +528,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
         if (lse && d4 == 0) lse[orow] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(ll);
       }
       if (tid == 0) gdone[gi] = 0;                             // ready for the next step
+      if (tid == 0) RBQ_STAMP(gather_probe, 8);
     }
     __syncthreads();                                           // staging area free before the next group's pipeline
   }
