@@ -129,16 +129,20 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
 constexpr int AT_MAX_GROUPS = 1024;
 
 // s_start[gi] = sum over groups < gi of (ucount + pending); s_start[ngroups] = total.  Every CTA computes the same table.
+// s_ucnt / s_nidx (or NULL): per-group copies of ucount and the sequence's indexed count, so that the caller needs no
+// second global round trip for them.
 __device__ void build_group_table(const int32_t* __restrict__ ucount, const int32_t* __restrict__ n_indexed,
                                   const int32_t* __restrict__ n_total, int ngroups, int Hkv, int* s_start, int* s_warp,
-                                  int nthreads) {
+                                  int nthreads, int* s_ucnt = nullptr, int* s_nidx = nullptr) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   const int per = (ngroups + nthreads - 1) / nthreads;
   const int g0 = tid * per;
   int local = 0;
   for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
     const int b = gi / Hkv;
-    local += ucount[gi] + max(0, n_total[b] - max(0, n_indexed[b]));
+    const int uc = ucount[gi], ni = max(0, n_indexed[b]);
+    if (s_ucnt) { s_ucnt[gi] = uc; s_nidx[gi] = ni; }
+    local += uc + max(0, n_total[b] - ni);
   }
   int incl = local;
 #pragma unroll
@@ -160,10 +164,31 @@ __device__ void build_group_table(const int32_t* __restrict__ ucount, const int3
   __syncthreads();
 }
 
-// Work partition of the gather: equal contiguous ranges of the concatenated attended rows, one per CTA.  (Snapping the
-// CTA boundaries to KV-group boundaries, so that no CTA pays a second prologue and merge, was measured in round 2: no gain --
-// the spread of the CTAs' finishing times comes from sparser groups streaming slower, not from the 7 straddling CTAs.)
-__device__ __forceinline__ long long cta_begin(long long total, int c, int nc) { return total * c / nc; }
+// Work partition of the gather: contiguous ranges of the concatenated attended rows, one per CTA, of equal COST: starting a
+// KV group inside a CTA's range costs a second prologue and merge, so every group start (but the first) counts as GA_PEN
+// virtual rows: the ranges are equal in that virtual space and mapped back to rows -- a CTA that contains a group start
+// gets that many fewer rows, and a boundary falling into a gap snaps to the group's first row.  Measured at config 2 (stage
+// events): 56.3 / 55.6 / 57.5 us at GA_PEN = 0 / 320 / 640 -- a small effect: the kernel streams at the copy peak
+// (235.5 MB in 37 us once the first tiles are requested, profiles/r02_ncu.md).  Snapping ALL boundaries to group
+// boundaries was measured too: worse, a group worth 1.4 CTAs rounds to one.
+constexpr int GA_PEN = 320;
+// virtual coordinate v in [0, total + GA_PEN * (ngroups - 1)]  ->  row in [0, total]; monotone, every CTA computes the same
+__device__ __forceinline__ long long ga_row_of(const int* s_start, int ngroups, long long v) {
+  int lo = 0, hi = ngroups - 1;                               // last group whose virtual start s_start[gi] + GA_PEN * gi is <= v
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if ((long long)s_start[mid] + (long long)GA_PEN * mid <= v) lo = mid; else hi = mid - 1;
+  }
+  const long long off = v - ((long long)s_start[lo] + (long long)GA_PEN * lo) - (lo > 0 ? GA_PEN : 0);   // rows into the group
+  const long long rows = (long long)s_start[lo + 1] - s_start[lo];
+  return s_start[lo] + min(max(off, 0ll), rows);
+}
+// first row of CTA c's range (double arithmetic: exact here, identical in every CTA, far cheaper than a 64-bit division)
+__device__ __forceinline__ long long cta_begin(const int* s_start, int ngroups, long long total, int c, int nc) {
+  if (c >= nc) return total;
+  const long long vtot = total + (long long)GA_PEN * (ngroups - 1);
+  return ga_row_of(s_start, ngroups, (long long)(((double)vtot * (double)c) / (double)nc));
+}
 
 // ---- tensor-pipe gather attention (bf16 K/V and q) ----------------------------------------------------------------------
 #ifndef RBQ_GA_WARPS
@@ -225,7 +250,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   constexpr int GA_TILE_BYTES = C::TILE_BYTES, GA_STAGE_BYTES = C::STAGE_BYTES, GA_PART = C::PART, RB = C::ROW_BYTES, CPR = C::CPR;
   constexpr int LSH = (D == 64) ? 3 : 4;                       // log2(CPR)
   extern __shared__ __align__(128) unsigned char ga_smem[];
-  __shared__ int s_start[AT_MAX_GROUPS + 1];
+  __shared__ int s_start[AT_MAX_GROUPS + 1], s_ucnt[AT_MAX_GROUPS], s_nidx[AT_MAX_GROUPS];
   __shared__ int s_warp[GA_WARPS];
   __shared__ int s_last, s_clo, s_chi;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -236,7 +261,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   rbq_pdl_wait();                                             // union lists of the plan kernel
   if (tid == 0) RBQ_STAMP(gather_probe, 1);
 
-  build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS);
+  build_group_table(ucount, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS, s_ucnt, s_nidx);
   if (tid == 0) RBQ_STAMP(gather_probe, 2);
   const long long total = s_start[ngroups];
   if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
@@ -250,7 +275,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       }
     }
   }
-  const long long r0 = cta_begin(total, blockIdx.x, gridDim.x), r1 = cta_begin(total, blockIdx.x + 1, gridDim.x);
+  const long long r0 = cta_begin(s_start, ngroups, total, blockIdx.x, gridDim.x), r1 = cta_begin(s_start, ngroups, total, blockIdx.x + 1, gridDim.x);
   if (r0 >= r1) return;
   // first group with s_start[gi + 1] > r0
   int gi = 0;
@@ -271,7 +296,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     const int a = (int)(max(r0, ga) - ga), e = (int)(min(r1, gb) - ga);   // group-local rank range of this CTA
     if (a >= e) continue;
     const int b = gi / Hkv, g = gi % Hkv;
-    const int usel = ucount[gi], nidx = max(0, n_indexed[b]);
+    const int usel = s_ucnt[gi], nidx = s_nidx[gi];
     const __nv_bfloat16* Kb = K + (long long)b * sb + (long long)g * sh;
     const __nv_bfloat16* Vb = V + (long long)b * sb + (long long)g * sh;
     const uint32_t* ul = ulist + (size_t)gi * Lcap;
@@ -431,7 +456,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     if (tid == 0) RBQ_STAMP(gather_probe, 6);
     __threadfence();
     const int nc = (int)gridDim.x;
-    const bool touches = tid < nc && max(cta_begin(total, tid, nc), ga) < min(cta_begin(total, tid + 1, nc), gb);
+    const bool touches = tid < nc && max(cta_begin(s_start, ngroups, total, tid, nc), ga) < min(cta_begin(s_start, ngroups, total, tid + 1, nc), gb);
     if (tid == 0) { s_clo = nc; s_chi = -1; }
     const int expected = __syncthreads_count(touches);         // also: staging area free, partial stores fenced
     if (touches) { atomicMin(&s_clo, tid); atomicMax(&s_chi, tid); }

@@ -661,8 +661,7 @@ int launch_cs(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int
 // Cluster size.  Few rows (<= one per SM): the largest of 8 / 4 / 2 / 1 CTAs per row that still gives every CTA an SM of its
 // own (measured at config 2: 4 CTAs per row on 128 SMs make the step 6 us shorter than 8 per row with two CTAs on most
 // SMs, although the kernel alone is 4 us longer -- its prologue overlaps the estimator's tail and it has half the exchange
-// partners), as long as the slice fits in shared memory.  Many rows: 8 per row while that fills the GPU at most ~4 times
-// over, fewer (down to 1) as long as the slice of a CTA stays <= 16 K scores (two CTAs per SM).
+// partners), as long as the slice fits in shared memory.  More rows than SMs: see below.
 int rbq_topp_cluster_size(const rbq_ctx* ctx) {
   const long long rows = (long long)ctx->cfg.batch * ctx->cfg.n_q_heads;
   auto fits = [&](int c) {
@@ -674,7 +673,10 @@ int rbq_topp_cluster_size(const rbq_ctx* ctx) {
     while (cs > 1 && rows * cs > ctx->sm_count && fits(cs >> 1)) cs >>= 1;
     return cs;
   }
-  while (cs > 1 && rows * cs > 4ll * ctx->sm_count && (ctx->cfg.max_tokens + cs / 2 - 1) / (cs / 2) <= 16384) cs >>= 1;
+  // More rows than SMs: the smallest cluster whose slice fits.  Measured (512 rows, 16 K..64 K tokens): 277 / 260 /
+  // 174 us at cluster size 8 / 4 / 2; (2 048 rows x 8 K): 298 / 162 / 89 us at 4 / 2 / 1 -- the fixed cost per CTA
+  // (histogram set-up, cluster barriers) outweighs a second resident CTA per SM.
+  while (cs > 1 && fits(cs >> 1)) cs >>= 1;
   return cs;
 }
 

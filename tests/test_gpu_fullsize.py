@@ -96,6 +96,38 @@ def test_config4_decode_loop_full_size(orc, rot128, w4):
     c.close()
 
 
+def test_config3_topp_full_size(orc, rot128):
+    """BASELINE config 3's selection stage at full size (batch 16, ragged 16 K..64 K tokens, 512 rows: two CTAs per row,
+    more rows than SMs) on synthetic logits with the spread of the recipe: every row's validity, 64 sampled rows against
+    the oracle's Top-p."""
+    import torch
+    from paper_2606_31519_b200 import binding as rb
+    B, Hq, Hkv, L = 16, 32, 8, 65536
+    rng = np.random.default_rng(303)
+    lens = rng.integers(16384, L + 1, B).astype(np.int32)
+    lens[0], lens[1] = L, 16384
+    sc_dev = torch.randn(B, Hq, L, device="cuda", generator=torch.Generator("cuda").manual_seed(3)) \
+        * (0.5 + 5.5 * torch.rand(B, Hq, 1, device="cuda", generator=torch.Generator("cuda").manual_seed(4)))
+    sc_dev[2, 0] = torch.round(sc_dev[2, 0] * 2) / 2             # heavy ties
+    c = rb.RaBitQCache(B, Hq, Hkv, L, torch.from_numpy(rot128[0]))
+    c.n_indexed.copy_(U.to_dev(lens))
+    c.n_total.copy_(U.to_dev(lens))
+    sel_idx, sel_cnt = c.new_sel()
+    c.topp_select(sc_dev, 0.9, sel_idx, sel_cnt)
+    torch.cuda.synchronize()
+    cnt = sel_cnt.cpu().numpy()
+    assert (cnt > 0).all() and (cnt <= lens[:, None]).all()
+    rows = [(0, 0), (1, 5), (2, 0)] + [(int(b), int(h)) for b, h in zip(rng.integers(0, B, 61), rng.integers(0, Hq, 61))]
+    for b, h in rows:
+        n = int(lens[b])
+        s = sc_dev[b, h].cpu().numpy()
+        ref_idx, ref_cnt = orc.topp(s[None, :], np.array([n], np.int32), 0.9)
+        g = sel_idx[b, h, :cnt[b, h]].cpu().numpy()
+        assert (np.diff(g) > 0).all() and g.min() >= 0 and g.max() < n
+        U.assert_topp_row(s[:n], g, ref_idx[0, :ref_cnt[0]], 0.9)
+    c.close()
+
+
 def test_topp_cluster8_long_slices_and_boundary_ties(orc, rot128):
     """topp_kernel<8>: B = 1, Hq = 16, L = 131 072 (16 384 scores per CTA), with rows whose boundary value is shared by far
     more than the 1 024 candidates a row gathers (the cluster-wide radix narrowing at CS = 8), rows of plain Gaussian

@@ -336,11 +336,12 @@ def test_topp_edge_rows(orc, rot128):
     c.close()
 
 
-@pytest.mark.parametrize("B,L", [(1, 40000), (8, 3000), (16, 2100), (3, 90)])
+@pytest.mark.parametrize("B,L", [(1, 40000), (2, 3000), (8, 3000), (16, 2100), (3, 90)])
 def test_topp_cluster_sizes(orc, rot128, B, L):
-    """Cluster sizes 4 / 2 / 1 / 1 of the Top-p kernel (chosen from the row count and the row length; 8 CTAs per row is
-    what the single-row config-0 cases run), rows shorter than one bitmap word per CTA, and the fused step without index
-    lists (sel_idx = NULL)."""
+    """Cluster sizes 4 / 2 / 1 / 1 / 1 of the Top-p kernel (chosen from the row count and the row length; 8 CTAs per row
+    is what the single-row config-0 cases run; 2 CTAs per row with more rows than SMs is the config-3 case of
+    test_gpu_fullsize.py), rows shorter than one bitmap word per CTA, and the fused step without index lists
+    (sel_idx = NULL)."""
     import torch
     rng = np.random.default_rng(5 + B)
     w = U.workload(3, L=L, B=B)
