@@ -621,7 +621,7 @@ def leg_encode(rb, w2, steps):
     return out
 
 
-def leg_decode_loop(rb, w, rot, n_steps, label):
+def leg_decode_loop(rb, w, rot, n_steps, label, peak):
     """Configs 3 and 4 (ii): n_steps decode steps, one token per sequence appended per step (rbq_append_tokens, W = 64:
     a batched flush encode every 64 steps), decode step after every append; mean us per (append + step) with the flush on
     the main stream vs on a side stream, and the latency of the flush itself."""
@@ -671,6 +671,25 @@ def leg_decode_loop(rb, w, rot, n_steps, label):
     torch.cuda.synchronize()
     res["flush_call_us"] = a.elapsed_time(b) * 1e3
     res["flush_units"] = w.B * w.Hkv * W
+    # per-stage times (library stage events) and achieved bandwidth of the two streaming kernels at this batch size
+    c.profile_enable(True)
+    for i in range(16):
+        c.decode_step(pool[i % 8], w.p, out_t)
+    torch.cuda.synchronize()
+    ms, k = c.profile_read()
+    c.profile_enable(False)
+    st = {key: v * 1e3 / max(1, k) for key, v in ms.items()}
+    sel = c.new_sel()
+    c.decode_step(pool[0], w.p, out_t, sel[0], sel[1])
+    torch.cuda.synchronize()
+    n_idx, n_tot = c.n_indexed.cpu().numpy(), c.n_total.cpu().numpy()
+    uni, per_head = union_rows(sel[0].cpu().numpy(), sel[1].cpu().numpy(), n_idx, n_tot, w.Hkv)
+    est_b = float(n_idx.sum()) * w.Hkv * (w.D // 8 + 4)
+    att_b = float(uni) * 2 * w.D * 2
+    res["stages_us"] = st
+    res["estimator"] = {"bytes": est_b, "gbs": est_b / st["estimator"] / 1e3, "frac_measured": est_b / st["estimator"] / 1e3 / peak}
+    res["attn_gather"] = {"bytes": att_b, "gbs": att_b / st["attn_gather"] / 1e3, "frac_measured": att_b / st["attn_gather"] / 1e3 / peak}
+    res["budget_mean_tokens"] = float(sel[1].float().mean().item())
     res["overflow_flag"] = c.status_flags()
     c.close()
     return res
@@ -790,10 +809,10 @@ def run_legs(args, rb, w2, rot, peak):
         from paper_2606_31519_b200 import synth
         guarded("config3_decode_loop", lambda: leg_decode_loop(
             rb, synth.make_workload(3, extra_cap=512), rot, 128,
-            "BASELINE config 3: B=16, contexts U[16384, 65536], 32 q / 8 KV heads, bf16, p=0.9, W=64"))
+            "BASELINE config 3: B=16, contexts U[16384, 65536], 32 q / 8 KV heads, bf16, p=0.9, W=64", peak))
         guarded("config4_decode_loop", lambda: leg_decode_loop(
             rb, synth.make_workload(4, extra_cap=512), rot, 128,
-            "BASELINE config 4 (ii): B=4 x 131072, 32 q / 8 KV heads, bf16, p=0.9, W=64"))
+            "BASELINE config 4 (ii): B=4 x 131072, 32 q / 8 KV heads, bf16, p=0.9, W=64", peak))
     return legs
 
 

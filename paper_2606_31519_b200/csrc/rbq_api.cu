@@ -105,6 +105,12 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
     return RBQ_ERR_CUDA;
   }
   layout_workspace(c);
+  if (rbq_topp_init(c) != RBQ_OK) {
+    cudaEventDestroy(c->ev_copy);
+    cudaEventDestroy(c->ev_flush);
+    delete c;
+    return RBQ_ERR_CUDA;
+  }
   *out = c;
   return RBQ_OK;
 }

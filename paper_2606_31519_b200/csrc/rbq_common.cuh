@@ -240,6 +240,7 @@ int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, flo
 int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t);
 // S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.
 // rowmax_key: order-preserving keys of the row maxima [B*Hq] (written by S5), or NULL to compute them here.
+int rbq_topp_init(rbq_ctx* ctx);   // uploads the Top-p kernel's fp64 tables (once per context)
 int rbq_launch_topp(rbq_ctx*, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
                     uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
 // Alg.3 selector (ternary threshold search in fp64): ascending sel_idx, sel_cnt, optional iteration counts [B*Hq].

@@ -8,9 +8,11 @@
 // once.  The selection is an exact cut in the total order (score descending, index ascending), i.e.
 // on the composite key  C(t) = (orderkey(score_t) << 32) | ~t  whose values are all distinct.
 // The row maximum m comes with the scores (S5 epilogue, or rowmax_kernel for caller-provided scores):
-//   pass 1  : the slice is loaded by cp.async (whole slice in flight) and histogrammed: 2048 bins of width 1/64 in
-//             u = m - score (monotone in C).  Per bin a (count, sum of r) pair, r = 2^(22 - (64u - j) log2(e)/64) in
-//             2^-22 fixed point, so the bin mass is exp(-j/64) * sum(r): integer sums => order-independent, deterministic.
+//   pass 1  : the slice is loaded by cp.async (whole slice in flight) and histogrammed: 2048 bins of width 1/128 in
+//             u = m - score (monotone in C).  Per bin a (count, sum of r) pair, r = 2^(22 - (128u - j) log2(e)/128) in
+//             2^-22 fixed point, so the bin mass is exp(-j/128) * sum(r): integer sums => order-independent, deterministic.
+//             The body is branch-free (two unpredicated shared-memory reductions per token; tokens too deep to be
+//             selected -- tp_overflow_bin -- are summed in registers): the pass is bound by issue slots, not by the atomics.
 //             Only a 64-bin coarse summary (fp64) and then the 32 fine bins of the crossing coarse bin travel
 //             through distributed shared memory (DSMEM is ~20 B/clk per SM).
 //   pass 2  : ONE more pass over the resident slice classifies every token: bins above the crossing bin are selected (their
@@ -45,11 +47,19 @@ namespace cg = cooperative_groups;
 #define TP_STAMP(slot) do {} while (0)
 #endif
 
+// exp(-32 k / TP_SCALE), k < 64, then exp(-i / TP_SCALE), i < 32: the bin-edge weights in fp64, computed once on the host
+// (rbq_topp_init)
+__device__ double g_tp_tab[64 + 32];
+
 namespace {
 
-constexpr int TP_THREADS = 512;
+#ifndef RBQ_TP_THREADS
+#define RBQ_TP_THREADS 1024
+#endif
+constexpr int TP_THREADS = RBQ_TP_THREADS;     // 512 or 1024
 constexpr int TP_WARPS = TP_THREADS / 32;
-constexpr int TP_NB = 4 * TP_THREADS;          // 2048 bins, 4 per thread in the scans
+constexpr int TP_NB = 2048;                    // fine bins
+constexpr int TP_BPT = TP_NB / TP_THREADS;     // bins (and bitmap words) per thread in the scans: 4 or 2
 constexpr int TP_NC = 64;                      // coarse bins (32 fine bins each)
 constexpr int TP_CAND = 1024;                  // candidates gathered per row
 constexpr unsigned FULL = 0xffffffffu;
@@ -59,9 +69,9 @@ struct TpSmall {
   u64 wt_u[TP_WARPS];
   uint32_t wt_c[TP_WARPS];
   u64 red_lo[TP_WARPS], red_hi[TP_WARPS];
-  double tabA[TP_NC], tabB[32];                // exp(-k/2), exp(-i/64)
+  double tabA[TP_NC], tabB[32];                // exp(-32 k / TP_SCALE), exp(-i / TP_SCALE)
   // results broadcast inside the CTA
-  double trem;            // mass still needed inside the candidate range, in units of 2^-22 * exp(-bx/64)
+  double trem;            // mass still needed inside the candidate range, in units of 2^-22 * exp(-bx / TP_SCALE)
   u64 lo64, hi64;         // candidate range on C
   u64 cstar;
   uint32_t bx, cntx, cnt_above, found, ksel;
@@ -84,19 +94,39 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// fine bin j of u = m - s and the fixed-point residual weight r = exp(-(u - j/64)) * 2^22 = 2^(22 - (64u - j) log2(e)/64).
+// Bin width 1 / TP_SCALE in u = m - s (natural-log units).  128 bins per unit: 2048 bins reach 16 units, past the overflow
+// bin of a 128 K-token row at p = 0.9 (14.3 units); at 64 per unit the crossing bin of such a row held twice the tokens
+// and the all-pairs ranking of the candidates (quadratic) cost four times as much.
+constexpr float TP_SCALE = 128.0f;
+constexpr float TP_FRAC_LOG2E = -1.4426950408889634f / TP_SCALE;
+// fine bin j of u and the fixed-point residual weight r = exp(-(u - j/TP_SCALE)) * 2^22 = 2^(22 - (TP_SCALE u - j) log2(e)/TP_SCALE).
 // The XU pipe (conversions, MUFU) is the scarce unit of the histogram pass, so floor() and both float <-> int conversions
 // are done with the 2^23 magic-number add on the FMA pipe (round-down for the floor); only ex2 remains on the XU pipe.
 // 2^-22 is the resolution of ex2.approx itself.
-__device__ __forceinline__ void bin0(float m, float s, int& j, uint32_t& rfix) {
-  const float t = __fmul_rn(__fsub_rn(m, s), 64.0f);          // >= 0
-  const float jm = __fadd_rd(fminf(t, (float)(TP_NB - 1)), 8388608.0f);   // 2^23 + min(floor(t), TP_NB - 1), exact
+// jof (integer-valued, <= TP_NB - 1) is the row's OVERFLOW bin: it takes every token with u >= jof / TP_SCALE, r relative to its
+// lower edge.  Tokens that deep can never be selected (see tp_overflow_bin), so pass 1 sums them in registers.
+// t = TP_SCALE u by ONE FMA on ms = TP_SCALE m: rn(128 m - 128 s) = 128 rn(m - s), scaling by a power of two commutes with
+// rounding.
+__device__ __forceinline__ float tp_t(float ms, float s) { return fmaf(-TP_SCALE, s, ms); }   // >= 0
+__device__ __forceinline__ void bin0(float ms_, float s, float jof, int& j, uint32_t& rfix) {
+  const float t = tp_t(ms_, s);
+  const float jm = __fadd_rd(fminf(t, jof), 8388608.0f);      // 2^23 + min(floor(t), jof), exact
   j = __float_as_int(jm) - 0x4B000000;
-  const float f = __fsub_rn(t, __fsub_rn(jm, 8388608.0f));    // exact for j < TP_NB - 1; large in the overflow bin
-  rfix = __float_as_uint(__fadd_rn(ex2_approx(fmaf(f, -0.022542110013890053f, 22.0f)), 8388608.0f)) - 0x4B000000u;
+  const float f = __fsub_rn(t, __fsub_rn(jm, 8388608.0f));    // exact for j < jof; large in the overflow bin
+  rfix = __float_as_uint(__fadd_rn(ex2_approx(fmaf(f, TP_FRAC_LOG2E, 22.0f)), 8388608.0f)) - 0x4B000000u;
+}
+// Overflow bin of a row of n tokens at mass p: the tokens with u = m - s > c = ln(1.25 n / (1 - p)) have a total mass below
+// n exp(-c) = (1 - p) / 1.25 < (1 - p) Z  (Z >= 1: the maximum itself has weight 1), so the row without them still
+// covers p: the minimal covering prefix ends above them and none of them is selected.  They only count towards Z, which
+// needs no histogram: all bins from ceil(TP_SCALE c) on are one bin.  (Exactness does not rest on this bound -- a crossing inside
+// the overflow bin is resolved by the radix levels on C like any crowded bin -- only the cost does.)  At config 2 this keeps
+// 4 % .. 89 % of a row's tokens (40 % on average) out of the shared-memory atomics.  The same value in every CTA of the row.
+__device__ __forceinline__ float tp_overflow_bin(int n, float p) {
+  const float c = TP_SCALE * __logf(1.25f * (float)n / (1.0f - p));
+  return fminf(fmaxf(ceilf(c) + 1.0f, TP_SCALE), (float)(TP_NB - 1));
 }
 __device__ __forceinline__ u64 composite(float s, int t) {
-  return ((u64)rbq_fkey(s) << 32) | (u64)(~(uint32_t)t);
+  return ((u64)rbq_fkey(__fadd_rn(s, 0.0f)) << 32) | (u64)(~(uint32_t)t);   // -0 -> +0: one key for equal scores
 }
 // Histogram = two u32 arrays (all 32 banks in use): hist[j] = low 32 bits of the mass, hist[TP_NB + j] = (count << 12) |
 // (mass >> 32).  hist[j] += (count c, mass v):
@@ -110,44 +140,46 @@ __device__ __forceinline__ void hist_add(uint32_t hist_sa, int j, u64 v, uint32_
   const uint32_t carry = (old + lo < old) ? 1u : 0u;
   asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 4u * TP_NB), "r"((c << 12) + (uint32_t)(v >> 32) + carry) : "memory");
 }
-// Pass-1 form of the histogram: three u32 arrays (mass bits 0..11, mass >> 12, count) updated by three independent
-// reductions without return value -- no carry, so nothing waits for an atomic's result.  Sums stay below 2^32: at most
-// 2^16 tokens per CTA with r < 2^23.  Folded into the (lo, count | hi) form after the pass.
-__device__ __forceinline__ void hist_add3(uint32_t hist_sa, int j, u64 v, uint32_t c) {
-  const uint32_t sa = hist_sa + 4u * (uint32_t)j;
-  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa), "r"((uint32_t)v & 0xFFFu) : "memory");
-  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 4u * TP_NB), "r"((uint32_t)(v >> 12)) : "memory");
-  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(sa + 8u * TP_NB), "r"(c) : "memory");
+// Pass-1 form of the histogram: two u32 arrays, hist[j] = sum of d = 2^22 - r and hist[TP_NB + j] = count.  Inside a
+// bin r lies in (0.989 * 2^22, 2^22], so d < 2^16 and the sums of a CTA's <= 41 K tokens stay below 2^31 (read back as
+// signed: ex2.approx may return 2^22 + 1 ulp).  Two reductions without return value, never predicated: a token that is
+// not histogrammed (overflow bin, inactive lane) adds to a per-lane dummy word behind the histogram instead (ptxas turns
+// predicated shared atomics into branch + reconvergence pairs, ~3 extra issue slots each).  Folded into the
+// (lo, count | hi) form after the pass.
+__device__ __forceinline__ void hist_add2(uint32_t sa, uint32_t d, uint32_t c) {
+  asm volatile("red.shared.add.u32 [%0], %1;\n\tred.shared.add.u32 [%0 + %3], %2;" ::"r"(sa), "r"(d), "r"(c), "n"(4 * TP_NB) : "memory");
 }
 __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
   cnt = v.y >> 12;
   R = ((u64)(v.y & 0xFFFu) << 32) | v.x;
 }
 
-// totals of this thread's 4 bins over the CS histograms of the cluster (cluster-wide radix levels only)
+// totals of this thread's TP_BPT bins over the CS histograms of the cluster (cluster-wide radix levels only)
 template <int CS>
-__device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint32_t* hist, int tid, uint32_t (&cnt)[4], u64 (&R)[4]) {
+__device__ __forceinline__ void gather_bins(cg::cluster_group& cluster, uint32_t* hist, int tid, uint32_t (&cnt)[TP_BPT], u64 (&R)[TP_BPT]) {
 #pragma unroll
-  for (int k = 0; k < 4; ++k) { cnt[k] = 0; R[k] = 0; }
+  for (int k = 0; k < TP_BPT; ++k) { cnt[k] = 0; R[k] = 0; }
 #pragma unroll
   for (int r = 0; r < CS; ++r) {
     const uint32_t* rh = CS == 1 ? hist : cluster.map_shared_rank(hist, r);
-    const uint4 a = reinterpret_cast<const uint4*>(rh)[tid], b = reinterpret_cast<const uint4*>(rh + TP_NB)[tid];
-    uint32_t c; u64 v;
-    unpack_bin(make_uint2(a.x, b.x), c, v); cnt[0] += c; R[0] += v;
-    unpack_bin(make_uint2(a.y, b.y), c, v); cnt[1] += c; R[1] += v;
-    unpack_bin(make_uint2(a.z, b.z), c, v); cnt[2] += c; R[2] += v;
-    unpack_bin(make_uint2(a.w, b.w), c, v); cnt[3] += c; R[3] += v;
+#pragma unroll
+    for (int k = 0; k < TP_BPT; ++k) {
+      uint32_t c; u64 v;
+      unpack_bin(make_uint2(rh[TP_BPT * tid + k], rh[TP_NB + TP_BPT * tid + k]), c, v);
+      cnt[k] += c; R[k] += v;
+    }
   }
 }
 
-// Integer block scan over TP_NB bins (4 per thread, ascending bin = descending C): finds the bin where the inclusive
+// Integer block scan over TP_NB bins (TP_BPT per thread, ascending bin = descending C): finds the bin where the inclusive
 // prefix of R first reaches sh.trem (clamped to the total), and updates sh.{trem, cnt_above, cntx, lo64, hi64}.
 // `lo64`, `hi64`, `shift` describe the binning  bin = TP_NB-1 - ((C - lo64) >> shift).  Ends with a block barrier.
-__device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4], const u64 (&R)[4], u64 lo64, u64 hi64, int shift) {
+__device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[TP_BPT], const u64 (&R)[TP_BPT], u64 lo64, u64 hi64, int shift) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const u64 tsum = R[0] + R[1] + R[2] + R[3];
-  const uint32_t csum = cnt[0] + cnt[1] + cnt[2] + cnt[3];
+  u64 tsum = 0;
+  uint32_t csum = 0;
+#pragma unroll
+  for (int k = 0; k < TP_BPT; ++k) { tsum += R[k]; csum += cnt[k]; }
   u64 si = tsum;
   uint32_t ci = csum;
 #pragma unroll
@@ -171,14 +203,14 @@ __device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4]
     uint32_t cc = wc + ci - csum;
     int kx = -1;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < TP_BPT; ++k) {
       if (kx < 0) {
         if (tot > 0 ? ((double)(c + R[k]) >= trem) : (cnt[k] > 0)) kx = k;
         else { c += R[k]; cc += cnt[k]; }
       }
     }
-    if (kx < 0) kx = 3;
-    const int bsel = 4 * tid + kx;
+    if (kx < 0) kx = TP_BPT - 1;
+    const int bsel = TP_BPT * tid + kx;
     const u64 nmin = lo64 + ((u64)(TP_NB - 1 - bsel) << shift);
     const u64 nmax = nmin + (((u64)1 << shift) - 1ull);
     sh.lo64 = max(nmin, lo64);
@@ -193,7 +225,7 @@ __device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[4]
 // grid = (CS, rows); cluster = CS CTAs along x.
 // smem: TpSmall | hist u32[2][TP_NB] (later: selection words) | cand_all | cand_loc | scores slice [s_cap]
 template <int CS>
-__global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, 2)
+__global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, TP_THREADS == 512 ? 2 : 1)
 topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
@@ -242,86 +274,110 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
 
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
-  for (int i = tid; i < 3 * TP_NB; i += TP_THREADS) hist[i] = 0u;   // third array: start of the candidate area, free until S1
-  if (tid < TP_NC) sh.tabA[tid] = exp(-0.5 * (double)tid);
-  else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = exp(-0.015625 * (double)(tid - TP_NC));
+  const double tabv = tid < TP_NC + 32 ? g_tp_tab[tid] : 0.0;    // written at rbq_create, not by a kernel of the chain
+  for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   rbq_pdl_wait();                                             // scores and row maxima of S5
   TP_STAMP(1);
   const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
+  const float ms_ = __fmul_rn(m, TP_SCALE);
+  const float jof_f = tp_overflow_bin(n, p_f);
+  const int jof = (int)jof_f;
   __syncthreads();
   {
-    uint32_t of_c = 0;                                        // overflow bin kept in registers (can be half the row)
-    u64 of_r = 0;
+    uint32_t of_c = 0, of_r = 0;                              // overflow bin in registers (<= 128 tokens per thread, r <= 2^22 + 1)
     const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
+    const float4* sc4 = reinterpret_cast<const float4*>(sc);
     const int n4 = (len + 3) >> 2;                            // whole float4 groups (Lcap % 4 == 0: in bounds)
-    // the whole slice in flight at once (16-byte cp.async, one latency round), then histogrammed from shared memory
+    // the whole slice in flight at once (16-byte cp.async, one latency round), then histogrammed from shared memory.
+    // (Committing the rounds in four groups and starting on the first while the rest is in flight was measured: the
+    // first group lands when nearly everything has -- no gain.)
     {
       const uint32_t sdst = (uint32_t)__cvta_generic_to_shared(sc);
       for (int i4 = tid; i4 < n4; i4 += TP_THREADS)
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst + 16u * (uint32_t)i4), "l"(src + i4) : "memory");
       asm volatile("cp.async.commit_group;" ::: "memory");
+      if (tid < TP_NC) sh.tabA[tid] = tabv;                    // fp64 tables: loaded at kernel entry, first used after the pass
+      else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = tabv;
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
+    TP_STAMP(10);
+    // Branch-free body over the FULL float4 groups (each thread reads back exactly the groups it copied): an inactive lane of
+    // the last round re-reads the last group with its reductions sent to the dummy word.  The issue slots are the limiter
+    // here (measured: dropping atomics changes little).
+    const int n4f = len >> 2;
+    const uint32_t dummy_sa = hist_sa + 4u * (uint32_t)(2 * TP_NB + lane);   // and + 4 TP_NB: both in the candidate area, free until S1
 #pragma unroll 2
-    for (int base = warp * 32; base < n4; base += TP_THREADS) {
+    for (int base = warp * 32; base < n4f; base += TP_THREADS) {
       const int i4 = base + lane;
-      float v[4] = {0.f, 0.f, 0.f, 0.f};
-      if (i4 < n4) {                                            // each thread reads back exactly the groups it copied
-        const float4 t4 = reinterpret_cast<const float4*>(sc)[i4];
-        v[0] = __fadd_rn(t4.x, 0.0f); v[1] = __fadd_rn(t4.y, 0.0f); v[2] = __fadd_rn(t4.z, 0.0f); v[3] = __fadd_rn(t4.w, 0.0f);   // -0 -> +0
-        reinterpret_cast<float4*>(sc)[i4] = make_float4(v[0], v[1], v[2], v[3]);
-      }
+      const bool act = i4 < n4f;
+      const float4 t4 = sc4[act ? i4 : n4f - 1];
+      const float v[4] = {t4.x, t4.y, t4.z, t4.w};
       int j[4];
       uint32_t rf[4];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        j[k] = -1; rf[k] = 0;
-        if (4 * i4 + k < len) bin0(m, v[k], j[k], rf[k]);
-      }
+      for (int k = 0; k < 4; ++k) bin0(ms_, v[k], jof_f, j[k], rf[k]);
       const int j0 = __shfl_sync(FULL, j[0], 0);
-      if (__all_sync(FULL, j[0] == j0 && j[1] == j0 && j[2] == j0 && j[3] == j0)) {   // 128 tokens in one bin (ties)
-        u64 t = (u64)rf[0] + rf[1] + rf[2] + rf[3];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
-        if (lane == 0) {
-          if (j0 == TP_NB - 1) { of_c += 128; of_r += t; } else hist_add3(hist_sa, j0, t, 128u);
-        }
+      const bool same = act && j[0] == j0 && j[1] == j0 && j[2] == j0 && j[3] == j0;
+      if (__all_sync(FULL, same) && j0 != jof) {              // 128 tokens in one bin (ties): one pair of reductions
+        const uint32_t d = __reduce_add_sync(FULL, (4u << 22) - (rf[0] + rf[1] + rf[2] + rf[3]));
+        if (lane == 0) hist_add2(hist_sa + 4u * (uint32_t)j0, d, 128u);
       } else {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          const bool of = j[k] == TP_NB - 1;
-          of_c += of ? 1u : 0u;
-          of_r += of ? (u64)rf[k] : 0ull;
-          if (j[k] >= 0 && !of) hist_add3(hist_sa, j[k], (u64)rf[k], 1u);
+          const bool of = j[k] == jof;
+          of_c += (act && of) ? 1u : 0u;
+          of_r += (act && of) ? rf[k] : 0u;
+          hist_add2((act && !of) ? hist_sa + 4u * (uint32_t)j[k] : dummy_sa, (1u << 22) - rf[k], 1u);
         }
       }
     }
+    if ((len & 3) && tid == (n4f & (TP_THREADS - 1))) {        // the ragged tail (<= 3 tokens), by the thread that copied it
+      for (int k = 0; k < (len & 3); ++k) {
+        int j;
+        uint32_t rf;
+        bin0(ms_, sc[4 * n4f + k], jof_f, j, rf);
+        const bool of = j == jof;
+        of_c += of ? 1u : 0u;
+        of_r += of ? rf : 0u;
+        hist_add2(!of ? hist_sa + 4u * (uint32_t)j : dummy_sa, (1u << 22) - rf, 1u);
+      }
+    }
+    of_c = __reduce_add_sync(FULL, of_c);
+    u64 of_m = of_r;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { of_c += __shfl_xor_sync(FULL, of_c, o); of_r += __shfl_xor_sync(FULL, of_r, o); }
-    if (lane == 0 && of_c) hist_add3(hist_sa, TP_NB - 1, of_r, of_c);
+    for (int o = 16; o > 0; o >>= 1) of_m += __shfl_xor_sync(FULL, of_m, o);
+    if (lane == 0) { sh.wt_u[warp] = of_m; sh.wt_c[warp] = of_c; }
   }
   __syncthreads();
+  // slice padded to whole bitmap words with -inf (t = +inf: neither selected nor a candidate): pass 2 runs unguarded
+  if (tid < nwords * 32 - len) sc[len + tid] = -INFINITY;
   for (int b = tid; b < TP_NB; b += TP_THREADS) {               // fold into hist[b] = mass lo, hist[TP_NB + b] = count << 12 | mass hi
-    const u64 mass = (u64)hist[b] + ((u64)hist[TP_NB + b] << 12);
+    uint32_t cnt = hist[TP_NB + b];
+    u64 mass = ((u64)cnt << 22) - (u64)(long long)(int)hist[b];
+    if (b == jof) {                                             // the overflow bin: per-warp register totals
+      cnt = 0; mass = 0;
+      for (int w = 0; w < TP_WARPS; ++w) { cnt += sh.wt_c[w]; mass += sh.wt_u[w]; }
+    }
     hist[b] = (uint32_t)mass;
-    hist[TP_NB + b] = (hist[2 * TP_NB + b] << 12) | (uint32_t)(mass >> 32);
+    hist[TP_NB + b] = (cnt << 12) | (uint32_t)(mass >> 32);
   }
   __syncthreads();
-  // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins 4t..4t+3, 8 threads per coarse bin
+  // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins TP_BPT t .., 32 / TP_BPT threads per coarse bin
   {
+    constexpr int TPC = 32 / TP_BPT;
     double ms = 0.0;
     uint32_t cs = 0;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < TP_BPT; ++k) {
       uint32_t c; u64 R;
-      unpack_bin(make_uint2(hist[4 * tid + k], hist[TP_NB + 4 * tid + k]), c, R);
-      ms += (double)R * sh.tabB[(4 * tid + k) & 31];
+      unpack_bin(make_uint2(hist[TP_BPT * tid + k], hist[TP_NB + TP_BPT * tid + k]), c, R);
+      ms += (double)R * sh.tabB[(TP_BPT * tid + k) & 31];
       cs += c;
     }
 #pragma unroll
-    for (int o = 1; o < 8; o <<= 1) { ms += __shfl_xor_sync(FULL, ms, o); cs += __shfl_xor_sync(FULL, cs, o); }
-    if ((tid & 7) == 0) { sh.xc_mass[tid >> 3] = ms * sh.tabA[tid >> 3]; sh.xc_cnt[tid >> 3] = cs; }
+    for (int o = 1; o < TPC; o <<= 1) { ms += __shfl_xor_sync(FULL, ms, o); cs += __shfl_xor_sync(FULL, cs, o); }
+    if ((tid & (TPC - 1)) == 0) { sh.xc_mass[tid / TPC] = ms * sh.tabA[tid / TPC]; sh.xc_cnt[tid / TPC] = cs; }
   }
   TP_STAMP(2);
   csync();                                                    // S1: histograms and coarse summaries complete
@@ -402,7 +458,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   TP_STAMP(4);
   const int bx = (int)sh.bx;
   uint32_t cntx = sh.cntx;
-  const float u_lo = (float)bx * 0.015625f, u_hi = (bx == TP_NB - 1) ? INFINITY : (float)(bx + 1) * 0.015625f;
+  const float t_lo = (float)bx, t_hi = (bx == jof) ? INFINITY : (float)(bx + 1);   // the crossing bin in t = TP_SCALE u
   bool use_range = false;
 
   // ---- heavy ties only: narrow the candidate range by cluster-wide 11-bit radix levels on C --------------
@@ -410,8 +466,8 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     u64 mn = ~0ull, mx = 0ull;
     for (int i = tid; i < len; i += TP_THREADS) {
       const float s = sc[i];
-      const float u = __fsub_rn(m, s);
-      if (u >= u_lo && u < u_hi) { const u64 c = composite(s, lo + i); mn = min(mn, c); mx = max(mx, c); }
+      const float t = tp_t(ms_, s);
+      if (t >= t_lo && t < t_hi) { const u64 c = composite(s, lo + i); mn = min(mn, c); mx = max(mx, c); }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { mn = min(mn, __shfl_xor_sync(FULL, mn, o)); mx = max(mx, __shfl_xor_sync(FULL, mx, o)); }
@@ -440,7 +496,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
           const u64 c = composite(s, lo + i);
           if (c >= lo64 && c <= hi64) {
             int j_unused;
-            bin0(m, s, j_unused, rfix);
+            bin0(ms_, s, jof_f, j_unused, rfix);
             j = TP_NB - 1 - (int)((c - lo64) >> shift);       // ascending bin = descending C
           }
         }
@@ -455,8 +511,8 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
         }
       }
       csync();
-      uint32_t cnt[4];
-      u64 R[4];
+      uint32_t cnt[TP_BPT];
+      u64 R[TP_BPT];
       gather_bins<CS>(cluster, hist, tid, cnt, R);
       radix_scan(sh, cnt, R, lo64, hi64, shift);
       csync();                                                // peers done reading this level's histogram
@@ -466,41 +522,50 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   }
 
   // ---- pass 2: every token classified once: above the crossing bin -> its bit (8 lanes assemble one 32-token word);
-  //      in the crossing bin (and, after a radix narrowing, inside the candidate range) -> local candidate list ----------
+  //      in the crossing bin (and, after a radix narrowing, inside the candidate range) -> local candidate list.
+  //      Unguarded and branch-free over whole words (the pad is -inf); the candidates (a few hundred per row) take a
+  //      warp-uniform side branch ----------
   {
     u64 lo64 = 0, hi64 = 0;
     if (use_range) { lo64 = sh.lo64; hi64 = sh.hi64; }
-    const int n4r = nwords * 8;                               // float4 groups, rounded up to whole words
+    const float4* sc4 = reinterpret_cast<const float4*>(sc);
+    const int n4r = nwords * 8;                               // float4 groups of whole words
 #pragma unroll 2
     for (int base = warp * 32; base < n4r; base += TP_THREADS) {
       const int i4 = base + lane;
-      const float4 v4 = (i4 < n4r) ? reinterpret_cast<const float4*>(sc)[i4] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const bool act = i4 < n4r;
+      const float4 v4 = sc4[act ? i4 : n4r - 1];
       const float v[4] = {v4.x, v4.y, v4.z, v4.w};
-      uint32_t nib = 0;
+      uint32_t nib = 0, cm = 0;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const int i = 4 * i4 + k;
-        const float u = __fsub_rn(m, v[k]);
-        bool sel = (i < len) && (u < u_lo);
-        if (i < len && u >= u_lo && u < u_hi) {
-          const u64 c = composite(v[k], lo + i);
-          if (!use_range || (c >= lo64 && c <= hi64)) {
-            int j_unused;
-            uint32_t rfix;
-            bin0(m, v[k], j_unused, rfix);
-            const uint32_t slot = atomicAdd(&sh.lcount, 1u);
-            if (slot < TP_CAND) { loc_comp[slot] = c; loc_rfix[slot] = rfix; }
-          } else if (c > hi64) {
-            sel = true;                                       // narrowed range: above it = selected for sure
+        const float t = tp_t(ms_, v[k]);
+        nib |= (t < t_lo) ? (1u << k) : 0u;
+        cm |= (t >= t_lo && t < t_hi) ? (1u << k) : 0u;
+      }
+      if (!act) cm = 0;
+      if (__any_sync(FULL, cm != 0)) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (cm & (1u << k)) {
+            const u64 c = composite(v[k], lo + 4 * i4 + k);
+            if (!use_range || (c >= lo64 && c <= hi64)) {
+              int j_unused;
+              uint32_t rfix;
+              bin0(ms_, v[k], jof_f, j_unused, rfix);
+              const uint32_t slot = atomicAdd(&sh.lcount, 1u);
+              if (slot < TP_CAND) { loc_comp[slot] = c; loc_rfix[slot] = rfix; }
+            } else if (c > hi64) {
+              nib |= 1u << k;                                 // narrowed range: above it = selected for sure
+            }
           }
         }
-        nib |= sel ? (1u << k) : 0u;
       }
       uint32_t word = nib << (4 * (lane & 7));
       word |= __shfl_xor_sync(FULL, word, 1);
       word |= __shfl_xor_sync(FULL, word, 2);
       word |= __shfl_xor_sync(FULL, word, 4);
-      if ((lane & 7) == 0 && i4 < n4r) selw[i4 >> 3] = word;
+      if ((lane & 7) == 0 && act) selw[i4 >> 3] = word;
     }
   }
   TP_STAMP(5);
@@ -588,11 +653,11 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   if (rank == 0 && tid == 0) sel_cnt[row] = (int32_t)total_sel;
   if (sel_idx) {
     __syncthreads();
-    // exclusive scan of popc(selw) over the (<= TP_NB) words of the slice, 4 words per thread
-    uint32_t pc[4], tsum = 0;
+    // exclusive scan of popc(selw) over the (<= TP_NB) words of the slice, TP_BPT words per thread
+    uint32_t pc[TP_BPT], tsum = 0;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int w = 4 * tid + k;
+    for (int k = 0; k < TP_BPT; ++k) {
+      const int w = TP_BPT * tid + k;
       pc[k] = (w < nwords) ? __popc(selw[w]) : 0u;
       tsum += pc[k];
     }
@@ -608,8 +673,8 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     for (int w = 0; w < TP_WARPS; ++w) { if (w < warp) wp += sh.wt_c[w]; tot += sh.wt_c[w]; }
     uint32_t run = wp + si - tsum;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int w = 4 * tid + k;
+    for (int k = 0; k < TP_BPT; ++k) {
+      const int w = TP_BPT * tid + k;
       if (w < nwords) woff[w] = run;
       run += pc[k];
     }
@@ -703,6 +768,15 @@ int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, con
     case 2: return launch_cs<2>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
     default: return launch_cs<1>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
   }
+}
+
+// the fp64 bin-edge tables of the Top-p kernel, once per context (the symbol is per device)
+int rbq_topp_init(rbq_ctx* ctx) {
+  double tab[64 + 32];
+  for (int k = 0; k < 64; ++k) tab[k] = exp(-32.0 * (double)k / (double)TP_SCALE);
+  for (int i = 0; i < 32; ++i) tab[64 + i] = exp(-(double)i / (double)TP_SCALE);
+  RBQ_CUDA_OK(ctx, cudaMemcpyToSymbol(g_tp_tab, tab, sizeof(tab)));
+  return RBQ_OK;
 }
 
 int rbq_probe_copy_topp(unsigned long long* host) {
