@@ -41,10 +41,15 @@ __global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, cons
 constexpr int PL_THREADS = 1024;
 constexpr int PL_MAX_SPLIT = 16;
 
-// grid = (PL_SPLIT, B*Hkv); PL_SPLIT = the largest of 16, 8, 4, 2, 1 that keeps the grid within one wave (2 CTAs per
-// SM).  Every CTA of a group recomputes the prefix over the 128-token blocks (one block per
-// thread: 4 words x G heads), then its warps expand the blocks with blk % PL_SPLIT == blockIdx.x cooperatively
-// (lane = token bit of a word, position by popcount prefix).
+// grid = (PL_SPLIT, B*Hkv); PL_SPLIT = the largest of 16, 8, 4, 2, 1 that keeps the grid within one wave (one CTA per
+// SM: with two per SM assumed, configs 3 and 4 ran 256 CTAs in two waves).  Every CTA of a group recomputes the prefix over
+// the 128-token blocks (one block per thread: 4 words x G heads), then its warps expand the blocks with
+// blk % PL_SPLIT == blockIdx.x cooperatively (lane = token bit of a word, position by popcount prefix).
+// Measured and dropped (config 4, in-kernel stamps: 5.5 K cycles of loads + scan, 12 K cycles of expansion): one word per
+// thread walking the set bits, with direct stores (32 scattered 4-byte transactions per instruction) or staged through
+// 32 KB of shared memory and written out coalesced with entry-balanced contiguous shares -- the expansion stayed at
+// 11-13 K cycles (37 % of the union's bits are set there: ~25 issue slots per entry either way) and the step got slower
+// (config 4: 271 -> 283-288 us).
 template <int PL_SPLIT>
 __global__ void __launch_bounds__(PL_THREADS)
 attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, const int32_t* __restrict__ n_total,
@@ -800,7 +805,7 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
   int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
   int split = PL_MAX_SPLIT;
-  while (split > 1 && (long long)groups * split > 2ll * ctx->sm_count) split >>= 1;
+  while (split > 1 && (long long)groups * split > (long long)ctx->sm_count) split >>= 1;   // one wave at ONE CTA per SM (40-64 registers x 1 024 threads)
 #define RBQ_PLAN_LAUNCH(SP)                                                                                          \
   RBQ_CUDA_OK(ctx, rbq_launch_pdl(attn_plan_kernel<SP>, dim3(SP, groups), dim3(PL_THREADS), 0, s, bits,                \
                                   (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, ctx->cfg.n_q_heads,   \
