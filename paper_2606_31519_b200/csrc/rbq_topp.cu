@@ -279,11 +279,10 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   rbq_pdl_wait();                                             // scores and row maxima of S5
   TP_STAMP(1);
-  const float m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
-  const float ms_ = __fmul_rn(m, TP_SCALE);
   const float jof_f = tp_overflow_bin(n, p_f);
   const int jof = (int)jof_f;
   __syncthreads();
+  float m, ms_;                                               // row maximum: loaded behind the slice copies (one latency, not two)
   {
     uint32_t of_c = 0, of_r = 0;                              // overflow bin in registers (<= 128 tokens per thread, r <= 2^22 + 1)
     const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
@@ -297,6 +296,8 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
       for (int i4 = tid; i4 < n4; i4 += TP_THREADS)
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst + 16u * (uint32_t)i4), "l"(src + i4) : "memory");
       asm volatile("cp.async.commit_group;" ::: "memory");
+      m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
+      ms_ = __fmul_rn(m, TP_SCALE);
       if (tid < TP_NC) sh.tabA[tid] = tabv;                    // fp64 tables: loaded at kernel entry, first used after the pass
       else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = tabv;
       asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -691,7 +692,8 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   }
   TP_STAMP(9);
   TP_STAMP(13);
-  csync();                                                    // keep shared memory alive until every peer has read it
+  // keep shared memory alive until every peer has read it: after S3 only the index-list path reads a peer (x_tot)
+  if (sel_idx) csync();
   TP_STAMP(14);
 }
 
