@@ -20,7 +20,7 @@
 //             candidates; these are gathered from all CTAs in one DSMEM round; every CTA ranks its share of them against all
 //             of them with integer prefix masses (8 threads per candidate) and the one thread that finds the cut C*
 //             writes it into every CTA of the cluster.  If the crossing bin holds more than TP_CAND tokens (heavy ties),
-//             it is first narrowed by cluster-wide 11-bit radix levels on C.
+//             it is first narrowed by cluster-wide radix levels (TP_LOG_NB bits each) on C.
 //   (A variant in which the last of a KV group's row clusters also built the group's union list for S7 in its tail was
 //   measured and dropped: on 8 x 4 CTAs the expansion took 32 K cycles, the stand-alone plan kernel on 128 CTAs 8 us.)
 //   pass 3  : only the CANDIDATES are revisited: candidate t is selected  <=>  C(t) >= C*; its bit is OR-ed into the words.
@@ -47,9 +47,12 @@ namespace cg = cooperative_groups;
 #define TP_STAMP(slot) do {} while (0)
 #endif
 
-// exp(-32 k / TP_SCALE), k < 64, then exp(-i / TP_SCALE), i < 32: the bin-edge weights in fp64, computed once on the host
-// (rbq_topp_init)
-__device__ double g_tp_tab[64 + 32];
+#ifndef RBQ_TP_LOG_BINS
+#define RBQ_TP_LOG_BINS 11
+#endif
+// exp(-32 k / TP_SCALE), k < TP_NC, then exp(-i / TP_SCALE), i < 32: the bin-edge weights in fp64, computed once on the
+// host (rbq_topp_init)
+__device__ double g_tp_tab[(1 << RBQ_TP_LOG_BINS) / 32 + 32];
 
 namespace {
 
@@ -58,9 +61,11 @@ namespace {
 #endif
 constexpr int TP_THREADS = RBQ_TP_THREADS;     // 512 or 1024
 constexpr int TP_WARPS = TP_THREADS / 32;
-constexpr int TP_NB = 2048;                    // fine bins
+constexpr int TP_LOG_NB = RBQ_TP_LOG_BINS;     // 11 or 12
+constexpr int TP_NB = 1 << TP_LOG_NB;          // fine bins
+constexpr int TP_MAXW = 2048;                  // bitmap words of a slice (<= 65 536 scores per CTA)
 constexpr int TP_BPT = TP_NB / TP_THREADS;     // bins (and bitmap words) per thread in the scans: 4 or 2
-constexpr int TP_NC = 64;                      // coarse bins (32 fine bins each)
+constexpr int TP_NC = TP_NB / 32;              // coarse bins (32 fine bins each)
 constexpr int TP_CAND = 1024;                  // candidates gathered per row
 constexpr unsigned FULL = 0xffffffffu;
 typedef unsigned long long u64;
@@ -87,17 +92,19 @@ constexpr size_t TP_OFF_HIST = (sizeof(TpSmall) + 127) & ~size_t(127);
 constexpr size_t TP_OFF_A = TP_OFF_HIST + TP_NB * sizeof(uint2);                 // 24 KB: cand_all | cand_loc
 constexpr size_t TP_A_HALF = TP_CAND * 12;                                       // comp u64 + rfix u32
 constexpr size_t TP_OFF_SELW = TP_OFF_A + 2 * TP_A_HALF;                          // 8 KB: selection words of the slice (<= 2048)
-constexpr size_t TP_OFF_SC = TP_OFF_SELW + 2048 * sizeof(uint32_t);
+constexpr size_t TP_OFF_SC = TP_OFF_SELW + TP_MAXW * sizeof(uint32_t);
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// Bin width 1 / TP_SCALE in u = m - s (natural-log units).  128 bins per unit: 2048 bins reach 16 units, past the overflow
-// bin of a 128 K-token row at p = 0.9 (14.3 units); at 64 per unit the crossing bin of such a row held twice the tokens
-// and the all-pairs ranking of the candidates (quadratic) cost four times as much.
-constexpr float TP_SCALE = 128.0f;
+// Bin width 1 / TP_SCALE in u = m - s (natural-log units).  The bins reach 16 units, past the overflow bin of a 128 K-token
+// row at p = 0.9 (14.3 units).  Narrow bins keep the crossing bin small: the all-pairs ranking of its tokens (the
+// candidates) is quadratic -- 6.6 K cycles at config 2 with 2048 bins of 1/64, 4.8 K with 2048 of 1/128, 3.6 K with 4096
+// of 1/256 (RBQ_TP_LOG_BINS = 12), which however costs more in the set-up and the crossing search than it saves:
+// config 2 step 93.7 vs 94.4 us, config 3 316.9 vs 313.2, config 4 270.6 vs 267.8 -- 2048 bins stay.
+constexpr float TP_SCALE = (float)(TP_NB / 16);   // 128 or 256
 constexpr float TP_FRAC_LOG2E = -1.4426950408889634f / TP_SCALE;
 // fine bin j of u and the fixed-point residual weight r = exp(-(u - j/TP_SCALE)) * 2^22 = 2^(22 - (TP_SCALE u - j) log2(e)/TP_SCALE).
 // The XU pipe (conversions, MUFU) is the scarce unit of the histogram pass, so floor() and both float <-> int conversions
@@ -385,18 +392,23 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   TP_STAMP(3);
   if (rank == 0 && tid == 0) rowmax_key[row] = 0u;            // every CTA of the row has read its maximum: clear the key for the next step
   if (warp == 0) {
-    // coarse crossing: lane l owns coarse bins 2l, 2l+1 (totals over the cluster in rank order), warp scan in fp64;
-    // then the 32 fine bins of the crossing coarse bin, one per lane
-    double m0 = 0.0, m1 = 0.0;
-    uint32_t c0 = 0, c1 = 0;
+    // coarse crossing: lane l owns coarse bins CPL l .. CPL l + CPL - 1 (totals over the cluster in rank order), warp scan
+    // in fp64; then the 32 fine bins of the crossing coarse bin, one per lane
+    constexpr int CPL = TP_NC / 32;
+    double mk[CPL], msum = 0.0;
+    uint32_t ck[CPL], csum = 0;
+#pragma unroll
+    for (int k = 0; k < CPL; ++k) { mk[k] = 0.0; ck[k] = 0; }
 #pragma unroll
     for (int r = 0; r < CS; ++r) {
       const TpSmall* ps = peer(r);
-      m0 += ps->xc_mass[2 * lane]; m1 += ps->xc_mass[2 * lane + 1];
-      c0 += ps->xc_cnt[2 * lane]; c1 += ps->xc_cnt[2 * lane + 1];
+#pragma unroll
+      for (int k = 0; k < CPL; ++k) { mk[k] += ps->xc_mass[CPL * lane + k]; ck[k] += ps->xc_cnt[CPL * lane + k]; }
     }
-    double si2 = m0 + m1;
-    uint32_t ci2 = c0 + c1;
+#pragma unroll
+    for (int k = 0; k < CPL; ++k) { msum += mk[k]; csum += ck[k]; }
+    double si2 = msum;
+    uint32_t ci2 = csum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const double v = __shfl_up_sync(FULL, si2, o);
@@ -405,11 +417,20 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     }
     const double Z = __shfl_sync(FULL, si2, 31);
     double T = (double)p_f * Z;
-    const double ex2 = si2 - (m0 + m1);
-    const uint32_t cex = ci2 - (c0 + c1);
-    const bool x0 = c0 > 0 && ex2 + m0 >= T, x1 = c1 > 0 && (ex2 + m0) + m1 >= T;
-    unsigned cb = __ballot_sync(FULL, x0 || x1);
-    const unsigned ne = __ballot_sync(FULL, (c0 | c1) != 0);
+    const double ex2 = si2 - msum;
+    const uint32_t cex = ci2 - csum;
+    int kfirst = -1, klast = 0;                                  // first crossing bin of this lane; its last non-empty bin
+    {
+      double run = ex2;
+#pragma unroll
+      for (int k = 0; k < CPL; ++k) {
+        if (kfirst < 0 && ck[k] > 0 && run + mk[k] >= T) kfirst = k;
+        if (ck[k] > 0) klast = k;
+        run += mk[k];
+      }
+    }
+    unsigned cb = __ballot_sync(FULL, kfirst >= 0);
+    const unsigned ne = __ballot_sync(FULL, csum != 0);
     bool forced = false;
     if (cb == 0u) { cb = ne ? (1u << (31 - __clz(ne))) : 1u; forced = true; }   // rounding at the last ulp: last non-empty bin
     const int lsel = __ffs(cb) - 1;
@@ -417,10 +438,12 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     double above = 0.0;
     uint32_t cab = 0;
     if (lane == lsel) {
-      const bool second = forced ? (c1 > 0) : !x0;
-      kx = 2 * lane + (second ? 1 : 0);
-      above = second ? ex2 + m0 : ex2;
-      cab = second ? cex + c0 : cex;
+      const int ks = forced ? klast : kfirst;
+      above = ex2;
+      cab = cex;
+#pragma unroll
+      for (int k = 0; k < CPL; ++k) if (k < ks) { above += mk[k]; cab += ck[k]; }
+      kx = CPL * lane + ks;
     }
     kx = __shfl_sync(FULL, kx, lsel); above = __shfl_sync(FULL, above, lsel); cab = __shfl_sync(FULL, cab, lsel);
     uint32_t c = 0;
@@ -485,7 +508,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     use_range = true;
     while (cntx > TP_CAND) {
       const u64 range = hi64 - lo64;
-      const int shift = max(0, (64 - __clzll((long long)range)) - 11);
+      const int shift = max(0, (64 - __clzll((long long)range)) - TP_LOG_NB);
       for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
       __syncthreads();
       for (int base = warp * 32; base < len; base += TP_THREADS) {
@@ -733,7 +756,7 @@ int rbq_topp_cluster_size(const rbq_ctx* ctx) {
   const long long rows = (long long)ctx->cfg.batch * ctx->cfg.n_q_heads;
   auto fits = [&](int c) {
     const long long s_cap = ((((ctx->cfg.max_tokens + c - 1) / c) + 31) & ~31) + 32;
-    return TP_OFF_SC + (size_t)s_cap * 4 <= 227 * 1024 && s_cap <= 32 * TP_NB;
+    return TP_OFF_SC + (size_t)s_cap * 4 <= 227 * 1024 && s_cap <= 32 * TP_MAXW;
   };
   int cs = 8;
   if (rows <= ctx->sm_count) {
@@ -754,7 +777,7 @@ int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, con
   const int wpr = rbq_words_per_row(ctx);
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
   const int s_cap = ((((ctx->cfg.max_tokens + cs - 1) / cs) + 31) & ~31) + 32;
-  if (TP_OFF_SC + (size_t)s_cap * 4 > 227 * 1024 || s_cap > 32 * TP_NB)
+  if (TP_OFF_SC + (size_t)s_cap * 4 > 227 * 1024 || s_cap > 32 * TP_MAXW)
     RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "rbq_topp_select: max_tokens %d exceeds the cluster-resident limit", ctx->cfg.max_tokens);
   if (!rowmax_key) {
     uint32_t* rk = reinterpret_cast<uint32_t*>(static_cast<char*>(ctx->ws) + ctx->off_rowmax);
@@ -774,9 +797,9 @@ int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, con
 
 // the fp64 bin-edge tables of the Top-p kernel, once per context (the symbol is per device)
 int rbq_topp_init(rbq_ctx* ctx) {
-  double tab[64 + 32];
-  for (int k = 0; k < 64; ++k) tab[k] = exp(-32.0 * (double)k / (double)TP_SCALE);
-  for (int i = 0; i < 32; ++i) tab[64 + i] = exp(-(double)i / (double)TP_SCALE);
+  double tab[TP_NC + 32];
+  for (int k = 0; k < TP_NC; ++k) tab[k] = exp(-32.0 * (double)k / (double)TP_SCALE);
+  for (int i = 0; i < 32; ++i) tab[TP_NC + i] = exp(-(double)i / (double)TP_SCALE);
   RBQ_CUDA_OK(ctx, cudaMemcpyToSymbol(g_tp_tab, tab, sizeof(tab)));
   return RBQ_OK;
 }
