@@ -218,7 +218,7 @@ int rbq_query_quantize(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_
   RBQ_TRY(check_idx(ctx, idx, false));
   RBQ_TRY(need_ws(ctx));
   if (!q) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q null");
-  return rbq_launch_query(ctx, q, idx, qu, qparams, nullptr, (cudaStream_t)stream);
+  return rbq_launch_query(ctx, q, idx, qu, qparams, nullptr, false, (cudaStream_t)stream);
 }
 
 int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32_t* dot, int32_t* pop, void* stream) {
@@ -226,7 +226,7 @@ int rbq_int4_dot_binary(rbq_ctx* ctx, const void* q, const rbq_index* idx, int32
   RBQ_TRY(check_idx(ctx, idx, true));
   RBQ_TRY(need_ws(ctx));
   if (!q || !dot || !pop) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/dot/pop null");
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, false, (cudaStream_t)stream));
   return rbq_launch_estimate(ctx, idx, nullptr, dot, pop, nullptr, (cudaStream_t)stream);
 }
 
@@ -236,7 +236,7 @@ int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float
   RBQ_TRY(need_ws(ctx));
   if (!q || !scores) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/scores null");
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, (cudaStream_t)stream));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, nullptr, false, (cudaStream_t)stream));
   return rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, nullptr, (cudaStream_t)stream);
 }
 
@@ -292,7 +292,7 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   ctx->stage_ev = ev;
   uint32_t* rowmax = ws_ptr<uint32_t>(ctx, ctx->off_rowmax);   // zero between steps: S6 clears each key once it has read it
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[0], s));
-  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, q_copy, s));
+  RBQ_TRY(rbq_launch_query(ctx, q, idx, nullptr, nullptr, q_copy, /*pdl=*/q_copy == nullptr && ev == nullptr, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, rowmax, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));

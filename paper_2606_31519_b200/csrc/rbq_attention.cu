@@ -261,7 +261,6 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
   const int G = Hq / Hkv;
-  rbq_pdl_trigger();
   if (tid == 0) RBQ_STAMP(gather_probe, 0);
   rbq_pdl_wait();                                             // union lists of the plan kernel
   if (tid == 0) RBQ_STAMP(gather_probe, 1);
@@ -426,6 +425,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
       __syncwarp();                                            // tile consumed before its stage is refilled
     }
     cp_async_wait<0>();
+    rbq_pdl_trigger();                                        // dependents (the next step's S3) may become resident under the merge phase
     if (tid == 0) RBQ_STAMP(gather_probe, 5);
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);

@@ -235,7 +235,8 @@ int rbq_launch_set_counts(rbq_ctx*, const int32_t* seq_lens, int32_t* n_indexed,
 int rbq_launch_append_copy(rbq_ctx*, const void* k_new, const void* v_new, int n_new, const RbqKV&,
                            int32_t* n_indexed, int32_t* n_total, int commit, cudaStream_t);
 // q_copy (or NULL): device buffer that receives a verbatim copy of q (used when q lives in mapped host memory)
-int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t);
+// pdl: launched with programmatic stream serialisation (the kernel waits for its predecessor before it reads q or writes)
+int rbq_launch_query(rbq_ctx*, const void* q, const rbq_index*, uint8_t* qu, float* qparams, void* q_copy, bool pdl, cudaStream_t);
 // S4/S5 behind an rbq_launch_query.  rowmax_key: zeroed keys that receive the row maxima, or NULL.
 int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot, int32_t* pop, uint32_t* rowmax_key, cudaStream_t);
 // S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.

@@ -30,6 +30,8 @@
 //   score = f_scale*(cA*acc_d + cB*acc_p) + cD [+ sm_scale*f_bias].
 #include "rbq_common.cuh"
 
+RBQ_PROBE_DECL(est_probe);
+
 namespace {
 
 constexpr int EST_THREADS = 256;
@@ -107,6 +109,7 @@ estimate_kernel(const uint32_t* __restrict__ codes, const void* __restrict__ f_s
                 uint32_t* __restrict__ rowmax_key) {
   __shared__ int s_gstart[EST_MAX_B + 1];     // exclusive prefix over sequences of Hkv * ceil(n_b / 32)
   rbq_pdl_trigger();                            // the wait for S3 comes after the first code loads are in flight
+  if (threadIdx.x == 0) RBQ_STAMP(est_probe, 0);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3, G = Hq / Hkv;
   if (tid == 0) {
@@ -165,7 +168,7 @@ estimate_kernel(const uint32_t* __restrict__ codes, const void* __restrict__ f_s
     GroupLoad<W> l0 = load_at(g0), l1 = l0, l2 = l0;
     if (g0 + 1 < g1) l1 = load_at(g0 + 1);
     if (g0 + 2 < g1) l2 = load_at(g0 + 2);
-    if (first_segment) { rbq_pdl_wait(); first_segment = false; }   // S3's query constants and zeroed row maxima
+    if (first_segment) { rbq_pdl_wait(); first_segment = false; if (tid == 0) RBQ_STAMP(est_probe, 1); }   // S3's query constants and zeroed row maxima
     const RbqQConst* qc = qconst + bg;
     uint32_t bf[W][2];
 #pragma unroll
@@ -236,6 +239,7 @@ estimate_kernel(const uint32_t* __restrict__ codes, const void* __restrict__ f_s
     }
     gcur += g1 - g0;
   }
+  if (tid == 0) RBQ_STAMP(est_probe, 2);
 }
 
 template <int W, bool INT_OUT, bool HAS_BIAS, bool F16>
@@ -283,6 +287,11 @@ int rbq_launch_estimate(rbq_ctx* ctx, const rbq_index* idx, float* scores, int32
 }
 
 int rbq_probe_copy_estimate(unsigned long long* host) {
+#ifdef RBQ_PROBE
+  if (cudaDeviceSynchronize() != cudaSuccess) return RBQ_ERR_CUDA;
+  return cudaMemcpyFromSymbol(host, est_probe, sizeof(unsigned long long) * RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS) == cudaSuccess ? RBQ_OK : RBQ_ERR_CUDA;
+#else
   (void)host;
-  return RBQ_ERR_UNSUPPORTED;      // no stamps in this kernel
+  return RBQ_ERR_UNSUPPORTED;
+#endif
 }

@@ -31,6 +31,12 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
     }
     __syncthreads();                               // barrier initialised for everyone
   }
+  // Launched with programmatic stream serialisation inside the decode step: the launch latency and the copy of P (a
+  // constant of the context) overlap the tail of whatever precedes the step on the stream -- in a decode loop the merge
+  // phase of the previous step's gather attention, which triggers its dependents when its streaming loop is done.
+  // Everything else (q is the caller's, qconst is still read by that step's estimator until its chain has completed)
+  // waits here.  Returns at once after an ordinary launch.
+  rbq_pdl_wait();
   const int bgs[1] = {(int)blockIdx.x};
   const int rows0[1] = {((int)blockIdx.x / Hkv) * Hq + ((int)blockIdx.x % Hkv) * (Hq / Hkv)};
   rbq_qprep<TQ, D, 1, P_SMEM>(q, c_q, c_k, rot, s_rot, bar, rot_kind, Hq, Hkv, bgs, rows0, sm_scale, &sm, (int)threadIdx.x, QK_THREADS, 0,
@@ -38,30 +44,35 @@ query_kernel(const TQ* __restrict__ q, const float* __restrict__ c_q, const floa
 }
 
 template <typename TQ, int D>
-int launch_d(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t s) {
+int launch_d(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, bool pdl, cudaStream_t s) {
   const int BG = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   RbqQConst* qc = reinterpret_cast<RbqQConst*>(static_cast<char*>(ctx->ws) + ctx->off_qconst);
   const size_t smem = (ctx->cfg.rot_kind == RBQ_ROT_DENSE && D <= 128) ? (size_t)D * D * sizeof(float) : 0;
   auto kern = query_kernel<TQ, D>;
   RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_QUERY + (D == 64 ? 0 : D == 128 ? 1 : 2) * 2 + (sizeof(TQ) == 2 ? 0 : 1), kern, (D <= 128 ? D * D * sizeof(float) : 0));
-  kern<<<BG, QK_THREADS, smem, s>>>((const TQ*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind, ctx->cfg.n_q_heads,
-                                    ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, (TQ*)q_copy);
+  if (pdl)
+    RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, dim3(BG), dim3(QK_THREADS), smem, s, (const TQ*)q, (const float*)idx->c_q, (const float*)idx->c_k,
+                                    (const float*)ctx->cfg.rot, ctx->cfg.rot_kind, ctx->cfg.n_q_heads, ctx->cfg.n_kv_heads, ctx->sm_scale,
+                                    qu, qparams, qc, (TQ*)q_copy));
+  else
+    kern<<<BG, QK_THREADS, smem, s>>>((const TQ*)q, idx->c_q, idx->c_k, ctx->cfg.rot, ctx->cfg.rot_kind, ctx->cfg.n_q_heads,
+                                      ctx->cfg.n_kv_heads, ctx->sm_scale, qu, qparams, qc, (TQ*)q_copy);
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
 
 template <typename TQ>
-int launch_q(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t s) {
+int launch_q(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, bool pdl, cudaStream_t s) {
   switch (ctx->cfg.head_dim) {
-    case 64: return launch_d<TQ, 64>(ctx, q, idx, qu, qparams, q_copy, s);
-    case 256: return launch_d<TQ, 256>(ctx, q, idx, qu, qparams, q_copy, s);
-    default: return launch_d<TQ, 128>(ctx, q, idx, qu, qparams, q_copy, s);
+    case 64: return launch_d<TQ, 64>(ctx, q, idx, qu, qparams, q_copy, pdl, s);
+    case 256: return launch_d<TQ, 256>(ctx, q, idx, qu, qparams, q_copy, pdl, s);
+    default: return launch_d<TQ, 128>(ctx, q, idx, qu, qparams, q_copy, pdl, s);
   }
 }
 
 }  // namespace
 
-int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, cudaStream_t s) {
-  if (ctx->cfg.q_dtype == RBQ_BF16) return launch_q<__nv_bfloat16>(ctx, q, idx, qu, qparams, q_copy, s);
-  return launch_q<float>(ctx, q, idx, qu, qparams, q_copy, s);
+int rbq_launch_query(rbq_ctx* ctx, const void* q, const rbq_index* idx, uint8_t* qu, float* qparams, void* q_copy, bool pdl, cudaStream_t s) {
+  if (ctx->cfg.q_dtype == RBQ_BF16) return launch_q<__nv_bfloat16>(ctx, q, idx, qu, qparams, q_copy, pdl, s);
+  return launch_q<float>(ctx, q, idx, qu, qparams, q_copy, pdl, s);
 }
