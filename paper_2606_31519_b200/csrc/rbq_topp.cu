@@ -156,6 +156,32 @@ __device__ __forceinline__ void hist_add(uint32_t hist_sa, int j, u64 v, uint32_
 __device__ __forceinline__ void hist_add2(uint32_t sa, uint32_t d, uint32_t c) {
   asm volatile("red.shared.add.u32 [%0], %1;\n\tred.shared.add.u32 [%0 + %3], %2;" ::"r"(sa), "r"(d), "r"(c), "n"(4 * TP_NB) : "memory");
 }
+// Histogram step of pass 1 for the four scores of one float4 group.  A token of the overflow bin (or of an inactive lane:
+// d = c = 0) goes to one of TP_OFS per-(warp & 3, lane) slot pairs behind the histogram -- conflict-free, and no register
+// bookkeeping: <= 320 tokens per slot, d <= 2^22, so a slot's sum stays below 2^31.  128 tokens in one bin (ties): one pair
+// of reductions for the warp.
+constexpr int TP_OFS = 128;
+template <bool ALL_ACTIVE>
+__device__ __forceinline__ void tp_hist4(const float4 t4, bool act, float ms_, float jof_f, int jof, uint32_t hist_sa, uint32_t slot_sa, int lane) {
+  const float v[4] = {t4.x, t4.y, t4.z, t4.w};
+  int j[4];
+  uint32_t rf[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) bin0(ms_, v[k], jof_f, j[k], rf[k]);
+  const int j0 = __shfl_sync(FULL, j[0], 0);
+  const bool same = (ALL_ACTIVE || act) && j[0] == j0 && j[1] == j0 && j[2] == j0 && j[3] == j0;
+  if (__all_sync(FULL, same) && j0 != jof) {
+    const uint32_t d = __reduce_add_sync(FULL, (4u << 22) - (rf[0] + rf[1] + rf[2] + rf[3]));
+    if (lane == 0) hist_add2(hist_sa + 4u * (uint32_t)j0, d, 128u);
+  } else {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const bool tobin = (ALL_ACTIVE || act) && j[k] != jof;
+      const uint32_t d = (1u << 22) - rf[k];
+      hist_add2(tobin ? hist_sa + 4u * (uint32_t)j[k] : slot_sa, (ALL_ACTIVE || act) ? d : 0u, (ALL_ACTIVE || act) ? 1u : 0u);
+    }
+  }
+}
 __device__ __forceinline__ void unpack_bin(uint2 v, uint32_t& cnt, u64& R) {
   cnt = v.y >> 12;
   R = ((u64)(v.y & 0xFFFu) << 32) | v.x;
@@ -283,6 +309,7 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
   const double tabv = tid < TP_NC + 32 ? g_tp_tab[tid] : 0.0;    // written at rbq_create, not by a kernel of the chain
   for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
+  if (tid < TP_OFS) { hist[2 * TP_NB + tid] = 0u; hist[3 * TP_NB + tid] = 0u; }   // overflow slots (candidate area, free until S1)
   if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   rbq_pdl_wait();                                             // scores and row maxima of S5
   TP_STAMP(1);
@@ -291,7 +318,6 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   __syncthreads();
   float m, ms_;                                               // row maximum: loaded behind the slice copies (one latency, not two)
   {
-    uint32_t of_c = 0, of_r = 0;                              // overflow bin in registers (<= 128 tokens per thread, r <= 2^22 + 1)
     const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
     const float4* sc4 = reinterpret_cast<const float4*>(sc);
     const int n4 = (len + 3) >> 2;                            // whole float4 groups (Lcap % 4 == 0: in bounds)
@@ -310,65 +336,55 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     TP_STAMP(10);
-    // Branch-free body over the FULL float4 groups (each thread reads back exactly the groups it copied): an inactive lane of
-    // the last round re-reads the last group with its reductions sent to the dummy word.  The issue slots are the limiter
-    // here (measured: dropping atomics changes little).
+    // Branch-free body over the FULL float4 groups (each thread reads back exactly the groups it copied); whole rounds first,
+    // then the last, partial round, whose inactive lanes re-read the last group and add zeros.  The issue slots are the
+    // limiter here (measured: dropping atomics changes little; ncu: 'not selected' is the top stall).
     const int n4f = len >> 2;
-    const uint32_t dummy_sa = hist_sa + 4u * (uint32_t)(2 * TP_NB + lane);   // and + 4 TP_NB: both in the candidate area, free until S1
+    const uint32_t slot_sa = hist_sa + 4u * (uint32_t)(2 * TP_NB + (warp & 3) * 32 + lane);   // count slot: + 4 TP_NB
+    const int full = n4f & ~(TP_THREADS - 1);
 #pragma unroll 2
-    for (int base = warp * 32; base < n4f; base += TP_THREADS) {
-      const int i4 = base + lane;
+    for (int i4 = tid; i4 < full; i4 += TP_THREADS) tp_hist4<true>(sc4[i4], true, ms_, jof_f, jof, hist_sa, slot_sa, lane);
+    if (full + warp * 32 < n4f) {                              // warp-uniform
+      const int i4 = full + tid;
       const bool act = i4 < n4f;
-      const float4 t4 = sc4[act ? i4 : n4f - 1];
-      const float v[4] = {t4.x, t4.y, t4.z, t4.w};
-      int j[4];
-      uint32_t rf[4];
-#pragma unroll
-      for (int k = 0; k < 4; ++k) bin0(ms_, v[k], jof_f, j[k], rf[k]);
-      const int j0 = __shfl_sync(FULL, j[0], 0);
-      const bool same = act && j[0] == j0 && j[1] == j0 && j[2] == j0 && j[3] == j0;
-      if (__all_sync(FULL, same) && j0 != jof) {              // 128 tokens in one bin (ties): one pair of reductions
-        const uint32_t d = __reduce_add_sync(FULL, (4u << 22) - (rf[0] + rf[1] + rf[2] + rf[3]));
-        if (lane == 0) hist_add2(hist_sa + 4u * (uint32_t)j0, d, 128u);
-      } else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const bool of = j[k] == jof;
-          of_c += (act && of) ? 1u : 0u;
-          of_r += (act && of) ? rf[k] : 0u;
-          hist_add2((act && !of) ? hist_sa + 4u * (uint32_t)j[k] : dummy_sa, (1u << 22) - rf[k], 1u);
-        }
-      }
+      tp_hist4<false>(sc4[act ? i4 : n4f - 1], act, ms_, jof_f, jof, hist_sa, slot_sa, lane);
     }
     if ((len & 3) && tid == (n4f & (TP_THREADS - 1))) {        // the ragged tail (<= 3 tokens), by the thread that copied it
       for (int k = 0; k < (len & 3); ++k) {
         int j;
         uint32_t rf;
         bin0(ms_, sc[4 * n4f + k], jof_f, j, rf);
-        const bool of = j == jof;
-        of_c += of ? 1u : 0u;
-        of_r += of ? rf : 0u;
-        hist_add2(!of ? hist_sa + 4u * (uint32_t)j : dummy_sa, (1u << 22) - rf, 1u);
+        hist_add2(j != jof ? hist_sa + 4u * (uint32_t)j : slot_sa, (1u << 22) - rf, 1u);
       }
     }
-    of_c = __reduce_add_sync(FULL, of_c);
-    u64 of_m = of_r;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) of_m += __shfl_xor_sync(FULL, of_m, o);
-    if (lane == 0) { sh.wt_u[warp] = of_m; sh.wt_c[warp] = of_c; }
   }
   __syncthreads();
   // slice padded to whole bitmap words with -inf (t = +inf: neither selected nor a candidate): pass 2 runs unguarded
   if (tid < nwords * 32 - len) sc[len + tid] = -INFINITY;
   for (int b = tid; b < TP_NB; b += TP_THREADS) {               // fold into hist[b] = mass lo, hist[TP_NB + b] = count << 12 | mass hi
-    uint32_t cnt = hist[TP_NB + b];
-    u64 mass = ((u64)cnt << 22) - (u64)(long long)(int)hist[b];
-    if (b == jof) {                                             // the overflow bin: per-warp register totals
-      cnt = 0; mass = 0;
-      for (int w = 0; w < TP_WARPS; ++w) { cnt += sh.wt_c[w]; mass += sh.wt_u[w]; }
-    }
+    if (b == jof) continue;                                     // the overflow bin: from its slots, below
+    const uint32_t cnt = hist[TP_NB + b];
+    const u64 mass = ((u64)cnt << 22) - (u64)(long long)(int)hist[b];
     hist[b] = (uint32_t)mass;
     hist[TP_NB + b] = (cnt << 12) | (uint32_t)(mass >> 32);
+  }
+  if (warp == 0) {                                              // overflow bin = its own (empty) histogram word + the TP_OFS slots
+    uint32_t cnt = 0;
+    long long dsum = 0;
+#pragma unroll
+    for (int k = 0; k < TP_OFS / 32; ++k) {
+      cnt += hist[3 * TP_NB + 32 * k + lane];
+      dsum += (long long)(int)hist[2 * TP_NB + 32 * k + lane];
+    }
+    cnt = __reduce_add_sync(FULL, cnt);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dsum += __shfl_xor_sync(FULL, dsum, o);
+    if (lane == 0) {
+      cnt += hist[TP_NB + jof];
+      const u64 mass = ((u64)cnt << 22) - (u64)(dsum + (long long)(int)hist[jof]);
+      hist[jof] = (uint32_t)mass;
+      hist[TP_NB + jof] = (cnt << 12) | (uint32_t)(mass >> 32);
+    }
   }
   __syncthreads();
   // coarse summary of this CTA: 64 bins of 32 fine bins; thread t owns fine bins TP_BPT t .., 32 / TP_BPT threads per coarse bin
