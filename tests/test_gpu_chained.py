@@ -92,6 +92,37 @@ def test_decode_step_chained_f16_factors(orc, cfg, kw, D, kind):
     c.close()
 
 
+def test_back_to_back_steps_with_different_queries(orc, rot128):
+    """Six decode steps enqueued back to back without a host synchronize, each with its own q and its own output buffer:
+    S3 of step n + 1 is launched with programmatic stream serialisation and may become resident under the tail of step
+    n's gather attention, so it must neither overwrite the query constants step n still reads nor read q early.  Every
+    step's output, budgets and selected sets against the oracle; then the same six queries again in reverse order."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    w = U.workload(1, L=9001)
+    rot = rot128[0]
+    o = U.oracle_index(orc, w, rot, ROT_DENSE)
+    c = U.make_cache(w, rot)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    pool = synth.query_pool(w, 6)
+    dt = U.torch_dtype(w)
+    q_dev = [U.to_dev(pool[i], dt) for i in range(6)]
+    refs = [orc.decode_step(pool[i], w.K, w.V, o["codes"], o["f_scale"], None, o["c_k"], None, o["n_indexed"], o["n_total"],
+                            ROT_DENSE, rot, w.p, U.SM_SCALE) for i in range(6)]
+    for order in (range(6), reversed(range(6))):
+        order = list(order)
+        outs = [c.new_out() for _ in order]
+        cnts = [c.new_sel()[1] for _ in order]
+        for k, i in enumerate(order):
+            c.decode_step(q_dev[i], w.p, outs[k], None, cnts[k])
+        torch.cuda.synchronize()
+        for k, i in enumerate(order):
+            U.assert_attention_close(outs[k].cpu().numpy(), refs[i]["out"], w.kv_dtype)
+            d = np.abs(cnts[k].cpu().numpy().astype(np.int64) - refs[i]["sel_cnt"])
+            assert d.max() <= max(2, int(0.002 * refs[i]["sel_cnt"].max())), f"step {k} (query {i}): budgets differ by {d.max()}"
+    c.close()
+
+
 def test_decode_step_chained_with_cq(orc, rot128):
     _chained(orc, U.workload(0, with_cq=True), rot128[0], ROT_DENSE, 0.9, with_cq=True)
 
