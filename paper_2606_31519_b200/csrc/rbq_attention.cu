@@ -59,10 +59,12 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
   __shared__ uint32_t s_pre[PL_THREADS], s_cntb[PL_THREADS];
   __shared__ uint32_t s_base;
   rbq_pdl_trigger();
-  rbq_pdl_wait();                                             // selection bitmaps of S6
   const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // n_indexed is an input of the step (committed before S3, which starts only when the kernel in front of it has
+  // completed): loaded before the wait, one dependent round trip less behind it
   const int nidx = max(0, n_indexed[b]);
+  rbq_pdl_wait();                                             // selection bitmaps of S6
   const int nw = (nidx + 31) >> 5, nblk = (nw + 3) >> 2;
   const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
   uint32_t* __restrict__ out = ulist + (size_t)gi * Lcap;
