@@ -695,6 +695,32 @@ def leg_decode_loop(rb, w, rot, n_steps, label, peak):
     return res
 
 
+def leg_gather4(rb, rot, peak):
+    """SURVEY 7 hard part 5 / VERDICT r1 item 5(c): random 256-byte row gathers by 16-byte cp.async (what S7 uses) against TMA
+    tile::gather4, on separate K and V matrices and on one matrix of interleaved K | V rows; rbq_diag_gather streams ~462 K
+    of 1 M rows (config 2's union density) with the gather kernel's launch shape and pipeline depth, cold L2 over 4 replicas."""
+    import torch
+    c = rb.RaBitQCache(1, 32, 8, 4096, rot)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(3)
+    n_rows, R = 8 * 131072, 4
+    Ks = [torch.randn(n_rows, 128, device="cuda", generator=g).to(torch.bfloat16) for _ in range(R)]
+    Vs = [torch.randn(n_rows, 128, device="cuda", generator=g).to(torch.bfloat16) for _ in range(R)]
+    rows = torch.nonzero(torch.rand(n_rows, device="cuda", generator=g) < 0.44).flatten().to(torch.int32)
+    cs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    out = {"rows": int(rows.numel()), "of_rows": n_rows, "bytes": int(rows.numel()) * 512}
+    names = {0: "cp_async_separate_kv", 1: "tma_gather4_separate_kv", 2: "cp_async_interleaved_kv", 3: "tma_gather4_interleaved_kv"}
+    for mode in (0, 1, 2, 3):
+        if mode == 2:
+            Ks = [torch.cat([Ks[r], Vs[r]], dim=1).contiguous() for r in range(R)]
+            Vs = [None] * R
+            torch.cuda.empty_cache()
+        us = ev_time_us(lambda i: rb.rbq_diag_gather(c.ctx, Ks[i % R], Vs[i % R], rows, mode, cs), 40)
+        out[names[mode]] = {"us": us, "gbs": out["bytes"] / us / 1e3, "frac_measured": out["bytes"] / us / 1e3 / peak}
+    c.close()
+    return out
+
+
 def leg_prefill(rb, w1, rot, steps):
     """SURVEY 8(f3) / PAPER.md:L213, L341 (<10 % TTFT overhead): one layer's causal prefill attention (torch SDPA, a library
     call standing in for the model) on the main stream, alone vs with rbq_encode_keys of the same keys on a low-priority
@@ -805,6 +831,7 @@ def run_legs(args, rb, w2, rot, peak):
     guarded("estimator_variants", lambda: leg_estimator_variants(rb, steps, peak))
     guarded("config4_encode", lambda: leg_encode(rb, w2, steps))
     guarded("prefill_overlap", lambda: leg_prefill(rb, build_workload(1, None), rot, steps))
+    guarded("gather4_experiment", lambda: leg_gather4(rb, rot, peak))
     if not args.quick:
         from paper_2606_31519_b200 import synth
         guarded("config3_decode_loop", lambda: leg_decode_loop(

@@ -216,6 +216,19 @@ int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host);
  * uint64 to out_host.  The regular library returns RBQ_ERR_UNSUPPORTED.                                             */
 int rbq_probe_dump(rbq_ctx* ctx, int kernel, uint64_t* out_host);
 
+/* ---- row-gather experiment (measurement aid, hard part 5; Alg.2 line 14: the gather of the
+ * selected K / V rows) --------------------------------------------------------------------------------------------------- */
+/* Streams the rows rows[0 .. n) (device, int32, each in [0, n_rows_total)) of two bf16 matrices K and V (device,
+ * [n_rows_total][128], contiguous 256-byte rows) through shared memory with the launch shape and pipeline depth of the gather
+ * attention kernel (one persistent CTA per SM, 8 warps x 3 stages x 16-row K + V tiles) and adds the sum of all gathered
+ * 32-bit words to *checksum (device, uint64, NOT cleared by the call).  mode 0: 16-byte cp.async per lane (what S7 uses);
+ * mode 1: TMA cp.async.bulk.tensor.2d tile::gather4, four rows per instruction; modes 2 / 3: the same two with K pointing at
+ * ONE matrix of interleaved K | V rows ([n_rows_total][256], 512-byte rows; V is ignored and may be NULL).  Asynchronous on
+ * `stream`; nothing of the context's state is touched.  Errors: RBQ_ERR_INVALID_ARG, RBQ_ERR_UNSUPPORTED (no tensor-map
+ * entry point in the driver), RBQ_ERR_CUDA.                                                                            */
+int rbq_diag_gather(rbq_ctx* ctx, const void* K, const void* V, long long n_rows_total, const int32_t* rows, long long n,
+                    int mode, unsigned long long* checksum, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

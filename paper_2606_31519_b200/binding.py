@@ -31,7 +31,7 @@ RBQ_CK_GIVEN = 1
 EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspace", "rbq_last_error",
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
            "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_topp_select_alg3", "rbq_sparse_attention",
-           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags", "rbq_probe_dump"]
+           "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags", "rbq_probe_dump", "rbq_diag_gather"]
 N_STAGES = 5
 STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather"]
 
@@ -88,6 +88,7 @@ def load():
         "rbq_profile_read": ([vp, C.POINTER(C.c_float), C.POINTER(i32)], C.c_int),
         "rbq_status_flags": ([vp, C.POINTER(u32), vp], C.c_int),
         "rbq_probe_dump": ([vp, C.c_int, vp], C.c_int),
+        "rbq_diag_gather": ([vp, vp, vp, C.c_longlong, vp, C.c_longlong, C.c_int, vp, vp], C.c_int),
     }
     for name, (args, res) in sig.items():
         fn = getattr(lib, name)
@@ -223,6 +224,20 @@ def rbq_probe_dump(ctx, kernel: int) -> np.ndarray:
     out = np.zeros((256, 16), np.uint64)
     _check(ctx, load().rbq_probe_dump(ctx, int(kernel), out.ctypes.data_as(C.c_void_p)), "rbq_probe_dump")
     return out
+
+
+def rbq_diag_gather(ctx, K, V, rows, mode: int, checksum, stream=None) -> None:
+    """Row-gather experiment (rbq.h): modes 0 / 1: K, V bf16 [n_rows_total][128] contiguous; modes 2 / 3: K = interleaved
+    K | V rows, bf16 [n_rows_total][256], V = None.  rows int32 [n], checksum int64 [1] (added to).  Even modes: cp.async
+    staging, odd modes: TMA tile::gather4."""
+    width = 128 if mode < 2 else 256
+    assert K.dtype == torch.bfloat16 and K.is_contiguous() and K.shape[-1] == width
+    assert rows.dtype == torch.int32 and checksum.dtype == torch.int64
+    if mode < 2:
+        assert V.dtype == torch.bfloat16 and V.is_contiguous() and V.shape == K.shape
+    n_total = K.numel() // width
+    _check(ctx, load().rbq_diag_gather(ctx, _ptr(K), _ptr(V) if mode < 2 else None, n_total, _ptr(rows), rows.numel(), int(mode),
+                                       _ptr(checksum), _stream(stream)), "rbq_diag_gather")
 
 
 def rbq_status_flags(ctx, stream=None) -> int:
