@@ -154,6 +154,19 @@ int rbq_estimate_scores(rbq_ctx* ctx, const void* q, const rbq_index* idx, float
 int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p,
                     int32_t* sel_idx, int32_t* sel_cnt, void* stream);
 
+/* The same operation (same kernels, same results bit for bit) for callers that cannot allocate device memory or hand over
+ * a workspace (code under CUDA graph capture, tight serving loops): needs NO workspace (rbq_set_workspace may never have been
+ * called) and calls no cudaMalloc / cudaFree / allocating routine.  Its scratch -- the row-maximum keys and the per-row
+ * selection bitmaps, 4 * (roundup(B*Hq, 64) + B*Hq * roundup(ceil(Lcap/32), 4)) bytes -- lives in ONE static device array
+ * of 2 MiB inside the library (every GPU that loads the library holds it until exit), so
+ *   B*Hq * (Lcap/32 + 1)  must stay below 524 288 words (e.g. 32 rows x 131 072 tokens; 128 rows x 65 536 tokens);
+ * beyond that: RBQ_ERR_UNSUPPORTED with the sizes in rbq_last_error -- use rbq_topp_select.  All calls (all contexts of the
+ * process on one device) share the array: it keeps the last call's contents (what must start at zero is cleared per call),
+ * and two calls that overlap on the GPU (different streams, no ordering) race.  Arguments, layouts, ownership and the
+ * other errors as for rbq_topp_select; asynchronous on `stream`.                                                      */
+int rbq_topp_select_static(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p,
+                           int32_t* sel_idx, int32_t* sel_cnt, void* stream);
+
 /* ---- S6'  the paper's Top-p operator: Algorithm 3, ternary threshold search (L217-252; 4.1 L256-264;
  *           App. B.1) -- alternative selector, SURVEY.md 8(f) row 2 --------------------- */
 /* Per row: prob = softmax(scores[b][h][0..n_indexed[b])) in fp64; low = 0, high = max(prob); repeat

@@ -30,7 +30,7 @@ RBQ_CK_GIVEN = 1
 
 EXPORTS = ["rbq_create", "rbq_destroy", "rbq_workspace_bytes", "rbq_set_workspace", "rbq_last_error",
            "rbq_launch_count", "rbq_encode_keys", "rbq_append_tokens", "rbq_query_quantize",
-           "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_topp_select_alg3", "rbq_sparse_attention",
+           "rbq_int4_dot_binary", "rbq_estimate_scores", "rbq_topp_select", "rbq_topp_select_static", "rbq_topp_select_alg3", "rbq_sparse_attention",
            "rbq_decode_step", "rbq_decode_step_host", "rbq_profile_enable", "rbq_profile_read", "rbq_status_flags", "rbq_probe_dump", "rbq_diag_gather"]
 N_STAGES = 5
 STAGE_NAMES = ["query_prep", "estimator", "topp", "attn_plan", "attn_gather"]
@@ -80,6 +80,7 @@ def load():
         "rbq_int4_dot_binary": ([vp, vp, C.POINTER(rbq_index), vp, vp, vp], C.c_int),
         "rbq_estimate_scores": ([vp, vp, C.POINTER(rbq_index), vp, vp], C.c_int),
         "rbq_topp_select": ([vp, vp, C.POINTER(rbq_index), f32, vp, vp, vp], C.c_int),
+        "rbq_topp_select_static": ([vp, vp, C.POINTER(rbq_index), f32, vp, vp, vp], C.c_int),
         "rbq_topp_select_alg3": ([vp, vp, C.POINTER(rbq_index), f32, vp, vp, vp, vp], C.c_int),
         "rbq_sparse_attention": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), vp, vp, vp, vp, vp], C.c_int),
         "rbq_decode_step": ([vp, vp, C.POINTER(rbq_kv), C.POINTER(rbq_index), f32, vp, vp, vp, vp], C.c_int),
@@ -185,6 +186,12 @@ def rbq_estimate_scores(ctx, q, idx: rbq_index, scores, stream=None):
 def rbq_topp_select(ctx, scores, idx: rbq_index, p, sel_idx, sel_cnt, stream=None):
     _check(ctx, load().rbq_topp_select(ctx, _ptr(scores), C.byref(idx), float(p), _ptr(sel_idx), _ptr(sel_cnt),
                                        _stream(stream)), "rbq_topp_select")
+
+
+def rbq_topp_select_static(ctx, scores, idx: rbq_index, p, sel_idx, sel_cnt, stream=None):
+    """rbq_topp_select without workspace or allocation: scratch in the library's static 2 MiB device array (rbq.h)."""
+    _check(ctx, load().rbq_topp_select_static(ctx, _ptr(scores), C.byref(idx), float(p), _ptr(sel_idx), _ptr(sel_cnt),
+                                              _stream(stream)), "rbq_topp_select_static")
 
 
 def rbq_topp_select_alg3(ctx, scores, idx: rbq_index, p, sel_idx, sel_cnt, iters=None, stream=None):
@@ -328,6 +335,9 @@ class RaBitQCache:
 
     def topp_select(self, scores, p, sel_idx, sel_cnt, stream=None):
         rbq_topp_select(self.ctx, scores, self.idx, p, sel_idx, sel_cnt, stream)
+
+    def topp_select_static(self, scores, p, sel_idx, sel_cnt, stream=None):
+        rbq_topp_select_static(self.ctx, scores, self.idx, p, sel_idx, sel_cnt, stream)
 
     def topp_select_alg3(self, scores, p, sel_idx, sel_cnt, iters=None, stream=None):
         rbq_topp_select_alg3(self.ctx, scores, self.idx, p, sel_idx, sel_cnt, iters, stream)

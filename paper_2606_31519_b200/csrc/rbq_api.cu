@@ -252,6 +252,16 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
                          (cudaStream_t)stream);
 }
 
+int rbq_topp_select_static(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
+                           void* stream) {
+  RBQ_CTX(ctx);
+  RBQ_TRY(check_idx(ctx, idx, false));                          // no need_ws: this entry point uses no workspace
+  if (!scores || !sel_idx || !sel_cnt) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores/sel_idx/sel_cnt null");
+  if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
+  if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
+  return rbq_launch_topp_static(ctx, scores, idx->n_indexed, p, sel_idx, sel_cnt, (cudaStream_t)stream);
+}
+
 int rbq_topp_select_alg3(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
                          int32_t* iters, void* stream) {
   RBQ_CTX(ctx);

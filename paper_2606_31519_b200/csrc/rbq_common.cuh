@@ -242,6 +242,9 @@ int rbq_launch_estimate(rbq_ctx*, const rbq_index*, float* scores, int32_t* dot,
 // S6 writes the per-row selection bitmap sel_bits [B*Hq][rbq_words_per_row] (always), sel_cnt, and sel_idx if non-NULL.
 // rowmax_key: order-preserving keys of the row maxima [B*Hq] (written by S5), or NULL to compute them here.
 int rbq_topp_init(rbq_ctx* ctx);   // uploads the Top-p kernel's fp64 tables (once per context)
+// S6 on caller-provided scores with its scratch in a static device array (no workspace, no allocation; rbq_topp.cu)
+int rbq_launch_topp_static(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx, int32_t* sel_cnt,
+                           cudaStream_t);
 int rbq_launch_topp(rbq_ctx*, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
                     uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
 // Alg.3 selector (ternary threshold search in fp64): ascending sel_idx, sel_cnt, optional iteration counts [B*Hq].

@@ -820,6 +820,54 @@ int rbq_topp_init(rbq_ctx* ctx) {
   return RBQ_OK;
 }
 
+// ---- rbq_topp_select_static: S6 on caller-provided scores with NO workspace and no allocation ----------------------------
+// The scratch of the stage (the row-maximum keys and the per-row selection bitmaps the kernel always writes) lives in this
+// file-scope device array: 2 MB that every GPU which loads the library holds until exit.  In host code the array's NAME is a
+// host-side stand-in, not a device address: its device address comes from cudaGetSymbolAddress, once per device, with that
+// device current.  Every call shares the array (contents of the last call stay; the keys are cleared per call): calls that
+// overlap on the GPU race.
+constexpr size_t TP_STATIC_WORDS = 512 * 1024;
+static __device__ __align__(256) uint32_t g_tp_static_scratch[TP_STATIC_WORDS];
+constexpr int TP_STATIC_MAX_DEVICES = 64;
+static uint32_t* g_tp_static_addr[TP_STATIC_MAX_DEVICES];       // device address of the array on each device, 0 = not yet asked
+
+int rbq_launch_topp_static(rbq_ctx* ctx, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx,
+                           int32_t* sel_cnt, cudaStream_t s) {
+  const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads, wpr = rbq_words_per_row(ctx);
+  const size_t key_words = ((size_t)rows + 63) & ~size_t(63);   // bitmaps start 256-byte aligned
+  const size_t need = key_words + (size_t)rows * wpr;
+  if (need > TP_STATIC_WORDS)
+    RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED,
+             "rbq_topp_select_static: batch*n_q_heads = %d rows x max_tokens %d need %zu bytes of scratch, the static array holds %zu "
+             "(rows * (max_tokens / 32 + 1) must stay below ~%zu words); use rbq_topp_select with a workspace",
+             rows, ctx->cfg.max_tokens, need * 4, TP_STATIC_WORDS * 4, TP_STATIC_WORDS);
+  int dev = -1;
+  RBQ_CUDA_OK(ctx, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= TP_STATIC_MAX_DEVICES) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "rbq_topp_select_static: device ordinal %d", dev);
+  if (!g_tp_static_addr[dev]) {                                   // set-up, once per device, that device current
+    uint32_t* ptr = nullptr;
+    RBQ_CUDA_OK(ctx, cudaGetSymbolAddress((void**)&ptr, g_tp_static_scratch));
+    if (!ptr) RBQ_FAIL(ctx, RBQ_ERR_CUDA, "rbq_topp_select_static: no device address for the scratch array");
+    g_tp_static_addr[dev] = ptr;
+  }
+  uint32_t* keys = g_tp_static_addr[dev];
+  uint32_t* bits = keys + key_words;
+  const int cs = rbq_topp_cluster_size(ctx);
+  const int s_cap = ((((ctx->cfg.max_tokens + cs - 1) / cs) + 31) & ~31) + 32;
+  if (TP_OFF_SC + (size_t)s_cap * 4 > 227 * 1024 || s_cap > 32 * TP_MAXW)
+    RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "rbq_topp_select_static: max_tokens %d exceeds the cluster-resident limit", ctx->cfg.max_tokens);
+  RBQ_CUDA_OK(ctx, cudaMemsetAsync(keys, 0, (size_t)rows * sizeof(uint32_t), s));   // the maxima are an atomicMax over zeroed keys
+  dim3 grid(max(1, min(32, (ctx->cfg.max_tokens + 4095) / 4096)), rows);
+  rowmax_kernel<<<grid, 256, 0, s>>>(scores, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, keys);
+  RBQ_LAUNCH_OK(ctx);
+  switch (cs) {
+    case 8: return launch_cs<8>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    case 4: return launch_cs<4>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    case 2: return launch_cs<2>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    default: return launch_cs<1>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+  }
+}
+
 int rbq_probe_copy_topp(unsigned long long* host) {
 #ifdef RBQ_PROBE
   if (cudaDeviceSynchronize() != cudaSuccess) return RBQ_ERR_CUDA;
