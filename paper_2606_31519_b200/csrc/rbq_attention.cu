@@ -22,6 +22,18 @@
 
 RBQ_PROBE_DECL(gather_probe);
 RBQ_PROBE_DECL(plan_probe);
+#ifdef RBQ_PROBE
+#define PL_STAMP(slot)                                                                                           \
+  do {                                                                                                           \
+    const unsigned cta_ = blockIdx.y * gridDim.x + blockIdx.x;                                                    \
+    if (threadIdx.x == 0 && cta_ < RBQ_PROBE_CTAS) {                                                              \
+      plan_probe[cta_ * RBQ_PROBE_SLOTS + (slot)] = (unsigned long long)clock64();                                \
+      if ((slot) == 0) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); plan_probe[cta_ * RBQ_PROBE_SLOTS + 15] = gt_; } \
+    }                                                                                                            \
+  } while (0)
+#else
+#define PL_STAMP(slot) do {} while (0)
+#endif
 
 namespace {
 
@@ -59,12 +71,14 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
   __shared__ uint32_t s_pre[PL_THREADS], s_cntb[PL_THREADS];
   __shared__ uint32_t s_base;
   rbq_pdl_trigger();
+  PL_STAMP(0);
   const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   // n_indexed is an input of the step (committed before S3, which starts only when the kernel in front of it has
   // completed): loaded before the wait, one dependent round trip less behind it
   const int nidx = max(0, n_indexed[b]);
   rbq_pdl_wait();                                             // selection bitmaps of S6
+  PL_STAMP(1);
   const int nw = (nidx + 31) >> 5, nblk = (nw + 3) >> 2;
   const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
   uint32_t* __restrict__ out = ulist + (size_t)gi * Lcap;
@@ -95,6 +109,7 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
     s_pre[tid] = s_base + wp + si - c;
     s_cntb[tid] = c;
     __syncthreads();
+    PL_STAMP(2);
     // this warp's blocks: lb = blockIdx.x + PL_SPLIT * (warp + 32 i), i < PL_BPW.  Lane l < 16 prefetches word (l & 3) of head
     // (l >> 2) of each block first (one round of independent loads), then the words are broadcast by shuffles.
     const unsigned lt = (1u << lane) - 1u;
@@ -125,10 +140,12 @@ attn_plan_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ 
         pos += __popc(u);
       }
     }
+    PL_STAMP(3);
     __syncthreads();
     if (tid == 0) s_base += tot;
     __syncthreads();
   }
+  PL_STAMP(4);
   if (blockIdx.x == 0 && tid == 0) { ucount[gi] = (int32_t)s_base; gdone[gi] = 0; }
 }
 
@@ -190,11 +207,14 @@ __device__ __forceinline__ long long ga_row_of(const int* s_start, int ngroups, 
   const long long rows = (long long)s_start[lo + 1] - s_start[lo];
   return s_start[lo] + min(max(off, 0ll), rows);
 }
-// first row of CTA c's range (double arithmetic: exact here, identical in every CTA, far cheaper than a 64-bit division)
+// first row of CTA c's range: floor(vtot * c / nc) in 32-bit integer arithmetic (vtot = q0 nc + r0: q0 c + floor(r0 c / nc),
+// r0 c < nc^2); identical in every CTA.  (fp64 here cost ~1.5 K cycles of dependent DFMAs on the critical path of every
+// CTA, a 64-bit division about as much.)
 __device__ __forceinline__ long long cta_begin(const int* s_start, int ngroups, long long total, int c, int nc) {
   if (c >= nc) return total;
-  const long long vtot = total + (long long)GA_PEN * (ngroups - 1);
-  return ga_row_of(s_start, ngroups, (long long)(((double)vtot * (double)c) / (double)nc));
+  const unsigned vtot = (unsigned)(total + (long long)GA_PEN * (ngroups - 1));       // < 2^31 + 320 * 1024
+  const unsigned q0 = vtot / (unsigned)nc, r0 = vtot - q0 * (unsigned)nc;
+  return ga_row_of(s_start, ngroups, (long long)q0 * c + (long long)((r0 * (unsigned)c) / (unsigned)nc));
 }
 
 // ---- tensor-pipe gather attention (bf16 K/V and q) ----------------------------------------------------------------------
@@ -307,6 +327,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
     const __nv_bfloat16* Vb = V + (long long)b * sb + (long long)g * sh;
     const uint32_t* ul = ulist + (size_t)gi * Lcap;
 
+    if (tid == 0) RBQ_STAMP(gather_probe, 12);
     // A operand: Q rows of the group's heads (rows >= G are zero)
     uint32_t qa[D / 16][2];
     {
@@ -351,7 +372,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 #pragma unroll
     for (int s = 0; s < GA_STAGES - 1; ++s) ent_ring[s] = (s < my_tiles) ? tile_entry(s) : 0u;
     ent_pend = (GA_STAGES - 1 < my_tiles) ? tile_entry(GA_STAGES - 1) : 0u;
-    if (tid == 0) RBQ_STAMP(gather_probe, 11 + (ent_ring[0] == 0xdeadbeefu));
+    if (tid == 0) RBQ_STAMP(gather_probe, 11);
 #pragma unroll
     for (int s = 0; s < GA_STAGES - 1; ++s) {
       if (s < my_tiles) issue(s, ent_ring[s]);

@@ -177,10 +177,12 @@ enum { RBQ_PROBE_ESTIMATE = 0, RBQ_PROBE_TOPP = 1, RBQ_PROBE_GATHER = 2, RBQ_PRO
 #define RBQ_STAMP(buf, slot)                                                                                   \
   do {                                                                                                         \
     if (blockIdx.x < RBQ_PROBE_CTAS) {                                                                         \
-      unsigned long long gt_;                                                                                  \
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_));                                                  \
       (buf)[blockIdx.x * RBQ_PROBE_SLOTS + (slot)] = (unsigned long long)clock64();                            \
-      if ((slot) == 0) (buf)[blockIdx.x * RBQ_PROBE_SLOTS + RBQ_PROBE_SLOTS - 1] = gt_;                        \
+      if ((slot) == 0) {                          /* the global timer only once: reading it is slow */           \
+        unsigned long long gt_;                                                                                \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_));                                                \
+        (buf)[blockIdx.x * RBQ_PROBE_SLOTS + RBQ_PROBE_SLOTS - 1] = gt_;                                       \
+      }                                                                                                        \
     }                                                                                                          \
   } while (0)
 #else
