@@ -225,7 +225,7 @@ int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host);
 /* ---- in-kernel timeline probes (measurement aid; only in the probe build of the library) ------------------------------ */
 /* `python -m paper_2606_31519_b200.build --probe` builds librbq_b200_probe.so with -DRBQ_PROBE: its kernels stamp clock64
  * of chosen points (slot 15: %globaltimer of slot 0) into a device buffer [256 CTAs][16 slots] per kernel.  kernel: 0 =
- * estimator, 1 = Top-p, 2 = gather attention, 3 = union plan.  BLOCKS (device synchronise + copy) and writes 256 * 16
+ * estimator, 1 = Top-p, 2 = gather attention, 3 = union plan, 4 = query preparation.  BLOCKS (device synchronise + copy) and writes 256 * 16
  * uint64 to out_host.  The regular library returns RBQ_ERR_UNSUPPORTED.                                             */
 int rbq_probe_dump(rbq_ctx* ctx, int kernel, uint64_t* out_host);
 

@@ -359,6 +359,7 @@ int rbq_probe_dump(rbq_ctx* ctx, int kernel, uint64_t* out_host) {
     case RBQ_PROBE_TOPP: return rbq_probe_copy_topp(o);
     case RBQ_PROBE_GATHER: return rbq_probe_copy_gather(o);
     case RBQ_PROBE_PLAN: return rbq_probe_copy_plan(o);
+    case RBQ_PROBE_QUERY: return rbq_probe_copy_query(o);
     default: RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "unknown probe kernel %d", kernel);
   }
 }

@@ -171,7 +171,7 @@ __device__ __forceinline__ void rbq_bulk_g2s(uint32_t dst, const void* src, uint
 // buffer [RBQ_PROBE_CTAS][RBQ_PROBE_SLOTS]; rbq_probe_dump(kernel id) copies it out.  Without the flag the macros vanish.
 #define RBQ_PROBE_CTAS 256
 #define RBQ_PROBE_SLOTS 16
-enum { RBQ_PROBE_ESTIMATE = 0, RBQ_PROBE_TOPP = 1, RBQ_PROBE_GATHER = 2, RBQ_PROBE_PLAN = 3, RBQ_PROBE_KERNELS = 4 };
+enum { RBQ_PROBE_ESTIMATE = 0, RBQ_PROBE_TOPP = 1, RBQ_PROBE_GATHER = 2, RBQ_PROBE_PLAN = 3, RBQ_PROBE_QUERY = 4, RBQ_PROBE_KERNELS = 5 };
 #ifdef RBQ_PROBE
 #define RBQ_PROBE_DECL(name) __device__ unsigned long long name[RBQ_PROBE_CTAS * RBQ_PROBE_SLOTS]
 #define RBQ_STAMP(buf, slot)                                                                                   \
@@ -193,6 +193,7 @@ int rbq_probe_copy_estimate(unsigned long long* host);      // defined in the .c
 int rbq_probe_copy_topp(unsigned long long* host);
 int rbq_probe_copy_gather(unsigned long long* host);
 int rbq_probe_copy_plan(unsigned long long* host);
+int rbq_probe_copy_query(unsigned long long* host);
 
 // ---- programmatic dependent launch (PDL) -----------------------------------------------------------
 // The kernels of a decode step are launched with programmatic stream serialisation: a kernel's CTAs may become

@@ -40,11 +40,15 @@ __device__ __forceinline__ void rbq_qprep(const TQ* __restrict__ q, const float*
                                           const float* __restrict__ rot, const float* s_rot, uint32_t p_bar_sa, int rot_kind, int Hq, int Hkv,
                                           const int (&bgs)[NP], const int (&rows0)[NP], float sm_scale, RbqQPrepSmem<D>* sm, int tid, int nt, int bar_id,
                                           RbqQConst* __restrict__ qc_out, uint8_t* __restrict__ qu_out,
-                                          float* __restrict__ qparams, TQ* __restrict__ q_copy) {
+                                          float* __restrict__ qparams, TQ* __restrict__ q_copy, int h_off = 0, int G_out = 0) {
+  // Single-head mode (h_off, G_out given; the caller passes Hq == Hkv, so that G == 1 in here, and rows0[p] = the head's
+  // own row): the caller works on head h_off of a group of G_out heads and writes only that head's share of qc_out[p] -- its
+  // constants, its column of the B-operand fragments with the ones-column beside it, and (h_off == 0) the unused columns.
   constexpr int W = D / 32;
   // G = Hq / Hkv is 1, 2 or 4 (rbq_create): every index split below is a shift or a mask, no integer division
   const int gsh = (Hq >= 4 * Hkv) ? 2 : (Hq >= 2 * Hkv) ? 1 : 0, G = 1 << gsh;
   constexpr int dsh = (D == 64) ? 6 : (D == 128) ? 7 : 8, wsh = dsh - 5;
+  if (G_out == 0) G_out = G;                                      // all heads of the group in this call
   const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
   auto row0 = [&](int p) { return (size_t)rows0[p]; };             // first query head row (b * Hq + kv head * G) of pair p
   auto sync = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nt) : "memory"); };
@@ -106,6 +110,24 @@ __device__ __forceinline__ void rbq_qprep(const TQ* __restrict__ q, const float*
     // read per head is bound by shared-memory bandwidth; all four heads per thread by the issue rate of four lone warps;
     // broadcasting u_i by shuffles instead of 16-byte shared-memory loads was slower still: measured 3.3 K / 3.3 K / 5.7 K clk)
     const int psh = (G > 2) ? 1 : 0, npair = 1 << psh;           // head pairs per KV head: 1 (G = 1, 2) or 2 (G = 4)
+    if (G == 1) {
+      // one head per pair (single-head mode, or G = 1): one canonical chain per thread; per step one read of P[i][j] and one
+      // broadcast of u_i
+      for (int it = tid; it < NP * D; it += nt) {
+        const int p = it >> dsh, jj = it & (D - 1);
+        float a0 = 0.0f;
+#pragma unroll 2
+        for (int i0 = 0; i0 < D; i0 += 8) {
+          float rv[8];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) rv[k] = P_SMEM ? s_rot[(i0 + k) * D + jj] : __ldg(rot + (size_t)(i0 + k) * D + jj);
+          const float4 xa = *reinterpret_cast<const float4*>(&sm[p].x[0][i0]), xb = *reinterpret_cast<const float4*>(&sm[p].x[0][i0 + 4]);
+          a0 = fmaf(xa.x, rv[0], a0); a0 = fmaf(xa.y, rv[1], a0); a0 = fmaf(xa.z, rv[2], a0); a0 = fmaf(xa.w, rv[3], a0);
+          a0 = fmaf(xb.x, rv[4], a0); a0 = fmaf(xb.y, rv[5], a0); a0 = fmaf(xb.z, rv[6], a0); a0 = fmaf(xb.w, rv[7], a0);
+        }
+        sm[p].y[0][jj] = a0;
+      }
+    } else
     for (int it = tid; it < NP * npair * D; it += nt) {
       const int p = it >> (dsh + psh), hp = ((it >> dsh) & (npair - 1)) * 2, jj = it & (D - 1), h1 = min(hp + 1, G - 1);
       float a0 = 0.0f, a1 = 0.0f;
@@ -214,26 +236,29 @@ __device__ __forceinline__ void rbq_qprep(const TQ* __restrict__ q, const float*
       float* o = qparams + (row0(p) + h) * 6;
       o[0] = qn; o[1] = ql; o[2] = delta; o[3] = (float)sumq; o[4] = q_ck; o[5] = cq_ck;
     }
-    qc_out[p].cA[h] = (float)((double)sm_scale * (double)qn * (double)delta * 0.25);
-    qc_out[p].cB[h] = (float)((double)sm_scale * (double)qn * (double)ql * 0.25);
-    qc_out[p].cD[h] = (float)((double)sm_scale * ((double)q_ck - (double)cq_ck));
-    qc_out[p].init_d[h] = 0x4B400000 - 4 * sumq;
-    if (h == 0) qc_out[p].init_p = 0x4B400000 - 4 * D;
+    const int ho = h + h_off;
+    qc_out[p].cA[ho] = (float)((double)sm_scale * (double)qn * (double)delta * 0.25);
+    qc_out[p].cB[ho] = (float)((double)sm_scale * (double)qn * (double)ql * 0.25);
+    qc_out[p].cD[ho] = (float)((double)sm_scale * ((double)q_ck - (double)cq_ck));
+    qc_out[p].init_d[ho] = 0x4B400000 - 4 * sumq;
+    if (ho == 0) qc_out[p].init_p = 0x4B400000 - 4 * D;
   }
   RBQ_QPREP_STAMP(14);
   // B-operand fragments (rbq_bfrag_dim): word (s, lane', r), byte i; column n = lane' >> 2: even -> head n/2, odd -> ones
   for (int w0 = tid; w0 < NP * W * 64; w0 += nt) {
     const int p = w0 >> (wsh + 6), w = w0 & (W * 64 - 1);
     const int s = w >> 6, ln = (w >> 1) & 31, r = w & 1;
-    const int gp = ln >> 2, tp = ln & 3;
+    const int gp = ln >> 2, tp = ln & 3, hc = gp >> 1;             // hc: the head this column (or its ones-column) belongs to
+    const bool mine = (hc >= h_off && hc < h_off + G) || (h_off == 0 && hc >= G_out);
+    if (!mine) continue;
     uint32_t word = 0;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       int dim, sh;
       rbq_bfrag_dim(W, s, tp, r, i, dim, sh);
       uint32_t val = 0;
-      if (gp & 1) val = ((gp >> 1) < G) ? 1u : 0u;
-      else if ((gp >> 1) < G) val = sm[p].qu[gp >> 1][dim];
+      if (gp & 1) val = (hc < G_out) ? 1u : 0u;
+      else if (hc < G_out) val = sm[p].qu[hc - h_off][dim];
       word |= (val << sh) << (8 * i);
     }
     qc_out[p].bfrag[s][ln][r] = word;
