@@ -1,6 +1,7 @@
 // rbq_api.cu -- host side of the C ABI declared in include/rbq.h: argument checks, workspace
 // carve-up, stream/event ordering of the lazy flush.  Every entry point only enqueues kernels.
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 
 #include "rbq_common.cuh"
@@ -22,6 +23,9 @@ void layout_workspace(rbq_ctx* c) {
   c->off_ulist = take(B * Hkv * L * sizeof(uint32_t));
   c->off_ucount = take(B * Hkv * sizeof(int32_t));
   c->off_gdone = take(B * Hkv * sizeof(int32_t));
+  c->off_gnext = take(B * Hkv * sizeof(int32_t));
+  c->off_ucnt = take(B * Hkv * RBQ_UNION_SLICES * sizeof(uint32_t));
+  c->off_garrive = take(B * Hkv * RBQ_UNION_SLICES * sizeof(int32_t));
   c->off_rowmax = take(rows * sizeof(uint32_t));
   c->off_part = take(rbq_attention_part_bytes(c));
   const size_t D = g.head_dim;
@@ -99,6 +103,7 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
   c->G = G;
   c->sm_scale = cfg->sm_scale > 0.0f ? cfg->sm_scale : (float)(1.0 / sqrt((double)cfg->head_dim));
   c->sm_count = sms;
+  { const char* e = getenv("RBQ_GATHER_PLAN"); c->gather_via_plan = (e && e[0] == '1') ? 1 : 0; }
   if (cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_flush, cudaEventDisableTiming) != cudaSuccess) {
     delete c;
@@ -147,6 +152,10 @@ int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes) {
   RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_flags, 0, sizeof(uint32_t)));
   // row-maximum keys: zero between decode steps (S5 accumulates with atomicMax, S6 clears after reading)
   RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_rowmax, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads * sizeof(uint32_t)));
+  // per-group arrival and chunk counters of S7: zero between steps (the last CTA to finish a group clears them)
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_gdone, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(int32_t)));
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_gnext, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(int32_t)));
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_garrive, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * RBQ_UNION_SLICES * sizeof(int32_t)));
   return RBQ_OK;
 }
 
@@ -249,7 +258,7 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
   if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
   return rbq_launch_topp(ctx, scores, nullptr, idx->n_indexed, p, ws_ptr<uint32_t>(ctx, ctx->off_selbits), sel_idx, sel_cnt,
-                         (cudaStream_t)stream);
+                         nullptr, nullptr, (cudaStream_t)stream);
 }
 
 int rbq_topp_select_static(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
@@ -280,7 +289,7 @@ int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const
   if (!q || !sel_idx || !sel_cnt || !out) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/sel_idx/sel_cnt/out null");
   uint32_t* bits = ws_ptr<uint32_t>(ctx, ctx->off_selbits);
   RBQ_TRY(rbq_launch_bits_from_lists(ctx, idx, sel_idx, sel_cnt, bits, (cudaStream_t)stream));
-  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, out, lse, (cudaStream_t)stream);
+  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, 0, out, lse, (cudaStream_t)stream);
 }
 
 // q_copy != NULL: q is readable by the device but far away (mapped host memory): S3 reads it once and leaves a device copy
@@ -306,9 +315,10 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, rowmax, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, ws_ptr<uint32_t>(ctx, ctx->off_ucnt),
+                          ws_ptr<int32_t>(ctx, ctx->off_garrive), s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
-  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, out, nullptr, s);   // records ev[4] after the plan
+  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, rbq_topp_cluster_size(ctx), out, nullptr, s);   // records ev[4] after the plan
   ctx->stage_ev = nullptr;
   if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[RBQ_N_STAGES], s));
   return rc;

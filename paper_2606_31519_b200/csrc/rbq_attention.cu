@@ -49,6 +49,33 @@ __global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, cons
   }
 }
 
+// union size of each KV group's G bitmaps, in RBQ_UNION_SLICES equal word ranges (what S6 leaves in a fused step);
+// grid = (RBQ_UNION_SLICES, B*Hkv), 256 threads
+__global__ void union_count_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, int Hq, int Hkv, int wpr,
+                                   uint32_t* __restrict__ ucnt) {
+  __shared__ uint32_t s_w[8];
+  const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
+  const int nw = (max(0, n_indexed[b]) + 31) >> 5;
+  const int wps = (nw + RBQ_UNION_SLICES - 1) / RBQ_UNION_SLICES;
+  const int w0 = blockIdx.x * wps, w1 = min(nw, w0 + wps);
+  const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
+  uint32_t c = 0;
+  for (int w = w0 + threadIdx.x; w < w1; w += blockDim.x) {
+    uint32_t u = 0;
+    for (int h = 0; h < G; ++h) u |= rows0[(size_t)h * wpr + w];
+    c += __popc(u);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t tot = 0;
+    for (int w = 0; w < 8; ++w) tot += s_w[w];
+    ucnt[(size_t)gi * RBQ_UNION_SLICES + blockIdx.x] = tot;
+  }
+}
+
 // ---- plan: union list per KV group ---------------------------------------------------------------------------------
 constexpr int PL_THREADS = 1024;
 constexpr int PL_MAX_SPLIT = 16;
@@ -587,6 +614,513 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
   }
 }
 
+// ---- gather attention straight from the selection bitmaps (no plan kernel, no union list in global memory) ----------------
+// The union of a KV group's G selection bitmaps is expanded where it is consumed.  Work unit: a warp chunk of GB_CHUNK = 128
+// tokens of one group (4 bitmap words per head; pending-window rows form extra chunks behind the bitmap chunks).  A warp
+// expands a chunk into its private ring of entries (token | head mask << 28) in shared memory, its cp.async pipeline takes
+// 16-entry tiles from the ring and runs on across chunk boundaries.
+//   * across groups the CTAs are placed by an ESTIMATE of every group's union size, computed by every CTA from the per-row
+//     selection counts S6 leaves (independent heads: n (1 - prod_h (1 - cnt_h / n)), clamped to [max_h cnt_h, min(n, sum_h cnt_h)])
+//     + the pending rows: equal contiguous ranges of the concatenated estimates, one per CTA, exactly as the union lists were
+//     cut before -- but a wrong estimate costs balance only, never correctness;
+//   * inside a group the chunks are handed out dynamically (one atomicAdd per chunk on the group's counter, claimed one chunk
+//     ahead so that its latency and that of the bitmap words hide behind the tiles in flight); the first chunk of every warp
+//     of the CTAs that START in the group is static, so no atomic sits in front of the first tile;
+//   * every CTA whose range touches a group arrives at it (possibly with an empty partial); the last one merges and resets
+//     the group's counters for the next step.
+constexpr int GB_CW = 8;                                     // bitmap words (32 tokens each) per claim at most: one word per lane and head
+constexpr int GB_CW0 = 4;                                    // words of a warp's static first claim
+constexpr int GB_RING = 512;                                 // entries per warp ring (>= 15 left over + one claim)
+#ifndef RBQ_GB_TOKDIV
+#define RBQ_GB_TOKDIV 14                                     // cost of a group = union rows + tokens / RBQ_GB_TOKDIV (scan + sparse-row penalty)
+#endif
+#ifndef RBQ_GB_SNAP
+#define RBQ_GB_SNAP 6                                        // CTA boundaries snap to boundaries between groups worth >= this many CTAs each
+#endif
+
+// s_start[gi] = sum over groups < gi of the attended rows (union of the group's selections + pending rows); every CTA
+// computes the same table from the per-slice union sizes S6 (or union_count_kernel) left in ucnt.
+__device__ void build_union_table(const uint32_t* __restrict__ ucnt, int n_slices, const int32_t* __restrict__ n_indexed,
+                                  const int32_t* __restrict__ n_total, int ngroups, int Hkv, int* s_start, int* s_warp,
+                                  int nthreads, int* s_nidx, int* s_npend) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  const int per = (ngroups + nthreads - 1) / nthreads;
+  const int g0 = tid * per;
+  int local = 0;
+  for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
+    const int b = gi / Hkv;
+    const int ni = max(0, n_indexed[b]), np = max(0, n_total[b] - ni);
+    uint32_t u = 0;
+    if (ni > 0) {                                             // S6 writes nothing for an empty index
+      const uint4 a = __ldcg(reinterpret_cast<const uint4*>(ucnt + (size_t)gi * RBQ_UNION_SLICES));
+      const uint4 c = __ldcg(reinterpret_cast<const uint4*>(ucnt + (size_t)gi * RBQ_UNION_SLICES + 4));
+      const uint32_t v[8] = {a.x, a.y, a.z, a.w, c.x, c.y, c.z, c.w};
+#pragma unroll
+      for (int r = 0; r < RBQ_UNION_SLICES; ++r) u += (r < n_slices) ? v[r] : 0u;
+    }
+    const int est = (int)min(u, (uint32_t)ni);
+    const int cost = (est + np > 0) ? est + np + ni / RBQ_GB_TOKDIV : 0;   // rows + what scanning the bitmaps of ni tokens costs
+    s_nidx[gi] = ni;
+    s_npend[gi] = np;
+    s_start[gi] = cost;                                       // the group's own cost for now, its prefix below
+    local += cost;
+  }
+  int incl = local;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  int woff = 0, total = 0;
+  for (int w = 0; w < nwarps; ++w) { if (w < warp) woff += s_warp[w]; total += s_warp[w]; }
+  int run = woff + incl - local;
+  for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
+    const int v = s_start[gi];
+    s_start[gi] = run;
+    run += v;
+  }
+  if (tid == 0) s_start[ngroups] = total;
+  __syncthreads();
+}
+
+// first estimated row of CTA c of nce (total >= nce >= 1): floor(total * c / nce), strictly increasing in c
+__device__ __forceinline__ int gb_begin(unsigned total, int c, int nce) {
+  if (c >= nce) return (int)total;
+  const unsigned q0 = total / (unsigned)nce, r0 = total - q0 * (unsigned)nce;
+  return (int)(q0 * (unsigned)c + (r0 * (unsigned)c) / (unsigned)nce);
+}
+
+// CTA boundaries in the cost space, snapped: s_bound[c] = floor(total c / nce), and the boundary nearest to the border
+// between two groups worth >= RBQ_GB_SNAP CTA shares each moves onto that border if it is less than half a share away, so
+// that large groups get whole CTAs (a CTA that straddles two groups pays a second prologue and merge at the very end of the
+// kernel; inside a group the work is shared dynamically anyway, so the price is an imbalance of at most half a CTA in
+// RBQ_GB_SNAP).  Strictly increasing in c (two boundaries a share apart cannot both be closer than half a share to one
+// border); identical in every CTA.
+__device__ void build_bounds(const int* s_start, int ngroups, unsigned total, int nce, int* s_bound, int nthreads) {
+  const int tid = threadIdx.x;
+  for (int c = tid; c <= nce; c += nthreads) s_bound[c] = gb_begin(total, c, nce);
+  __syncthreads();
+  const int share = (int)(total / (unsigned)nce);
+  const float c_per_cost = (float)nce / (float)total;
+  for (int k = 1 + tid; k < ngroups; k += nthreads) {
+    const int bnd = s_start[k];
+    const long long big = (long long)RBQ_GB_SNAP * share;
+    if ((long long)bnd - s_start[k - 1] < big || (long long)s_start[k + 1] - bnd < big) continue;
+    int c = (int)((float)bnd * c_per_cost + 0.5f);             // nearest boundary, up to rounding: look at its neighbours too
+    c = min(max(c, 1), nce - 1);
+    int best = -1, bd = 0x7fffffff;
+    for (int cc = max(1, c - 1); cc <= min(nce - 1, c + 1); ++cc) {
+      const int x = gb_begin(total, cc, nce), dist = x > bnd ? x - bnd : bnd - x;
+      if (dist < bd) { bd = dist; best = cc; }
+    }
+    if (best > 0 && 2 * bd < share) s_bound[best] = bnd;
+  }
+  __syncthreads();
+}
+
+// grid = number of SMs (persistent), GA_THREADS threads, GaCfg<D>::SMEM dynamic shared memory.
+// part: [gridDim.x + ngroups][G][GA_PART]; the partial of (CTA c, group gi) lives in slot c + gi.
+// gnext / gdone: [ngroups], zero on entry, zero again on exit.
+template <int D>
+__global__ void __launch_bounds__(GA_THREADS, 1)
+attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ K, const __nv_bfloat16* __restrict__ V,
+                        long long sb, long long sh, long long st, const uint32_t* __restrict__ bits, int wpr,
+                        const uint32_t* __restrict__ ucnt, int n_slices, const int32_t* __restrict__ n_indexed,
+                        const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, float scale_log2,
+                        float* __restrict__ part, int32_t* __restrict__ gdone, int32_t* __restrict__ gnext,
+                        void* __restrict__ out, int out_bf16, float* __restrict__ lse) {
+  using C = GaCfg<D>;
+  constexpr int GA_TILE_BYTES = C::TILE_BYTES, GA_STAGE_BYTES = C::STAGE_BYTES, GA_PART = C::PART, RB = C::ROW_BYTES, CPR = C::CPR;
+  constexpr int LSH = (D == 64) ? 3 : 4;                       // log2(CPR)
+  extern __shared__ __align__(128) unsigned char ga_smem[];
+  __shared__ int s_start[AT_MAX_GROUPS + 1], s_nidx[AT_MAX_GROUPS], s_npend[AT_MAX_GROUPS];
+  __shared__ uint32_t s_ring[GA_WARPS][GB_RING];
+  __shared__ int s_bound[GA_THREADS + 1];                     // snapped CTA boundaries in the cost space
+  __shared__ int s_warp[GA_WARPS];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g4 = lane >> 2, t4 = lane & 3;                    // MMA fragment coordinates
+  const int G = Hq / Hkv;
+  if (tid == 0) RBQ_STAMP(gather_probe, 0);
+#ifdef RBQ_PROBE
+  if (tid == 0 && blockIdx.x < RBQ_PROBE_CTAS) { gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 13] = 0; gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 14] = 0; }
+  __syncthreads();
+#endif
+  rbq_pdl_wait();                                             // selection bitmaps and counts of S6
+  if (tid == 0) RBQ_STAMP(gather_probe, 1);
+
+  build_union_table(ucnt, n_slices, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS, s_nidx, s_npend);
+  if (tid == 0) RBQ_STAMP(gather_probe, 2);
+  const unsigned total = (unsigned)s_start[ngroups];
+  if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
+    for (int gq = 0; gq < ngroups; ++gq) {
+      if (s_start[gq + 1] != s_start[gq]) continue;
+      for (int hd = tid; hd < G * D; hd += GA_THREADS) {
+        const size_t orow = (size_t)(gq / Hkv) * Hq + (size_t)(gq % Hkv) * G + hd / D;
+        if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * D + hd % D] = __float2bfloat16_rn(0.0f);
+        else reinterpret_cast<float*>(out)[orow * D + hd % D] = 0.0f;
+        if (lse && hd % D == 0) lse[orow] = -INFINITY;
+      }
+    }
+  }
+  const int nce = (int)min((unsigned)gridDim.x, total);       // CTAs with a non-empty range
+  if ((int)blockIdx.x >= nce) return;
+  build_bounds(s_start, ngroups, total, nce, s_bound, GA_THREADS);
+  const float c_per_cost = (float)nce / (float)total;
+  const int r0 = s_bound[blockIdx.x], r1 = s_bound[blockIdx.x + 1];
+  if (r0 >= r1) return;
+  int gi = 0;                                                 // first group with s_start[gi + 1] > r0
+  {
+    int lo = 0, hi = ngroups - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (s_start[mid + 1] > r0) hi = mid; else lo = mid + 1;
+    }
+    gi = lo;
+  }
+  if (tid == 0) RBQ_STAMP(gather_probe, 9);
+  unsigned char* my_smem = ga_smem + (size_t)warp * GA_STAGES * GA_STAGE_BYTES;
+  const uint32_t my_base = smem_u32(my_smem);
+  uint32_t* ring = s_ring[warp];
+  const unsigned lt = (1u << lane) - 1u;
+
+  for (; gi < ngroups && s_start[gi] < r1; ++gi) {
+    const int ga = s_start[gi], gb = s_start[gi + 1];
+    if (ga >= gb) continue;
+    const int b = gi / Hkv, g = gi % Hkv;
+    const int nidx = s_nidx[gi], npend = s_npend[gi];
+    // CTAs whose range touches [ga, gb): clo = last c with s_bound[c] <= ga, chi = last c with s_bound[c] < gb (the bounds are
+    // strictly increasing and within half a share of total c / nce: a guess and a short walk)
+    int clo = min(max((int)((float)ga * c_per_cost), 0), nce - 1);
+    while (clo < nce - 1 && s_bound[clo + 1] <= ga) ++clo;
+    while (clo > 0 && s_bound[clo] > ga) --clo;
+    int chi = min(max((int)((float)gb * c_per_cost), 0), nce - 1);
+    while (chi < nce - 1 && s_bound[chi + 1] < gb) ++chi;
+    while (chi > 0 && s_bound[chi] >= gb) --chi;
+    const int cfl = (s_bound[clo] >= ga) ? clo : clo + 1;
+    const int nw = (nidx + 31) >> 5;                           // bitmap words; pending rows follow as words of 32 rows
+    const int nwt = nw + ((npend + 31) >> 5);
+    const int nwg = max(1, chi - clo + 1) * GA_WARPS;          // warps that share the group
+    const int dyn_base = max(0, chi - cfl + 1) * GA_WARPS * GB_CW0;   // words below it are the static first claims
+    // words per claim: ~64 attended rows while plenty is left, down to one word at the end of the group
+    const int cw_max = min(GB_CW, max(GB_CW0, (int)(2.0f * (float)max(nidx, 1) / (float)max(gb - ga, 1))));
+    const __nv_bfloat16* Kb = K + (long long)b * sb + (long long)g * sh;
+    const __nv_bfloat16* Vb = V + (long long)b * sb + (long long)g * sh;
+    // lane l loads word (l & 7) of head (l >> 3) of a claim
+    const uint32_t* wsrc = bits + ((size_t)b * Hq + (size_t)g * G + min(lane >> 3, G - 1)) * wpr + (lane & 7);
+    const bool wlane = (lane >> 3) < G;
+    int32_t* cnt_ptr = gnext + gi;
+
+    if (tid == 0) RBQ_STAMP(gather_probe, 12);
+    // claim stream of this warp: [w_a, w_a + n_a) = words to expand next (bitmap words in pre_a); raw_b / n_b = the claim after
+    int w_a, n_a, raw_b = 0, n_b = 0;
+    uint32_t pre_a = 0u;
+    auto load_words = [&](int w0, int n) -> uint32_t {
+      return (wlane && (lane & 7) < n && w0 + (lane & 7) < nw) ? __ldcg(wsrc + w0) : 0u;
+    };
+    auto claim_size = [&](int from) -> int {                  // guided: half of an even share of what is left, 1 .. cw_max words
+      return max(1, min(cw_max, (nwt - from) / (2 * nwg)));
+    };
+    if ((int)blockIdx.x >= cfl) {
+      w_a = (((int)blockIdx.x - cfl) * GA_WARPS + warp) * GB_CW0;
+      n_a = GB_CW0;
+    } else {                                                   // second or later group of this CTA: every claim dynamic
+      n_a = cw_max;
+      int v = 0;
+      if (lane == 0) v = atomicAdd(cnt_ptr, n_a);
+      w_a = dyn_base + __shfl_sync(0xffffffffu, v, 0);
+    }
+    n_a = max(0, min(n_a, nwt - w_a));
+    if (n_a > 0) {
+      pre_a = load_words(w_a, n_a);
+      n_b = claim_size(w_a);
+      if (lane == 0) raw_b = atomicAdd(cnt_ptr, n_b);
+    }
+    // A operand: Q rows of the group's heads (rows >= G are zero)
+    uint32_t qa[D / 16][2];
+    {
+      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * D);
+#pragma unroll
+      for (int ks = 0; ks < D / 16; ++ks) {
+        qa[ks][0] = (g4 < G) ? qp[8 * ks + t4] : 0u;
+        qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
+      }
+    }
+    if (tid == 0) RBQ_STAMP(gather_probe, 10);
+    float m_run = -INFINITY, l_run = 0.0f;
+    float o[D / 8][4];
+#pragma unroll
+    for (int nt = 0; nt < D / 8; ++nt) { o[nt][0] = 0.0f; o[nt][1] = 0.0f; o[nt][2] = 0.0f; o[nt][3] = 0.0f; }
+
+    int head = 0, tail = 0;                                    // ring positions (monotone; slot = position & (GB_RING - 1))
+    // expand claims until a whole tile is available or the group's words are exhausted
+    auto fill = [&]() {
+      while (tail - head < GA_TILE && n_a > 0) {
+        for (int k = 0; k < n_a; ++k) {
+          const int w = w_a + k;
+          if (w < nw) {
+            uint32_t u = 0u, mask = 0u;
+#pragma unroll
+            for (int h = 0; h < RBQ_MAX_G; ++h) {
+              const uint32_t hwv = __shfl_sync(0xffffffffu, pre_a, 8 * h + k);
+              u |= hwv;
+              mask |= ((hwv >> lane) & 1u) << h;
+            }
+            if ((u >> lane) & 1u) ring[(tail + __popc(u & lt)) & (GB_RING - 1)] = (uint32_t)(w * 32 + lane) | (mask << 28);
+            tail += __popc(u);
+          } else {                                             // pending-window rows: attended by every head
+            const int pr = (w - nw) * 32 + lane, pc = min(32, npend - (w - nw) * 32);
+            if (lane < pc) ring[(tail + lane) & (GB_RING - 1)] = (uint32_t)(nidx + pr) | (0xFu << 28);
+            tail += pc;
+          }
+        }
+        w_a = dyn_base + __shfl_sync(0xffffffffu, raw_b, 0);   // claimed one claim ago
+        n_a = max(0, min(n_b, nwt - w_a));
+        if (n_a > 0) {
+          pre_a = load_words(w_a, n_a);
+          n_b = claim_size(w_a);
+          if (lane == 0) raw_b = atomicAdd(cnt_ptr, n_b);
+        }
+        __syncwarp();
+      }
+    };
+    auto issue = [&](int i, uint32_t ent) {
+      const uint32_t sbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES);
+#pragma unroll
+      for (int k = 0; k < GA_TILE * CPR / 32; ++k) {           // 32 lanes cover 32 / CPR rows per step
+        const int row = (32 / CPR) * k + (lane >> LSH), ch = lane & (CPR - 1);
+        const uint32_t re = __shfl_sync(0xffffffffu, ent, row);
+        const long long off = (long long)(re & 0x0FFFFFFFu) * st + ch * 8;
+        const uint32_t d = sbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4));
+        cp_async16(d, Kb + off);
+        cp_async16(d + GA_TILE_BYTES, Vb + off);
+      }
+    };
+    uint32_t ent_ring[GA_STAGES - 1];
+#pragma unroll
+    for (int s = 0; s < GA_STAGES - 1; ++s) ent_ring[s] = 0u;
+    int issued = 0;
+    for (int i = -(GA_STAGES - 1);; ++i) {
+      fill();
+      const int avail = tail - head;                           // >= GA_TILE, or what is left of an exhausted group
+      uint32_t ent_new = 0u;
+      if (avail > 0) {
+        if (lane < GA_TILE && lane < avail) ent_new = ring[(head + lane) & (GB_RING - 1)];
+        head += min(GA_TILE, avail);
+        issue(issued, ent_new);
+        ++issued;
+      }
+      cp_async_commit();
+      const uint32_t ent = ent_ring[0];
+#pragma unroll
+      for (int s = 0; s + 1 < GA_STAGES - 1; ++s) ent_ring[s] = ent_ring[s + 1];
+      ent_ring[GA_STAGES - 2] = ent_new;
+      if (i < 0) continue;
+      if (i >= issued) break;
+      cp_async_wait<GA_STAGES - 1>();
+      __syncwarp();
+      if (tid == 0 && i == 0) RBQ_STAMP(gather_probe, 4);
+      const uint32_t kbase = my_base + (uint32_t)((i % GA_STAGES) * GA_STAGE_BYTES), vbase = kbase + GA_TILE_BYTES;
+
+      // S = Q K^T : two n-tiles of 8 tokens
+      float s[2][4];
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        s[nt][0] = 0.0f; s[nt][1] = 0.0f; s[nt][2] = 0.0f; s[nt][3] = 0.0f;
+        const int row = nt * 8 + (lane & 7);
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) {
+          uint32_t bf[4];
+          const int ch = 4 * j + (lane >> 3);
+          ldsm_x4(bf, kbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4)));
+          mma_bf16(s[nt], qa[2 * j][0], 0u, qa[2 * j][1], 0u, bf[0], bf[1]);
+          mma_bf16(s[nt], qa[2 * j + 1][0], 0u, qa[2 * j + 1][1], 0u, bf[2], bf[3]);
+        }
+      }
+      // head masks, online softmax (row = head g4; this lane: tokens nt*8 + 2*t4, +1)
+      float tmax = -INFINITY;
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        const uint32_t e0 = __shfl_sync(0xffffffffu, ent, nt * 8 + 2 * t4);
+        const uint32_t e1 = __shfl_sync(0xffffffffu, ent, nt * 8 + 2 * t4 + 1);
+        const bool ok0 = (e0 >> (28 + (g4 & 3))) & 1u, ok1 = (e1 >> (28 + (g4 & 3))) & 1u;
+        s[nt][0] = (ok0 && g4 < G) ? s[nt][0] * scale_log2 : -INFINITY;
+        s[nt][1] = (ok1 && g4 < G) ? s[nt][1] * scale_log2 : -INFINITY;
+        tmax = fmaxf(tmax, fmaxf(s[nt][0], s[nt][1]));
+      }
+      tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+      tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+      const float m_new = fmaxf(m_run, tmax);
+      const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+      const float resc = exp2f(m_run - m_use);                 // m_run = -inf -> 0
+      m_run = m_new;
+      const float p00 = exp2f(s[0][0] - m_use), p01 = exp2f(s[0][1] - m_use);
+      const float p10 = exp2f(s[1][0] - m_use), p11 = exp2f(s[1][1] - m_use);
+      l_run = l_run * resc + ((p00 + p01) + (p10 + p11));
+      // P as bf16 hi + lo parts (two MMAs per V tile): keeps ~16 mantissa bits of the probabilities
+      const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+      const uint32_t pb0 = pack_bf16(p00 - rbq_bf16lo(pa0), p01 - rbq_bf16hi(pa0));
+      const uint32_t pb2 = pack_bf16(p10 - rbq_bf16lo(pa2), p11 - rbq_bf16hi(pa2));
+      // O = O * resc + P V
+#pragma unroll
+      for (int c2 = 0; c2 < D / 16; ++c2) {
+        uint32_t bf[4];
+        const int row = (lane & 7) + ((lane >> 3) & 1) * 8, ch = 2 * c2 + (lane >> 4);
+        ldsm_x4_t(bf, vbase + (uint32_t)(row * RB + ((ch ^ (row & 7)) << 4)));
+        o[2 * c2][0] *= resc; o[2 * c2][1] *= resc;
+        o[2 * c2 + 1][0] *= resc; o[2 * c2 + 1][1] *= resc;
+        mma_bf16(o[2 * c2], pa0, 0u, pa2, 0u, bf[0], bf[1]);
+        mma_bf16(o[2 * c2 + 1], pa0, 0u, pa2, 0u, bf[2], bf[3]);
+        mma_bf16(o[2 * c2], pb0, 0u, pb2, 0u, bf[0], bf[1]);
+        mma_bf16(o[2 * c2 + 1], pb0, 0u, pb2, 0u, bf[2], bf[3]);
+      }
+      __syncwarp();                                            // tile consumed before its stage is refilled
+    }
+    cp_async_wait<0>();
+    rbq_pdl_trigger();                                        // dependents (the next step's S3) may become resident under the merge phase
+    if (tid == 0) RBQ_STAMP(gather_probe, 5);
+#ifdef RBQ_PROBE
+    if (lane == 0 && blockIdx.x < RBQ_PROBE_CTAS) {
+      atomicAdd(&gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 14], (unsigned long long)issued);
+      if (warp == 0) { atomicAdd(&gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 13], 1ull << 32); atomicMax(&gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 13], (unsigned long long)gi | (gather_probe[blockIdx.x * RBQ_PROBE_SLOTS + 13] & ~0xFFFFull)); }
+    }
+#endif
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
+
+    // merge the warps of the CTA (staging area aliases the drained pipeline buffers)
+    __syncthreads();
+    float* stg = reinterpret_cast<float*>(ga_smem);            // [GA_WARPS][G][GA_PART]
+    if (g4 < G) {
+      float* dst = stg + ((size_t)warp * G + g4) * GA_PART;
+#pragma unroll
+      for (int nt = 0; nt < D / 8; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
+      if (t4 == 0) { dst[D] = m_run; dst[D + 1] = l_run; }
+    }
+    __syncthreads();
+    float* pdst = part + (size_t)(blockIdx.x + gi) * G * GA_PART;
+    for (int idx = tid; idx < G * D; idx += GA_THREADS) {
+      const int h = idx / D, d = idx % D;
+      float mm = -INFINITY;
+#pragma unroll
+      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[((size_t)w * G + h) * GA_PART + D]);
+      float oo = 0.0f, ll = 0.0f;
+#pragma unroll
+      for (int w = 0; w < GA_WARPS; ++w) {
+        const float* sp = stg + ((size_t)w * G + h) * GA_PART;
+        const float f = (sp[D] == -INFINITY) ? 0.0f : exp2f(sp[D] - mm);
+        oo = fmaf(f, sp[d], oo);
+        ll = fmaf(f, sp[D + 1], ll);
+      }
+      pdst[(size_t)h * GA_PART + d] = oo;
+      if (d == 0) { pdst[(size_t)h * GA_PART + D] = mm; pdst[(size_t)h * GA_PART + D + 1] = ll; }
+    }
+    // ---- arrival: the last CTA that finishes a group merges the group's partials into out / lse -------------------------
+    if (tid == 0) RBQ_STAMP(gather_probe, 6);
+    __threadfence();
+    const bool touches = tid >= clo && tid <= chi;
+    const int expected = chi - clo + 1;
+    __syncthreads();                                           // staging area free, partial stores fenced
+    if (tid == 0) s_last = (atomicAdd(&gdone[gi], 1) == expected - 1);
+    __syncthreads();
+    if (tid == 0) RBQ_STAMP(gather_probe, 7);
+    if (s_last) {
+      __threadfence();
+      float* s_f = stg;                                        // [G][GA_THREADS]: factor 2^(m - max) of slot c
+      constexpr int TPH = D / 4, ITEMS = RBQ_MAX_G * TPH;     // threads per head (4 dims each), (head, dim group) items
+      constexpr int NH = GA_THREADS / ITEMS;                   // slot subsets worked on in parallel (2 at D = 128, 4 at D = 64)
+      float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [NH - 1][ITEMS] partial sums of subsets 1 ..
+      // thread tid owns slot tid: per-head maximum and normaliser by block reductions (warp shuffles + one shared round)
+      float* s_red = stg + 2 * RBQ_MAX_G * GA_THREADS + 4 * (NH > 1 ? (NH - 1) * ITEMS : 1);   // [2][RBQ_MAX_G][GA_WARPS]
+      float pm[RBQ_MAX_G], pl[RBQ_MAX_G];
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        pm[h] = -INFINITY; pl[h] = 0.0f;
+        if (h < G && touches) {
+          const float* pp = part + ((size_t)(tid + gi) * G + h) * GA_PART;
+          pm[h] = __ldcg(pp + D); pl[h] = __ldcg(pp + D + 1);
+        }
+      }
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        float v = pm[h];
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o2));
+        if (lane == 0) s_red[h * GA_WARPS + warp] = v;
+      }
+      __syncthreads();
+      float mall[RBQ_MAX_G];
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        float v = -INFINITY;
+#pragma unroll
+        for (int w = 0; w < GA_WARPS; ++w) v = fmaxf(v, s_red[h * GA_WARPS + w]);
+        mall[h] = v;
+        const float f = (pm[h] == -INFINITY) ? 0.0f : exp2f(pm[h] - v);
+        s_f[h * GA_THREADS + tid] = f;
+        float fl = f * pl[h];
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) fl += __shfl_xor_sync(0xffffffffu, fl, o2);
+        if (lane == 0) s_red[(RBQ_MAX_G + h) * GA_WARPS + warp] = fl;
+      }
+      __syncthreads();
+      const int item = tid % ITEMS, half = tid / ITEMS, d4 = (item % TPH) * 4;
+      const int h = (half < NH) ? (item / TPH) : RBQ_MAX_G;     // threads beyond NH * ITEMS only take part in the barriers
+      float mm = -INFINITY;
+#pragma unroll
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) mm = (hh == h) ? mall[hh] : mm;
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      float ll = 0.0f;
+      if (h < G) {
+        const float* pcol = part + ((size_t)gi * G + h) * GA_PART + d4;
+        const size_t pstride = (size_t)G * GA_PART;
+        constexpr int MU = 24;                                  // slot partials in flight per thread: one round for <= 48 slots
+        for (int c0 = clo + half; c0 <= chi; c0 += MU * NH) {
+          float f[MU];
+          float4 v[MU];
+#pragma unroll
+          for (int k = 0; k < MU; ++k) {
+            const int c = c0 + NH * k;
+            f[k] = (c <= chi) ? s_f[h * GA_THREADS + c] : 0.0f;
+            v[k] = (f[k] != 0.0f) ? __ldcg(reinterpret_cast<const float4*>(pcol + (size_t)c * pstride)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+#pragma unroll
+          for (int k = 0; k < MU; ++k) {
+            acc.x = fmaf(f[k], v[k].x, acc.x); acc.y = fmaf(f[k], v[k].y, acc.y);
+            acc.z = fmaf(f[k], v[k].z, acc.z); acc.w = fmaf(f[k], v[k].w, acc.w);
+          }
+        }
+#pragma unroll
+        for (int w = 0; w < GA_WARPS; ++w) ll += s_red[(RBQ_MAX_G + h) * GA_WARPS + w];
+      }
+      if (half >= 1 && half < NH) s_o[(half - 1) * ITEMS + item] = acc;
+      __syncthreads();
+      if (half == 0 && h < G) {
+#pragma unroll
+        for (int k = 1; k < NH; ++k) {
+          const float4 o2 = s_o[(k - 1) * ITEMS + item];
+          acc.x += o2.x; acc.y += o2.y; acc.z += o2.z; acc.w += o2.w;
+        }
+        const bool empty = !(ll > 0.0f);
+        const float inv = empty ? 0.0f : 1.0f / ll;
+        const size_t orow = (size_t)b * Hq + (size_t)g * G + h;
+        const float r4[4] = {acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (out_bf16) reinterpret_cast<__nv_bfloat16*>(out)[orow * D + d4 + k] = __float2bfloat16_rn(r4[k]);
+          else reinterpret_cast<float*>(out)[orow * D + d4 + k] = r4[k];
+        }
+        if (lse && d4 == 0) lse[orow] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(ll);
+      }
+      if (tid == 0) { gdone[gi] = 0; gnext[gi] = 0; }          // every touching CTA has made its last claim: ready for the next step
+      if (tid == 0) RBQ_STAMP(gather_probe, 8);
+    }
+    __syncthreads();                                           // staging area free before the next group's pipeline
+  }
+}
+
 // ---- FP32-pipe kernel for fp32 K/V or q (parity config 0) and for head_dim 256: split-K over the group's union list ------
 constexpr int AT_THREADS = 256;
 constexpr int AT_WARPS = AT_THREADS / 32;
@@ -797,6 +1331,22 @@ static int launch_gather_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const r
   return RBQ_OK;
 }
 
+template <int D>
+static int launch_gather_bits_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits, int wpr,
+                                const uint32_t* ucnt, int n_slices, int groups, float* part, int32_t* gdone, int32_t* gnext, void* out, float* lse,
+                                cudaStream_t s) {
+  auto kern = attn_gather_bits_kernel<D>;
+  RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_GATHER + (D == 64 ? 2 : 3), kern, GaCfg<D>::SMEM);
+  const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the merge uses one thread per CTA
+  RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, dim3(nc), dim3(GA_THREADS), (size_t)GaCfg<D>::SMEM, s, (const __nv_bfloat16*)q,
+                                  (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, bits, wpr, ucnt, n_slices,
+                                  (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, groups, ctx->cfg.n_q_heads,
+                                  ctx->cfg.n_kv_heads, ctx->sm_scale * 1.4426950408889634f, part, gdone, gnext, out,
+                                  ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse));
+  RBQ_LAUNCH_OK(ctx);
+  return RBQ_OK;
+}
+
 size_t rbq_attention_part_bytes(const rbq_ctx* ctx) {
   const size_t rows = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads, groups = (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads;
   const size_t D = ctx->cfg.head_dim;
@@ -817,8 +1367,8 @@ int rbq_launch_bits_from_lists(rbq_ctx* ctx, const rbq_index* idx, const int32_t
 }
 
 // S7 from the per-row selection bitmaps in the workspace: plan -> gather -> merge.
-int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits, void* out,
-                         float* lse, cudaStream_t s) {
+int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits,
+                         int n_slices, void* out, float* lse, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads, groups = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   if (groups > AT_MAX_GROUPS) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch*n_kv_heads %d > %d", groups, AT_MAX_GROUPS);
   const int wpr = rbq_words_per_row(ctx);
@@ -827,6 +1377,21 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   int32_t* ucount = reinterpret_cast<int32_t*>(ws + ctx->off_ucount);
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
   int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
+  // bf16 tensor-pipe path: the gather expands the bitmaps itself (no plan launch, no union list)
+  if (rbq_attention_uses_mma(ctx) && !ctx->gather_via_plan) {
+    int32_t* gnext = reinterpret_cast<int32_t*>(ws + ctx->off_gnext);
+    uint32_t* ucnt = reinterpret_cast<uint32_t*>(ws + ctx->off_ucnt);
+    if (n_slices <= 0) {                                       // bitmaps not from S6: count the unions here
+      n_slices = RBQ_UNION_SLICES;
+      union_count_kernel<<<dim3(RBQ_UNION_SLICES, groups), 256, 0, s>>>(bits, (const int32_t*)idx->n_indexed, ctx->cfg.n_q_heads,
+                                                                        ctx->cfg.n_kv_heads, wpr, ucnt);
+      RBQ_LAUNCH_OK(ctx);
+    }
+    if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));   // the plan stage is empty on this path
+    if (ctx->cfg.head_dim == 64)
+      return launch_gather_bits_d<64>(ctx, q, kv, idx, bits, wpr, ucnt, n_slices, groups, part, gdone, gnext, out, lse, s);
+    return launch_gather_bits_d<128>(ctx, q, kv, idx, bits, wpr, ucnt, n_slices, groups, part, gdone, gnext, out, lse, s);
+  }
   int split = PL_MAX_SPLIT;
   while (split > 1 && (long long)groups * split > (long long)ctx->sm_count) split >>= 1;   // one wave at ONE CTA per SM (40-64 registers x 1 024 threads)
 #define RBQ_PLAN_LAUNCH(SP)                                                                                          \

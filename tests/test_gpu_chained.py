@@ -36,7 +36,7 @@ def _chained(orc, w, rot, kind, p, with_cq=False, factor_f16=False):
     out3, sel_cnt3 = c.new_out(), c.new_sel()[1]
     c.decode_step(q, p, out3, None, sel_cnt3)
     torch.cuda.synchronize()
-    assert (out3.cpu().numpy().view(np.uint32) == out2.cpu().numpy().view(np.uint32)).all(), "fused without lists != fused"
+    U.assert_same_step_output(out3.cpu().numpy(), out2.cpu().numpy(), "fused without lists != fused")
     assert (sel_cnt3.cpu().numpy() == sel_cnt2.cpu().numpy()).all()
     s = scores.cpu().numpy()
     U.assert_logits_close(s, o["scores"], w.seq_lens, w.Hq)
@@ -55,7 +55,7 @@ def _chained(orc, w, rot, kind, p, with_cq=False, factor_f16=False):
     # budgets of the oracle chain and the GPU chain agree closely (boundary tokens only)
     assert np.abs(cnt.astype(np.int64) - o["sel_cnt"]).max() <= max(2, int(0.002 * o["sel_cnt"].max()))
     U.assert_attention_close(out.cpu().numpy(), o["out"], w.kv_dtype)
-    assert (out.cpu().numpy().view(np.uint32) == out2.cpu().numpy().view(np.uint32)).all(), "fused != staged output"
+    U.assert_same_step_output(out.cpu().numpy(), out2.cpu().numpy(), "fused != staged output")
     c.close()
     return o
 
@@ -400,7 +400,8 @@ def test_decode_step_host_buffers(orc, rot128):
     out_host = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32).pin_memory()
     c.decode_step_host(q_host, 0.9, out_host)
     torch.cuda.synchronize()
-    # on a non-default stream the host step is captured once and replayed as a CUDA graph: same bits every time
+    # on a non-default stream the host step is captured once and replayed as a CUDA graph: same result every time (up to the
+    # accumulation order of S7, whose chunks are handed out dynamically)
     side = torch.cuda.Stream()
     outs = []
     for _ in range(4):
@@ -409,11 +410,11 @@ def test_decode_step_host_buffers(orc, rot128):
         side.synchronize()
         outs.append((out_host if _ else o2).clone())
     for o2 in outs[1:]:
-        assert (o2.numpy().view(np.uint32) == outs[0].numpy().view(np.uint32)).all(), "graph replay differs from the direct host step"
+        U.assert_same_step_output(o2.numpy(), outs[0].numpy(), "graph replay differs from the direct host step")
     out = c.new_out()
     c.decode_step(q_host.cuda(), 0.9, out)
     torch.cuda.synchronize()
-    assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+    U.assert_same_step_output(out.cpu().numpy(), out_host.numpy())
     # new query values in the SAME pinned buffer (what a decode loop does): the replayed graph must read them afresh
     from paper_2606_31519_b200 import synth
     q_new = torch.from_numpy(synth.query_pool(w, 2)[1]).to(torch.bfloat16)
@@ -422,12 +423,12 @@ def test_decode_step_host_buffers(orc, rot128):
     side.synchronize()
     c.decode_step(q_new.cuda(), 0.9, out)
     torch.cuda.synchronize()
-    assert (out.cpu().numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
-    assert not (out_host.numpy() == outs[0].numpy()).all()
+    U.assert_same_step_output(out.cpu().numpy(), out_host.numpy())
+    assert np.abs(out_host.numpy() - outs[0].numpy()).max() > 1e-2
     q_host.copy_(torch.from_numpy(w.q).to(torch.bfloat16))
     c.decode_step_host(q_host, 0.9, out_host, stream=side)
     side.synchronize()
-    assert (out_host.numpy().view(np.uint32) == outs[0].numpy().view(np.uint32)).all()
+    U.assert_same_step_output(out_host.numpy(), outs[0].numpy())
     # pageable host buffers take the staged path (pinned ones receive the result straight from the S7 merge)
     q_page = torch.from_numpy(w.q).to(torch.bfloat16).clone()
     out_page = torch.zeros(w.B, w.Hq, 128, dtype=torch.float32)
@@ -436,7 +437,7 @@ def test_decode_step_host_buffers(orc, rot128):
         out_page.zero_()
         c.decode_step_host(q_page, 0.9, out_page, stream=st)
         (side if st is not None else torch.cuda.current_stream()).synchronize()
-        assert (out_page.numpy().view(np.uint32) == out_host.numpy().view(np.uint32)).all()
+        U.assert_same_step_output(out_page.numpy(), out_host.numpy())
     assert c.launch_count() > 0
     c.close()
 
