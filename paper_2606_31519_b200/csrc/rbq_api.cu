@@ -103,13 +103,17 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
   c->G = G;
   c->sm_scale = cfg->sm_scale > 0.0f ? cfg->sm_scale : (float)(1.0 / sqrt((double)cfg->head_dim));
   c->sm_count = sms;
-  { const char* e = getenv("RBQ_GATHER_PLAN"); c->gather_via_plan = (e && e[0] == '1') ? 1 : 0; }
   if (cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_flush, cudaEventDisableTiming) != cudaSuccess) {
     delete c;
     return RBQ_ERR_CUDA;
   }
   layout_workspace(c);
+  // S7 straight from the bitmaps when S6 runs in one wave (its union-count tail then costs ~2 us once; with several waves of
+  // Top-p CTAs every wave pays it, and the many small groups of such configurations leave the dynamic hand-out nothing to
+  // balance): otherwise through the plan kernel and union lists.  RBQ_GATHER_PLAN=1 / 0 in the environment forces either.
+  c->gather_via_plan = ((long long)cfg->batch * cfg->n_q_heads * rbq_topp_cluster_size(c) > sms) ? 1 : 0;
+  { const char* e = getenv("RBQ_GATHER_PLAN"); if (e && (e[0] == '0' || e[0] == '1')) c->gather_via_plan = e[0] - '0'; }
   if (rbq_topp_init(c) != RBQ_OK) {
     cudaEventDestroy(c->ev_copy);
     cudaEventDestroy(c->ev_flush);
@@ -315,8 +319,9 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, rowmax, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, ws_ptr<uint32_t>(ctx, ctx->off_ucnt),
-                          ws_ptr<int32_t>(ctx, ctx->off_garrive), s));
+  const bool from_bits = rbq_attention_from_bits(ctx);         // then S6 also leaves the union sizes of the KV groups
+  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, from_bits ? ws_ptr<uint32_t>(ctx, ctx->off_ucnt) : nullptr,
+                          from_bits ? ws_ptr<int32_t>(ctx, ctx->off_garrive) : nullptr, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
   const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, rbq_topp_cluster_size(ctx), out, nullptr, s);   // records ev[4] after the plan
   ctx->stage_ev = nullptr;

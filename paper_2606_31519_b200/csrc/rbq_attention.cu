@@ -812,6 +812,12 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     const uint32_t* wsrc = bits + ((size_t)b * Hq + (size_t)g * G + min(lane >> 3, G - 1)) * wpr + (lane & 7);
     const bool wlane = (lane >> 3) < G;
     int32_t* cnt_ptr = gnext + gi;
+    // The last CTA of a group whose range runs on into the next group takes only its share of this one (per warp, in cost
+    // units) and moves on: what it leaves is picked up by the CTAs that end in the group.  Without the limit a CTA that is
+    // alone in a small group at first (its neighbour still busy with its own first group) would take all of it.
+    const bool leave_early = (int)blockIdx.x == chi && chi > clo && r1 > gb;
+    const int limit = leave_early ? max(1, (gb - max(r0, ga)) / GA_WARPS) : 0x7fffffff;
+    int consumed = 0;
 
     if (tid == 0) RBQ_STAMP(gather_probe, 12);
     // claim stream of this warp: [w_a, w_a + n_a) = words to expand next (bitmap words in pre_a); raw_b / n_b = the claim after
@@ -858,6 +864,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     // expand claims until a whole tile is available or the group's words are exhausted
     auto fill = [&]() {
       while (tail - head < GA_TILE && n_a > 0) {
+        consumed += (n_a * 32) / RBQ_GB_TOKDIV - tail;
         for (int k = 0; k < n_a; ++k) {
           const int w = w_a + k;
           if (w < nw) {
@@ -876,12 +883,13 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
             tail += pc;
           }
         }
+        consumed += tail;
         w_a = dyn_base + __shfl_sync(0xffffffffu, raw_b, 0);   // claimed one claim ago
         n_a = max(0, min(n_b, nwt - w_a));
         if (n_a > 0) {
           pre_a = load_words(w_a, n_a);
-          n_b = claim_size(w_a);
-          if (lane == 0) raw_b = atomicAdd(cnt_ptr, n_b);
+          n_b = (consumed < limit) ? claim_size(w_a) : 0;      // share taken: this claim is the last
+          if (n_b > 0 && lane == 0) raw_b = atomicAdd(cnt_ptr, n_b);
         }
         __syncwarp();
       }
@@ -1315,6 +1323,8 @@ static bool rbq_attention_uses_mma(const rbq_ctx* ctx) {
   return ctx->cfg.kv_dtype == RBQ_BF16 && ctx->cfg.q_dtype == RBQ_BF16 && ctx->cfg.head_dim <= 128;
 }
 
+bool rbq_attention_from_bits(const rbq_ctx* ctx) { return rbq_attention_uses_mma(ctx) && !ctx->gather_via_plan; }
+
 template <int D>
 static int launch_gather_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* ulist,
                            const int32_t* ucount, int groups, float* part, int32_t* gdone, void* out, float* lse, cudaStream_t s) {
@@ -1378,7 +1388,7 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   float* part = reinterpret_cast<float*>(ws + ctx->off_part);
   int32_t* gdone = reinterpret_cast<int32_t*>(ws + ctx->off_gdone);
   // bf16 tensor-pipe path: the gather expands the bitmaps itself (no plan launch, no union list)
-  if (rbq_attention_uses_mma(ctx) && !ctx->gather_via_plan) {
+  if (rbq_attention_from_bits(ctx)) {
     int32_t* gnext = reinterpret_cast<int32_t*>(ws + ctx->off_gnext);
     uint32_t* ucnt = reinterpret_cast<uint32_t*>(ws + ctx->off_ucnt);
     if (n_slices <= 0) {                                       // bitmaps not from S6: count the unions here

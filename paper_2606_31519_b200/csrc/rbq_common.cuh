@@ -46,7 +46,7 @@ struct rbq_ctx {
   // workspace carve-up (byte offsets), filled by rbq_layout_workspace
   size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_gdone, off_rowmax, off_part,
       off_stage_q, off_stage_out, off_centroid, off_gnext, off_ucnt, off_garrive, total_bytes;
-  int gather_via_plan;       // RBQ_GATHER_PLAN=1 in the environment at rbq_create: S7 through attn_plan_kernel + union lists (the round-2a path, kept for A/B)
+  int gather_via_plan;       // S7 through attn_plan_kernel + union lists (deterministic; chosen at rbq_create, see there) instead of straight from the bitmaps
   cudaEvent_t ev_copy, ev_flush;
   unsigned char attr_done[128];   // kernel instantiations whose MaxDynamicSharedMemorySize was set for THIS context's device (RBQ_ATTR_*)
   size_t off_flags;          // device status word (RBQ_FLAG_*), sticky
@@ -266,5 +266,6 @@ int rbq_launch_bits_from_lists(rbq_ctx*, const rbq_index*, const int32_t* sel_id
 int rbq_launch_attention(rbq_ctx*, const void* q, const RbqKV&, const rbq_index*, const uint32_t* sel_bits,
                          int n_slices, void* out, float* lse, cudaStream_t);
 size_t rbq_attention_part_bytes(const rbq_ctx*);
+bool rbq_attention_from_bits(const rbq_ctx*);   // bf16 tensor-pipe gather that expands the bitmaps itself (needs the union sizes)
 // 32-bit words per bitmap row, padded to a multiple of 4 (16-byte vector loads)
 static inline int rbq_words_per_row(const rbq_ctx* c) { return (((c->cfg.max_tokens + 31) / 32) + 3) & ~3; }

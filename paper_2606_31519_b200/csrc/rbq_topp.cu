@@ -736,9 +736,9 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   //      its own (shared memory) and stores the popcount.  Plain store: nothing to reset but the arrival counter.
   if (ucnt) {
     const int gi = row / G, hh0 = row - gi * G;
-    __threadfence();                                          // this thread's bitmap words before the arrival
-    __syncthreads();
+    __syncthreads();                                          // every thread's bitmap words ...
     if (tid == 0) {
+      __threadfence();                                        // ... ordered before the arrival (fences are cumulative)
       const int old = (G > 1) ? atomicAdd(&garrive[(size_t)gi * RBQ_UNION_SLICES + rank], 1) : 0;
       sh.found = (old == G - 1) ? 2u : 0u;
     }
