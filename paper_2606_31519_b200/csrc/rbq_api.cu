@@ -24,8 +24,8 @@ void layout_workspace(rbq_ctx* c) {
   c->off_ucount = take(B * Hkv * sizeof(int32_t));
   c->off_gdone = take(B * Hkv * sizeof(int32_t));
   c->off_gnext = take(B * Hkv * sizeof(int32_t));
-  c->off_ucnt = take(B * Hkv * RBQ_UNION_SLICES * sizeof(uint32_t));
-  c->off_garrive = take(B * Hkv * RBQ_UNION_SLICES * sizeof(int32_t));
+  c->off_rho = take(B * Hkv * sizeof(float));
+  c->off_uexact = take(B * Hkv * sizeof(int32_t));
   c->off_rowmax = take(rows * sizeof(uint32_t));
   c->off_part = take(rbq_attention_part_bytes(c));
   const size_t D = g.head_dim;
@@ -109,11 +109,9 @@ int rbq_create(const rbq_config* cfg, rbq_ctx** out) {
     return RBQ_ERR_CUDA;
   }
   layout_workspace(c);
-  // S7 straight from the bitmaps when S6 runs in one wave (its union-count tail then costs ~2 us once; with several waves of
-  // Top-p CTAs every wave pays it, and the many small groups of such configurations leave the dynamic hand-out nothing to
-  // balance): otherwise through the plan kernel and union lists.  RBQ_GATHER_PLAN=1 / 0 in the environment forces either.
-  c->gather_via_plan = ((long long)cfg->batch * cfg->n_q_heads * rbq_topp_cluster_size(c) > sms) ? 1 : 0;
-  { const char* e = getenv("RBQ_GATHER_PLAN"); if (e && (e[0] == '0' || e[0] == '1')) c->gather_via_plan = e[0] - '0'; }
+  // S7 (bf16, head_dim <= 128) straight from the bitmaps; RBQ_GATHER_PLAN=1 in the environment: through the plan kernel and
+  // union lists instead (static partition: bit-reproducible accumulation order, ~7 us slower at config 2)
+  { const char* e = getenv("RBQ_GATHER_PLAN"); c->gather_via_plan = (e && e[0] == '1') ? 1 : 0; }
   if (rbq_topp_init(c) != RBQ_OK) {
     cudaEventDestroy(c->ev_copy);
     cudaEventDestroy(c->ev_flush);
@@ -159,7 +157,9 @@ int rbq_set_workspace(rbq_ctx* ctx, void* dev, size_t bytes) {
   // per-group arrival and chunk counters of S7: zero between steps (the last CTA to finish a group clears them)
   RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_gdone, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(int32_t)));
   RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_gnext, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(int32_t)));
-  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_garrive, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * RBQ_UNION_SLICES * sizeof(int32_t)));
+  // union-size history of S7 (rho = 0: none yet) and its per-step row counters
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_rho, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(float)));
+  RBQ_CUDA_OK(ctx, cudaMemset(static_cast<char*>(dev) + ctx->off_uexact, 0, (size_t)ctx->cfg.batch * ctx->cfg.n_kv_heads * sizeof(int32_t)));
   return RBQ_OK;
 }
 
@@ -262,7 +262,7 @@ int rbq_topp_select(rbq_ctx* ctx, const float* scores, const rbq_index* idx, flo
   if (!aligned16(scores)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "scores must be 16-byte aligned");
   if (!(p > 0.0f)) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "p must be > 0");
   return rbq_launch_topp(ctx, scores, nullptr, idx->n_indexed, p, ws_ptr<uint32_t>(ctx, ctx->off_selbits), sel_idx, sel_cnt,
-                         nullptr, nullptr, (cudaStream_t)stream);
+                         (cudaStream_t)stream);
 }
 
 int rbq_topp_select_static(rbq_ctx* ctx, const float* scores, const rbq_index* idx, float p, int32_t* sel_idx, int32_t* sel_cnt,
@@ -293,7 +293,7 @@ int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const
   if (!q || !sel_idx || !sel_cnt || !out) RBQ_FAIL(ctx, RBQ_ERR_INVALID_ARG, "q/sel_idx/sel_cnt/out null");
   uint32_t* bits = ws_ptr<uint32_t>(ctx, ctx->off_selbits);
   RBQ_TRY(rbq_launch_bits_from_lists(ctx, idx, sel_idx, sel_cnt, bits, (cudaStream_t)stream));
-  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, 0, out, lse, (cudaStream_t)stream);
+  return rbq_launch_attention(ctx, q, dev_kv(cache), idx, bits, sel_cnt, out, lse, (cudaStream_t)stream);
 }
 
 // q_copy != NULL: q is readable by the device but far away (mapped host memory): S3 reads it once and leaves a device copy
@@ -319,11 +319,9 @@ static int decode_step_impl(rbq_ctx* ctx, const void* q, void* q_copy, const rbq
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[1], s));
   RBQ_TRY(rbq_launch_estimate(ctx, idx, scores, nullptr, nullptr, rowmax, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[2], s));
-  const bool from_bits = rbq_attention_from_bits(ctx);         // then S6 also leaves the union sizes of the KV groups
-  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, from_bits ? ws_ptr<uint32_t>(ctx, ctx->off_ucnt) : nullptr,
-                          from_bits ? ws_ptr<int32_t>(ctx, ctx->off_garrive) : nullptr, s));
+  RBQ_TRY(rbq_launch_topp(ctx, scores, rowmax, idx->n_indexed, p, bits, sel_idx, sn, s));
   if (ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[3], s));
-  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, rbq_topp_cluster_size(ctx), out, nullptr, s);   // records ev[4] after the plan
+  const int rc = rbq_launch_attention(ctx, q_copy ? q_copy : q, dev_kv(cache), idx, bits, sn, out, nullptr, s);   // records ev[4] after the plan
   ctx->stage_ev = nullptr;
   if (rc == RBQ_OK && ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ev[RBQ_N_STAGES], s));
   return rc;
@@ -355,9 +353,11 @@ int rbq_profile_read(rbq_ctx* ctx, float* ms_host, int32_t* n_steps_host) {
   for (int i = 0; i < ctx->prof_steps; ++i) {
     cudaEvent_t* ev = ctx->prof_ev + (size_t)i * (RBQ_N_STAGES + 1);
     RBQ_CUDA_OK(ctx, cudaEventSynchronize(ev[RBQ_N_STAGES]));
+    const bool no_plan = rbq_attention_from_bits(ctx);          // S7 straight from the bitmaps: event 4 is not recorded
     for (int k = 0; k < RBQ_N_STAGES; ++k) {
+      if (no_plan && k == 3) continue;                          // plan stage: no launch, 0 ms
       float ms = 0.0f;
-      RBQ_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ev[k], ev[k + 1]));
+      RBQ_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ev[(no_plan && k == 4) ? 3 : k], ev[k + 1]));
       ms_host[k] += ms;
     }
   }

@@ -49,33 +49,6 @@ __global__ void bits_from_lists_kernel(const int32_t* __restrict__ sel_idx, cons
   }
 }
 
-// union size of each KV group's G bitmaps, in RBQ_UNION_SLICES equal word ranges (what S6 leaves in a fused step);
-// grid = (RBQ_UNION_SLICES, B*Hkv), 256 threads
-__global__ void union_count_kernel(const uint32_t* __restrict__ bits, const int32_t* __restrict__ n_indexed, int Hq, int Hkv, int wpr,
-                                   uint32_t* __restrict__ ucnt) {
-  __shared__ uint32_t s_w[8];
-  const int gi = blockIdx.y, b = gi / Hkv, g = gi % Hkv, G = Hq / Hkv;
-  const int nw = (max(0, n_indexed[b]) + 31) >> 5;
-  const int wps = (nw + RBQ_UNION_SLICES - 1) / RBQ_UNION_SLICES;
-  const int w0 = blockIdx.x * wps, w1 = min(nw, w0 + wps);
-  const uint32_t* rows0 = bits + ((size_t)b * Hq + (size_t)g * G) * wpr;
-  uint32_t c = 0;
-  for (int w = w0 + threadIdx.x; w < w1; w += blockDim.x) {
-    uint32_t u = 0;
-    for (int h = 0; h < G; ++h) u |= rows0[(size_t)h * wpr + w];
-    c += __popc(u);
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = c;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    uint32_t tot = 0;
-    for (int w = 0; w < 8; ++w) tot += s_w[w];
-    ucnt[(size_t)gi * RBQ_UNION_SLICES + blockIdx.x] = tot;
-  }
-}
-
 // ---- plan: union list per KV group ---------------------------------------------------------------------------------
 constexpr int PL_THREADS = 1024;
 constexpr int PL_MAX_SPLIT = 16;
@@ -615,19 +588,23 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 }
 
 // ---- gather attention straight from the selection bitmaps (no plan kernel, no union list in global memory) ----------------
-// The union of a KV group's G selection bitmaps is expanded where it is consumed.  Work unit: a warp chunk of GB_CHUNK = 128
-// tokens of one group (4 bitmap words per head; pending-window rows form extra chunks behind the bitmap chunks).  A warp
-// expands a chunk into its private ring of entries (token | head mask << 28) in shared memory, its cp.async pipeline takes
-// 16-entry tiles from the ring and runs on across chunk boundaries.
-//   * across groups the CTAs are placed by an ESTIMATE of every group's union size, computed by every CTA from the per-row
-//     selection counts S6 leaves (independent heads: n (1 - prod_h (1 - cnt_h / n)), clamped to [max_h cnt_h, min(n, sum_h cnt_h)])
-//     + the pending rows: equal contiguous ranges of the concatenated estimates, one per CTA, exactly as the union lists were
-//     cut before -- but a wrong estimate costs balance only, never correctness;
-//   * inside a group the chunks are handed out dynamically (one atomicAdd per chunk on the group's counter, claimed one chunk
-//     ahead so that its latency and that of the bitmap words hide behind the tiles in flight); the first chunk of every warp
-//     of the CTAs that START in the group is static, so no atomic sits in front of the first tile;
-//   * every CTA whose range touches a group arrives at it (possibly with an empty partial); the last one merges and resets
-//     the group's counters for the next step.
+// The union of a KV group's G selection bitmaps is expanded where it is consumed.  Work unit: a CLAIM of 1 .. GB_CW
+// consecutive bitmap words (32 tokens each) of one group, all G rows; the pending-window rows follow the bitmap words as
+// words of 32 rows.  A warp expands a claim into its private ring of entries (token | head mask << 28) in shared memory;
+// its cp.async pipeline takes 16-entry tiles from the ring and runs on across claim boundaries.
+//   * across groups the CTAs are placed by the groups' COSTS = union rows + tokens / RBQ_GB_TOKDIV (sparse groups stream
+//     slower per row: more bitmap to scan, isolated 512-byte rows), the union size being an estimate (build_cost_table):
+//     equal contiguous ranges of the concatenated costs, one per CTA, boundaries snapped to the borders of large groups.  A
+//     wrong estimate costs balance only, never correctness;
+//   * inside a group the words are handed out dynamically: one atomicAdd per claim on the group's counter, issued one claim
+//     ahead so that its latency and that of the bitmap words hide behind the tiles in flight; guided sizes (GB_CW0 .. 8 words
+//     = ~64 rows while plenty is left, one word at the end of the group); the first claim of every warp of the CTAs that START
+//     in the group is static, so no atomic sits in front of the first tile;
+//   * every CTA whose range touches a group arrives at it (possibly with an empty partial); the last one merges the partials
+//     into out / lse, stores the group's exact-to-estimated union ratio for the next step and resets the counters.
+// The accumulation order of a group's rows therefore depends on the hand-out: results are reproducible to rounding (~1e-6
+// relative), not bit for bit; RBQ_GATHER_PLAN=1 selects the static plan + union-list path below, which is.
+// Measured at config 2: plan 8-10 us + gather 55 us -> 56 us, step 90.9 -> 83.4 us (profiles/r02_ncu.md).
 constexpr int GB_CW = 8;                                     // bitmap words (32 tokens each) per claim at most: one word per lane and head
 constexpr int GB_CW0 = 4;                                    // words of a warp's static first claim
 constexpr int GB_RING = 512;                                 // entries per warp ring (>= 15 left over + one claim)
@@ -638,30 +615,48 @@ constexpr int GB_RING = 512;                                 // entries per warp
 #define RBQ_GB_SNAP 6                                        // CTA boundaries snap to boundaries between groups worth >= this many CTAs each
 #endif
 
-// s_start[gi] = sum over groups < gi of the attended rows (union of the group's selections + pending rows); every CTA
-// computes the same table from the per-slice union sizes S6 (or union_count_kernel) left in ucnt.
-__device__ void build_union_table(const uint32_t* __restrict__ ucnt, int n_slices, const int32_t* __restrict__ n_indexed,
-                                  const int32_t* __restrict__ n_total, int ngroups, int Hkv, int* s_start, int* s_warp,
-                                  int nthreads, int* s_nidx, int* s_npend) {
+// s_start[gi] = sum over groups < gi of the groups' costs; every CTA computes the same table.  The size of a group's union is
+// not known when S7 starts (S6 leaves per-row counts); it is ESTIMATED as rho_g * n (1 - prod_h (1 - cnt_h / n)): the size G
+// independent selections of these counts would have, times the ratio rho_g = exact / independent that this kernel measured
+// for the same group in the previous step (the heads of a group correlate through the keys they share; the ratio is a
+// property of the group much more than of the query).  0 = no history yet: 1.  A wrong estimate costs balance only.
+__device__ void build_cost_table(const int32_t* __restrict__ sel_cnt, const float* __restrict__ rho, const int32_t* __restrict__ n_indexed,
+                                 const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, int* s_start, int* s_warp,
+                                 int nthreads, int* s_nidx, int* s_npend, float* s_ind) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  const int G = Hq / Hkv;
   const int per = (ngroups + nthreads - 1) / nthreads;
   const int g0 = tid * per;
   int local = 0;
   for (int gi = g0; gi < min(ngroups, g0 + per); ++gi) {
-    const int b = gi / Hkv;
+    const int b = gi / Hkv, g = gi % Hkv;
     const int ni = max(0, n_indexed[b]), np = max(0, n_total[b] - ni);
-    uint32_t u = 0;
-    if (ni > 0) {                                             // S6 writes nothing for an empty index
-      const uint4 a = __ldcg(reinterpret_cast<const uint4*>(ucnt + (size_t)gi * RBQ_UNION_SLICES));
-      const uint4 c = __ldcg(reinterpret_cast<const uint4*>(ucnt + (size_t)gi * RBQ_UNION_SLICES + 4));
-      const uint32_t v[8] = {a.x, a.y, a.z, a.w, c.x, c.y, c.z, c.w};
+    int cnt[RBQ_MAX_G];
 #pragma unroll
-      for (int r = 0; r < RBQ_UNION_SLICES; ++r) u += (r < n_slices) ? v[r] : 0u;
+    for (int h = 0; h < RBQ_MAX_G; ++h) cnt[h] = (h < G) ? __ldcg(sel_cnt + (size_t)b * Hq + (size_t)g * G + h) : 0;
+    const float r = __ldcg(rho + gi);
+    int est = 0;
+    float ind = 0.0f;
+    if (ni > 0) {
+      const float inv = 1.0f / (float)ni;
+      float keep = 1.0f;
+      int mx = 0;
+      long long sum = 0;
+#pragma unroll
+      for (int h = 0; h < RBQ_MAX_G; ++h) {
+        const int c = min(max(cnt[h], 0), ni);
+        keep *= 1.0f - (float)c * inv;
+        mx = max(mx, c);
+        sum += c;
+      }
+      ind = (float)ni * (1.0f - keep);
+      est = (int)(ind * (r > 0.0f ? r : 1.0f) + 0.5f);
+      est = min(max(est, mx), (int)min((long long)ni, sum));
     }
-    const int est = (int)min(u, (uint32_t)ni);
     const int cost = (est + np > 0) ? est + np + ni / RBQ_GB_TOKDIV : 0;   // rows + what scanning the bitmaps of ni tokens costs
     s_nidx[gi] = ni;
     s_npend[gi] = np;
+    s_ind[gi] = ind;
     s_start[gi] = cost;                                       // the group's own cost for now, its prefix below
     local += cost;
   }
@@ -700,9 +695,10 @@ __device__ __forceinline__ int gb_begin(unsigned total, int c, int nce) {
 // border); identical in every CTA.
 __device__ void build_bounds(const int* s_start, int ngroups, unsigned total, int nce, int* s_bound, int nthreads) {
   const int tid = threadIdx.x;
-  for (int c = tid; c <= nce; c += nthreads) s_bound[c] = gb_begin(total, c, nce);
+  const unsigned q0 = total / (unsigned)nce, r0 = total - q0 * (unsigned)nce;   // floor(total c / nce) = q0 c + floor(r0 c / nce)
+  for (int c = tid; c <= nce; c += nthreads) s_bound[c] = (c >= nce) ? (int)total : (int)(q0 * (unsigned)c + (r0 * (unsigned)c) / (unsigned)nce);
   __syncthreads();
-  const int share = (int)(total / (unsigned)nce);
+  const int share = (int)q0;
   const float c_per_cost = (float)nce / (float)total;
   for (int k = 1 + tid; k < ngroups; k += nthreads) {
     const int bnd = s_start[k];
@@ -711,8 +707,8 @@ __device__ void build_bounds(const int* s_start, int ngroups, unsigned total, in
     int c = (int)((float)bnd * c_per_cost + 0.5f);             // nearest boundary, up to rounding: look at its neighbours too
     c = min(max(c, 1), nce - 1);
     int best = -1, bd = 0x7fffffff;
-    for (int cc = max(1, c - 1); cc <= min(nce - 1, c + 1); ++cc) {
-      const int x = gb_begin(total, cc, nce), dist = x > bnd ? x - bnd : bnd - x;
+    for (int cc = max(1, c - 1); cc <= min(nce - 1, c + 1); ++cc) {   // (no other border is near enough to move these three)
+      const int x = s_bound[cc], dist = x > bnd ? x - bnd : bnd - x;
       if (dist < bd) { bd = dist; best = cc; }
     }
     if (best > 0 && 2 * bd < share) s_bound[best] = bnd;
@@ -727,7 +723,8 @@ template <int D>
 __global__ void __launch_bounds__(GA_THREADS, 1)
 attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ K, const __nv_bfloat16* __restrict__ V,
                         long long sb, long long sh, long long st, const uint32_t* __restrict__ bits, int wpr,
-                        const uint32_t* __restrict__ ucnt, int n_slices, const int32_t* __restrict__ n_indexed,
+                        const int32_t* __restrict__ sel_cnt, float* __restrict__ rho, int32_t* __restrict__ uexact,
+                        const int32_t* __restrict__ n_indexed,
                         const int32_t* __restrict__ n_total, int ngroups, int Hq, int Hkv, float scale_log2,
                         float* __restrict__ part, int32_t* __restrict__ gdone, int32_t* __restrict__ gnext,
                         void* __restrict__ out, int out_bf16, float* __restrict__ lse) {
@@ -738,6 +735,8 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
   __shared__ int s_start[AT_MAX_GROUPS + 1], s_nidx[AT_MAX_GROUPS], s_npend[AT_MAX_GROUPS];
   __shared__ uint32_t s_ring[GA_WARPS][GB_RING];
   __shared__ int s_bound[GA_THREADS + 1];                     // snapped CTA boundaries in the cost space
+  __shared__ float s_ind[AT_MAX_GROUPS];                      // union size of independent selections (the estimate before rho)
+  __shared__ int s_rows;                                      // entries this CTA expanded in the current group
   __shared__ int s_warp[GA_WARPS];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -751,7 +750,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
   rbq_pdl_wait();                                             // selection bitmaps and counts of S6
   if (tid == 0) RBQ_STAMP(gather_probe, 1);
 
-  build_union_table(ucnt, n_slices, n_indexed, n_total, ngroups, Hkv, s_start, s_warp, GA_THREADS, s_nidx, s_npend);
+  build_cost_table(sel_cnt, rho, n_indexed, n_total, ngroups, Hq, Hkv, s_start, s_warp, GA_THREADS, s_nidx, s_npend, s_ind);
   if (tid == 0) RBQ_STAMP(gather_probe, 2);
   const unsigned total = (unsigned)s_start[ngroups];
   if (blockIdx.x == 0) {                                      // groups with nothing to attend: out = 0, lse = -inf
@@ -999,6 +998,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
 
     // merge the warps of the CTA (staging area aliases the drained pipeline buffers)
+    if (tid == 0) s_rows = 0;
     __syncthreads();
     float* stg = reinterpret_cast<float*>(ga_smem);            // [GA_WARPS][G][GA_PART]
     if (g4 < G) {
@@ -1007,7 +1007,9 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
       for (int nt = 0; nt < D / 8; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
       if (t4 == 0) { dst[D] = m_run; dst[D + 1] = l_run; }
     }
+    if (lane == 0 && tail > 0) atomicAdd(&s_rows, tail);       // every entry of the group is expanded exactly once, by some warp
     __syncthreads();
+    if (tid == 0 && s_rows > 0) atomicAdd(&uexact[gi], s_rows);   // before this CTA's arrival (fence below)
     float* pdst = part + (size_t)(blockIdx.x + gi) * G * GA_PART;
     for (int idx = tid; idx < G * D; idx += GA_THREADS) {
       const int h = idx / D, d = idx % D;
@@ -1122,7 +1124,13 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
         }
         if (lse && d4 == 0) lse[orow] = empty ? -INFINITY : mm * 0.6931471805599453f + logf(ll);
       }
-      if (tid == 0) { gdone[gi] = 0; gnext[gi] = 0; }          // every touching CTA has made its last claim: ready for the next step
+      if (tid == 0) {                                          // every touching CTA has made its last claim: ready for the next step
+        gdone[gi] = 0; gnext[gi] = 0;
+        const int ux = __ldcg(uexact + gi) - npend;            // exact size of the union (every arrival has added its entries)
+        uexact[gi] = 0;
+        const float ind = s_ind[gi];
+        rho[gi] = (ind >= 1.0f && ux > 0) ? fminf(fmaxf((float)ux / ind, 0.05f), 4.0f) : 0.0f;
+      }
       if (tid == 0) RBQ_STAMP(gather_probe, 8);
     }
     __syncthreads();                                           // staging area free before the next group's pipeline
@@ -1343,13 +1351,13 @@ static int launch_gather_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const r
 
 template <int D>
 static int launch_gather_bits_d(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits, int wpr,
-                                const uint32_t* ucnt, int n_slices, int groups, float* part, int32_t* gdone, int32_t* gnext, void* out, float* lse,
+                                const int32_t* sel_cnt, float* rho, int32_t* uexact, int groups, float* part, int32_t* gdone, int32_t* gnext, void* out, float* lse,
                                 cudaStream_t s) {
   auto kern = attn_gather_bits_kernel<D>;
   RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_GATHER + (D == 64 ? 2 : 3), kern, GaCfg<D>::SMEM);
   const int nc = min(ctx->sm_count, GA_THREADS);             // one persistent CTA per SM; the merge uses one thread per CTA
   RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, dim3(nc), dim3(GA_THREADS), (size_t)GaCfg<D>::SMEM, s, (const __nv_bfloat16*)q,
-                                  (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, bits, wpr, ucnt, n_slices,
+                                  (const __nv_bfloat16*)kv.k, (const __nv_bfloat16*)kv.v, kv.sb, kv.sh, kv.st, bits, wpr, sel_cnt, rho, uexact,
                                   (const int32_t*)idx->n_indexed, (const int32_t*)idx->n_total, groups, ctx->cfg.n_q_heads,
                                   ctx->cfg.n_kv_heads, ctx->sm_scale * 1.4426950408889634f, part, gdone, gnext, out,
                                   ctx->cfg.out_dtype == RBQ_BF16 ? 1 : 0, lse));
@@ -1378,7 +1386,7 @@ int rbq_launch_bits_from_lists(rbq_ctx* ctx, const rbq_index* idx, const int32_t
 
 // S7 from the per-row selection bitmaps in the workspace: plan -> gather -> merge.
 int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq_index* idx, const uint32_t* bits,
-                         int n_slices, void* out, float* lse, cudaStream_t s) {
+                         const int32_t* sel_cnt, void* out, float* lse, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads, groups = ctx->cfg.batch * ctx->cfg.n_kv_heads;
   if (groups > AT_MAX_GROUPS) RBQ_FAIL(ctx, RBQ_ERR_UNSUPPORTED, "batch*n_kv_heads %d > %d", groups, AT_MAX_GROUPS);
   const int wpr = rbq_words_per_row(ctx);
@@ -1390,17 +1398,12 @@ int rbq_launch_attention(rbq_ctx* ctx, const void* q, const RbqKV& kv, const rbq
   // bf16 tensor-pipe path: the gather expands the bitmaps itself (no plan launch, no union list)
   if (rbq_attention_from_bits(ctx)) {
     int32_t* gnext = reinterpret_cast<int32_t*>(ws + ctx->off_gnext);
-    uint32_t* ucnt = reinterpret_cast<uint32_t*>(ws + ctx->off_ucnt);
-    if (n_slices <= 0) {                                       // bitmaps not from S6: count the unions here
-      n_slices = RBQ_UNION_SLICES;
-      union_count_kernel<<<dim3(RBQ_UNION_SLICES, groups), 256, 0, s>>>(bits, (const int32_t*)idx->n_indexed, ctx->cfg.n_q_heads,
-                                                                        ctx->cfg.n_kv_heads, wpr, ucnt);
-      RBQ_LAUNCH_OK(ctx);
-    }
-    if (ctx->stage_ev) RBQ_CUDA_OK(ctx, cudaEventRecord(ctx->stage_ev[4], s));   // the plan stage is empty on this path
+    float* rho = reinterpret_cast<float*>(ws + ctx->off_rho);
+    int32_t* uexact = reinterpret_cast<int32_t*>(ws + ctx->off_uexact);
+    // (stage events: there is no plan stage on this path; rbq_profile_read reports 0 for it and does not read event 4)
     if (ctx->cfg.head_dim == 64)
-      return launch_gather_bits_d<64>(ctx, q, kv, idx, bits, wpr, ucnt, n_slices, groups, part, gdone, gnext, out, lse, s);
-    return launch_gather_bits_d<128>(ctx, q, kv, idx, bits, wpr, ucnt, n_slices, groups, part, gdone, gnext, out, lse, s);
+      return launch_gather_bits_d<64>(ctx, q, kv, idx, bits, wpr, sel_cnt, rho, uexact, groups, part, gdone, gnext, out, lse, s);
+    return launch_gather_bits_d<128>(ctx, q, kv, idx, bits, wpr, sel_cnt, rho, uexact, groups, part, gdone, gnext, out, lse, s);
   }
   int split = PL_MAX_SPLIT;
   while (split > 1 && (long long)groups * split > (long long)ctx->sm_count) split >>= 1;   // one wave at ONE CTA per SM (40-64 registers x 1 024 threads)

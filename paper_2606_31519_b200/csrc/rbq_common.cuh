@@ -13,7 +13,6 @@
 #define RBQ_WORDS 4          // D/32 code words per token at D = 128
 #define RBQ_MAX_G 4          // query heads per KV head (N=8 MMA columns: G heads + G ones-columns)
 #define RBQ_MAX_KSTEPS 8     // k-steps of the estimator MMA: D/32 (2, 4, 8 for D = 64, 128, 256)
-#define RBQ_UNION_SLICES 8   // union sizes of a KV group's selection come in up to 8 slices (one per CTA of a Top-p cluster)
 
 // Private per-(sequence, KV head) query constants produced by S3 and consumed by S4/S5.
 // bfrag: B-operand fragments of mma.m16n8k32.u8 in register order [k-step][lane][2]
@@ -45,8 +44,9 @@ struct rbq_ctx {
   size_t ws_bytes;
   // workspace carve-up (byte offsets), filled by rbq_layout_workspace
   size_t off_qconst, off_scores, off_selbits, off_selcnt, off_ulist, off_ucount, off_gdone, off_rowmax, off_part,
-      off_stage_q, off_stage_out, off_centroid, off_gnext, off_ucnt, off_garrive, total_bytes;
-  int gather_via_plan;       // S7 through attn_plan_kernel + union lists (deterministic; chosen at rbq_create, see there) instead of straight from the bitmaps
+      off_stage_q, off_stage_out, off_centroid, off_gnext, off_rho, off_uexact, total_bytes;
+  int gather_via_plan;       // RBQ_GATHER_PLAN=1 in the environment at rbq_create: S7 through attn_plan_kernel + union lists (deterministic
+                             // accumulation order) instead of straight from the bitmaps
   cudaEvent_t ev_copy, ev_flush;
   unsigned char attr_done[128];   // kernel instantiations whose MaxDynamicSharedMemorySize was set for THIS context's device (RBQ_ATTR_*)
   size_t off_flags;          // device status word (RBQ_FLAG_*), sticky
@@ -250,21 +250,17 @@ int rbq_topp_init(rbq_ctx* ctx);   // uploads the Top-p kernel's fp64 tables (on
 // S6 on caller-provided scores with its scratch in a static device array (no workspace, no allocation; rbq_topp.cu)
 int rbq_launch_topp_static(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx, int32_t* sel_cnt,
                            cudaStream_t);
-// ucnt / garrive (or NULL, NULL): S6 also leaves the size of the UNION of each KV group's G selections, per slice of the
-// row (slice r = CTA r of the row's cluster): ucnt [B*Hkv][RBQ_UNION_SLICES]; garrive: same shape, zero between launches.
 int rbq_launch_topp(rbq_ctx*, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
-                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, uint32_t* ucnt, int32_t* garrive, cudaStream_t);
-int rbq_topp_cluster_size(const rbq_ctx*);
+                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t);
 // Alg.3 selector (ternary threshold search in fp64): ascending sel_idx, sel_cnt, optional iteration counts [B*Hq].
 int rbq_launch_topp_alg3(rbq_ctx*, const float* scores, const int32_t* n_indexed, float p, int32_t* sel_idx, int32_t* sel_cnt,
                          int32_t* iters, cudaStream_t);
 int rbq_launch_bits_from_lists(rbq_ctx*, const rbq_index*, const int32_t* sel_idx, const int32_t* sel_cnt,
                                uint32_t* sel_bits, cudaStream_t);
 // S7 from the selection bitmaps: union plan -> gather attention -> merge.
-// n_slices > 0: the union sizes ucnt [B*Hkv][RBQ_UNION_SLICES] in the workspace were written by S6 with that many slices
-// per row; 0: they are computed here from the bitmaps (stand-alone rbq_sparse_attention).
+// sel_cnt: per-row selection counts (device): the bitmap-driven gather sizes its work partition with them.
 int rbq_launch_attention(rbq_ctx*, const void* q, const RbqKV&, const rbq_index*, const uint32_t* sel_bits,
-                         int n_slices, void* out, float* lse, cudaStream_t);
+                         const int32_t* sel_cnt, void* out, float* lse, cudaStream_t);
 size_t rbq_attention_part_bytes(const rbq_ctx*);
 bool rbq_attention_from_bits(const rbq_ctx*);   // bf16 tensor-pipe gather that expands the bitmaps itself (needs the union sizes)
 // 32-bit words per bitmap row, padded to a multiple of 4 (16-byte vector loads)

@@ -261,7 +261,7 @@ template <int CS>
 __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, TP_THREADS == 512 ? 2 : 1)
 topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
-            int32_t* __restrict__ sel_cnt, int G, uint32_t* __restrict__ ucnt, int32_t* __restrict__ garrive) {
+            int32_t* __restrict__ sel_cnt) {
   rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
   TP_STAMP(0);
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -301,7 +301,6 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     }
     if (sel_idx) for (int i = tid; i < len; i += TP_THREADS) sel_idx[rbase + lo + i] = lo + i;
     if (rank == 0 && tid == 0) { sel_cnt[row] = n; rowmax_key[row] = 0u; }   // nobody reads the key on this path
-    if (ucnt && tid == 0) ucnt[(size_t)(row / G) * RBQ_UNION_SLICES + rank] = (uint32_t)len;   // every row of the group writes the same value
     return;
   }
   auto csync = [&]() { if (CS == 1) __syncthreads(); else cluster.sync(); };
@@ -731,39 +730,6 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
     }
   }
   TP_STAMP(9);
-  // ---- union size of the KV group over this slice, for the work partition of S7 (rbq_attention.cu): the G CTAs that hold
-  //      slice `rank` of the group's G rows count arrivals; the last one ORs the other rows' words (just written, L2) with
-  //      its own (shared memory) and stores the popcount.  Plain store: nothing to reset but the arrival counter.
-  if (ucnt) {
-    const int gi = row / G, hh0 = row - gi * G;
-    __syncthreads();                                          // every thread's bitmap words ...
-    if (tid == 0) {
-      __threadfence();                                        // ... ordered before the arrival (fences are cumulative)
-      const int old = (G > 1) ? atomicAdd(&garrive[(size_t)gi * RBQ_UNION_SLICES + rank], 1) : 0;
-      sh.found = (old == G - 1) ? 2u : 0u;
-    }
-    __syncthreads();
-    if (sh.found == 2u) {
-      __threadfence();
-      const uint32_t* grow = sel_bits + (size_t)(row - hh0) * wpr + (lo >> 5);
-      uint32_t c = 0;
-      for (int w = tid; w < nwords; w += TP_THREADS) {
-        uint32_t u = selw[w];
-        for (int hh = 0; hh < G; ++hh) if (hh != hh0) u |= __ldcg(grow + (size_t)hh * wpr + w);
-        c += __popc(u);
-      }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(FULL, c, o);
-      if (lane == 0) sh.wt_c[warp] = c;
-      __syncthreads();
-      if (tid == 0) {
-        uint32_t tot = 0;
-        for (int w = 0; w < TP_WARPS; ++w) tot += sh.wt_c[w];
-        ucnt[(size_t)gi * RBQ_UNION_SLICES + rank] = tot;
-        if (G > 1) garrive[(size_t)gi * RBQ_UNION_SLICES + rank] = 0;
-      }
-    }
-  }
   TP_STAMP(13);
   // keep shared memory alive until every peer has read it: after S3 only the index-list path reads a peer (x_tot)
   if (sel_idx) csync();
@@ -783,7 +749,7 @@ __global__ void rowmax_kernel(const float* __restrict__ scores, const int32_t* _
 
 template <int CS>
 int launch_cs(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p, uint32_t* bits,
-              int wpr, int32_t* sel_idx, int32_t* sel_cnt, uint32_t* ucnt, int32_t* garrive, cudaStream_t s) {
+              int wpr, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
   const int s_cap = ((((ctx->cfg.max_tokens + CS - 1) / CS) + 31) & ~31) + 32;
   const size_t smem = TP_OFF_SC + (size_t)s_cap * 4;
@@ -791,7 +757,7 @@ int launch_cs(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int
   RBQ_SET_SMEM_ATTR(ctx, RBQ_ATTR_TOPP + CS, kern, RBQ_MAX_DYN_SMEM);
   dim3 grid(CS, rows);
   RBQ_CUDA_OK(ctx, rbq_launch_pdl(kern, grid, dim3(TP_THREADS), smem, s, scores, rowmax_key, n_indexed, ctx->cfg.n_q_heads,
-                                  ctx->cfg.max_tokens, wpr, p, bits, sel_idx, sel_cnt, ctx->G, ucnt, garrive));
+                                  ctx->cfg.max_tokens, wpr, p, bits, sel_idx, sel_cnt));
   RBQ_LAUNCH_OK(ctx);
   return RBQ_OK;
 }
@@ -822,7 +788,7 @@ int rbq_topp_cluster_size(const rbq_ctx* ctx) {
 
 // rowmax_key == NULL: the maxima are computed here (rbq_topp_select on caller-provided scores).
 int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, const int32_t* n_indexed, float p,
-                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, uint32_t* ucnt, int32_t* garrive, cudaStream_t s) {
+                    uint32_t* sel_bits, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t s) {
   const int cs = rbq_topp_cluster_size(ctx);
   const int wpr = rbq_words_per_row(ctx);
   const int rows = ctx->cfg.batch * ctx->cfg.n_q_heads;
@@ -838,10 +804,10 @@ int rbq_launch_topp(rbq_ctx* ctx, const float* scores, uint32_t* rowmax_key, con
     rowmax_key = rk;
   }
   switch (cs) {
-    case 8: return launch_cs<8>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, ucnt, garrive, s);
-    case 4: return launch_cs<4>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, ucnt, garrive, s);
-    case 2: return launch_cs<2>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, ucnt, garrive, s);
-    default: return launch_cs<1>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, ucnt, garrive, s);
+    case 8: return launch_cs<8>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    case 4: return launch_cs<4>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    case 2: return launch_cs<2>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
+    default: return launch_cs<1>(ctx, scores, rowmax_key, n_indexed, p, sel_bits, wpr, sel_idx, sel_cnt, s);
   }
 }
 
@@ -895,10 +861,10 @@ int rbq_launch_topp_static(rbq_ctx* ctx, const float* scores, const int32_t* n_i
   rowmax_kernel<<<grid, 256, 0, s>>>(scores, n_indexed, ctx->cfg.n_q_heads, ctx->cfg.max_tokens, keys);
   RBQ_LAUNCH_OK(ctx);
   switch (cs) {
-    case 8: return launch_cs<8>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, nullptr, nullptr, s);
-    case 4: return launch_cs<4>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, nullptr, nullptr, s);
-    case 2: return launch_cs<2>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, nullptr, nullptr, s);
-    default: return launch_cs<1>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, nullptr, nullptr, s);
+    case 8: return launch_cs<8>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    case 4: return launch_cs<4>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    case 2: return launch_cs<2>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
+    default: return launch_cs<1>(ctx, scores, keys, n_indexed, p, bits, wpr, sel_idx, sel_cnt, s);
   }
 }
 

@@ -73,11 +73,10 @@ def test_decode_step_chained(orc, rot128, cfg, kw, p, kind):
 @pytest.mark.parametrize("cfg,kw,p", [(1, dict(L=5003), 0.9), (3, dict(L=3001, B=7), 0.9), (3, dict(L=2500, B=24), 0.8),
                                       (4, dict(L=4099, B=2), 0.95)])
 def test_decode_step_chained_both_gather_paths(orc, rot128, cfg, kw, p, force, monkeypatch):
-    """S7 has two paths for bf16 K/V: straight from the selection bitmaps (dynamic hand-out of a group's bitmap words, union
-    sizes from the Top-p tail) and through attn_plan_kernel + union lists; rbq_create picks one by the shape (one wave of
-    Top-p CTAs or more).  Both are forced here on shapes with one, a few and many KV groups per CTA (ranges that straddle
-    several groups, groups shared by several CTAs, whole groups inside one CTA's range) and run through the whole chain
-    against the oracle."""
+    """S7 has two paths for bf16 K/V: straight from the selection bitmaps (dynamic hand-out of a group's bitmap words, work
+    partition by estimated union sizes; the default) and through attn_plan_kernel + union lists (RBQ_GATHER_PLAN=1).  Both
+    are forced here on shapes with one, a few and many KV groups per CTA (ranges that straddle several groups, groups shared
+    by several CTAs, whole groups inside one CTA's range) and run through the whole chain against the oracle."""
     monkeypatch.setenv("RBQ_GATHER_PLAN", force)
     _chained(orc, U.workload(cfg, **kw), rot128[0], ROT_DENSE, p)
 
