@@ -224,9 +224,23 @@ __device__ __forceinline__ void radix_scan(TpSmall& sh, const uint32_t (&cnt)[TP
   const double trem_in = sh.trem;                               // read before the barrier: the claiming thread rewrites it
   if (lane == 31) { sh.wt_u[warp] = si; sh.wt_c[warp] = ci; }
   __syncthreads();
-  u64 wp = 0, tot = 0;
-  uint32_t wc = 0;
-  for (int w = 0; w < TP_WARPS; ++w) { if (w < warp) { wp += sh.wt_u[w]; wc += sh.wt_c[w]; } tot += sh.wt_u[w]; }
+  if (warp == 0) {                                              // warp totals -> exclusive prefixes + grand total, by one warp (every
+    const u64 v = lane < TP_WARPS ? sh.wt_u[lane] : 0ull;        // thread summing the <= 32 totals itself costs ~3 K cycles of shared-
+    const uint32_t c = lane < TP_WARPS ? sh.wt_c[lane] : 0u;     // memory loads at 1 024 threads)
+    u64 vi = v;
+    uint32_t cx = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const u64 v2 = __shfl_up_sync(FULL, vi, o);
+      const uint32_t c2 = __shfl_up_sync(FULL, cx, o);
+      if (lane >= o) { vi += v2; cx += c2; }
+    }
+    if (lane < TP_WARPS) { sh.wt_u[lane] = vi - v; sh.wt_c[lane] = cx - c; }
+    if (lane == 31) sh.red_lo[0] = vi;
+  }
+  __syncthreads();
+  const u64 wp = sh.wt_u[warp], tot = sh.red_lo[0];
+  const uint32_t wc = sh.wt_c[warp];
   const double trem = fmin(trem_in, (double)tot);
   const u64 excl = wp + si - tsum, incl = wp + si;
   // exact integers: exactly one thread claims.  tot == 0 (every candidate weight underflows): first non-empty bin.
@@ -634,6 +648,10 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
 
   // ---- exact cut: every CTA ranks its share of the candidates against all of them (8 threads per candidate, integer
   //      prefix masses); the one thread that finds the cut publishes it to every CTA of the cluster -----------------
+  //      (Measured and dropped: one local radix level over the gathered candidates first -- a TP_NB-bin histogram of their
+  //      composite keys, a block scan, the few candidates of the crossing bin compacted and ranked: its six block barriers
+  //      at 1 024 threads cost what the quadratic ranking of ~500 candidates costs split over the CTAs of the row: Top-p
+  //      24.8 against 24.4 us at config 2.)
   {
     const double trem = sh.trem;
     const int per = (ncand + CS - 1) / CS;
