@@ -184,7 +184,13 @@ int rbq_topp_select_alg3(rbq_ctx* ctx, const float* scores, const rbq_index* idx
 /* ---- S7  hybrid attention over selected U pending tokens (Alg.2 lines 14-15, L188-190, L215) -- */
 /* out[b][h] = sum_{t in A} softmax_A(<q,k_t> sm_scale)_t v_t, A = sel_idx[b][h][0..cnt) U
  * [n_indexed[b], n_total[b]); out_dtype [B][Hq][D]; lse float [B][Hq] or NULL (log-sum-exp over A).
- * Empty A gives out = 0, lse = -inf.                                                           */
+ * Empty A gives out = 0, lse = -inf.
+ * Summation order (the paper fixes none, R19): with bf16 K/V and q and head_dim <= 128 the rows of a KV group are
+ * handed to the warps of the GPU dynamically, so the fp32 accumulation order -- not the attended set -- varies from call to
+ * call and two calls agree to rounding (~1e-6 of the output scale), not bit for bit.  RBQ_GATHER_PLAN=1 in the environment
+ * when the context is created selects a static partition (bit-reproducible, one more kernel launch); fp32 inputs and
+ * head_dim 256 always take a static partition.  Calls on one context must not overlap on the GPU (shared workspace:
+ * selection bitmaps, per-group counters).                                                        */
 int rbq_sparse_attention(rbq_ctx* ctx, const void* q, const rbq_kv* cache, const rbq_index* idx,
                          const int32_t* sel_idx, const int32_t* sel_cnt, void* out, float* lse,
                          void* stream);
@@ -211,8 +217,9 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
 int64_t rbq_launch_count(const rbq_ctx* ctx);
 
 /* ---- per-stage device timing of rbq_decode_step (measurement aid) ----------------- */
-/* Stages: 0 = S3 query prep, 1 = S4/S5 estimator, 2 = S6 Top-p, 3 = S7 union plan, 4 = S7 gather
- * attention (including the merge of its partials).  While enabled, every rbq_decode_step records RBQ_N_STAGES + 1 timing
+/* Stages: 0 = S3 query prep, 1 = S4/S5 estimator, 2 = S6 Top-p, 3 = S7 union plan (a launch of its own only on the
+ * static-partition paths: 0 ms when the gather expands the selection bitmaps itself), 4 = S7 gather attention (including
+ * the merge of its partials).  While enabled, every rbq_decode_step records RBQ_N_STAGES + 1 timing
  * events on its stream (up to RBQ_PROFILE_MAX_STEPS steps, later steps are not recorded).
  * rbq_profile_read BLOCKS until the recorded steps have finished (the only call that waits),
  * writes the summed milliseconds per stage to ms_host[RBQ_N_STAGES] and the number of recorded
