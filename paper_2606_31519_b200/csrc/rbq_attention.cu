@@ -1041,53 +1041,68 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
       float* s_f = stg;                                        // [G][GA_THREADS]: factor 2^(m - max) of slot c
       constexpr int TPH = D / 4, ITEMS = RBQ_MAX_G * TPH;     // threads per head (4 dims each), (head, dim group) items
       constexpr int NH = GA_THREADS / ITEMS;                   // slot subsets worked on in parallel (2 at D = 128, 4 at D = 64)
+      constexpr int MU = 24;                                    // slot partials in flight per thread: one round for <= 48 slots
       float4* s_o = reinterpret_cast<float4*>(stg + 2 * RBQ_MAX_G * GA_THREADS);   // [NH - 1][ITEMS] partial sums of subsets 1 ..
       // thread tid owns slot tid: per-head maximum and normaliser by block reductions (warp shuffles + one shared round)
       float* s_red = stg + 2 * RBQ_MAX_G * GA_THREADS + 4 * (NH > 1 ? (NH - 1) * ITEMS : 1);   // [2][RBQ_MAX_G][GA_WARPS]
+      const int item = tid % ITEMS, half = tid / ITEMS, d4 = (item % TPH) * 4;
+      const int h = (half < NH) ? (item / TPH) : RBQ_MAX_G;     // threads beyond NH * ITEMS only take part in the barriers
+      const float* pcol = part + ((size_t)gi * G + min(h, G - 1)) * GA_PART + d4;
+      const size_t pstride = (size_t)G * GA_PART;
+      // the first round of partial sums is requested together with the (m, l) pairs: one L2 round trip instead of two on the
+      // path of the last CTA (the accumulators of the streaming loop are dead: registers are free)
+      float4 v0[MU];
+#pragma unroll
+      for (int k = 0; k < MU; ++k) {
+        const int c = clo + half + NH * k;
+        v0[k] = (h < G && c <= chi) ? __ldcg(reinterpret_cast<const float4*>(pcol + (size_t)c * pstride)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
       float pm[RBQ_MAX_G], pl[RBQ_MAX_G];
 #pragma unroll
-      for (int h = 0; h < RBQ_MAX_G; ++h) {
-        pm[h] = -INFINITY; pl[h] = 0.0f;
-        if (h < G && touches) {
-          const float* pp = part + ((size_t)(tid + gi) * G + h) * GA_PART;
-          pm[h] = __ldcg(pp + D); pl[h] = __ldcg(pp + D + 1);
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) {
+        pm[hh] = -INFINITY; pl[hh] = 0.0f;
+        if (hh < G && touches) {
+          const float* pp = part + ((size_t)(tid + gi) * G + hh) * GA_PART;
+          pm[hh] = __ldcg(pp + D); pl[hh] = __ldcg(pp + D + 1);
         }
       }
 #pragma unroll
-      for (int h = 0; h < RBQ_MAX_G; ++h) {
-        float v = pm[h];
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) {
+        float v = pm[hh];
 #pragma unroll
         for (int o2 = 16; o2 > 0; o2 >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o2));
-        if (lane == 0) s_red[h * GA_WARPS + warp] = v;
+        if (lane == 0) s_red[hh * GA_WARPS + warp] = v;
       }
       __syncthreads();
       float mall[RBQ_MAX_G];
 #pragma unroll
-      for (int h = 0; h < RBQ_MAX_G; ++h) {
+      for (int hh = 0; hh < RBQ_MAX_G; ++hh) {
         float v = -INFINITY;
 #pragma unroll
-        for (int w = 0; w < GA_WARPS; ++w) v = fmaxf(v, s_red[h * GA_WARPS + w]);
-        mall[h] = v;
-        const float f = (pm[h] == -INFINITY) ? 0.0f : exp2f(pm[h] - v);
-        s_f[h * GA_THREADS + tid] = f;
-        float fl = f * pl[h];
+        for (int w = 0; w < GA_WARPS; ++w) v = fmaxf(v, s_red[hh * GA_WARPS + w]);
+        mall[hh] = v;
+        const float f = (pm[hh] == -INFINITY) ? 0.0f : exp2f(pm[hh] - v);
+        s_f[hh * GA_THREADS + tid] = f;
+        float fl = f * pl[hh];
 #pragma unroll
         for (int o2 = 16; o2 > 0; o2 >>= 1) fl += __shfl_xor_sync(0xffffffffu, fl, o2);
-        if (lane == 0) s_red[(RBQ_MAX_G + h) * GA_WARPS + warp] = fl;
+        if (lane == 0) s_red[(RBQ_MAX_G + hh) * GA_WARPS + warp] = fl;
       }
       __syncthreads();
-      const int item = tid % ITEMS, half = tid / ITEMS, d4 = (item % TPH) * 4;
-      const int h = (half < NH) ? (item / TPH) : RBQ_MAX_G;     // threads beyond NH * ITEMS only take part in the barriers
       float mm = -INFINITY;
 #pragma unroll
       for (int hh = 0; hh < RBQ_MAX_G; ++hh) mm = (hh == h) ? mall[hh] : mm;
       float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
       float ll = 0.0f;
       if (h < G) {
-        const float* pcol = part + ((size_t)gi * G + h) * GA_PART + d4;
-        const size_t pstride = (size_t)G * GA_PART;
-        constexpr int MU = 24;                                  // slot partials in flight per thread: one round for <= 48 slots
-        for (int c0 = clo + half; c0 <= chi; c0 += MU * NH) {
+#pragma unroll
+        for (int k = 0; k < MU; ++k) {                          // first round: already here
+          const int c = clo + half + NH * k;
+          const float f = (c <= chi) ? s_f[h * GA_THREADS + c] : 0.0f;   // an empty partial (f = 0) holds zeros
+          acc.x = fmaf(f, v0[k].x, acc.x); acc.y = fmaf(f, v0[k].y, acc.y);
+          acc.z = fmaf(f, v0[k].z, acc.z); acc.w = fmaf(f, v0[k].w, acc.w);
+        }
+        for (int c0 = clo + half + MU * NH; c0 <= chi; c0 += MU * NH) {   // groups shared by more than MU * NH CTAs
           float f[MU];
           float4 v[MU];
 #pragma unroll
