@@ -790,6 +790,16 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     if (ga >= gb) continue;
     const int b = gi / Hkv, g = gi % Hkv;
     const int nidx = s_nidx[gi], npend = s_npend[gi];
+    // A operand: Q rows of the group's heads (rows >= G are zero); requested first, used after the claim set-up below
+    uint32_t qa[D / 16][2];
+    {
+      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * D);
+#pragma unroll
+      for (int ks = 0; ks < D / 16; ++ks) {
+        qa[ks][0] = (g4 < G) ? qp[8 * ks + t4] : 0u;
+        qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
+      }
+    }
     // CTAs whose range touches [ga, gb): clo = last c with s_bound[c] <= ga, chi = last c with s_bound[c] < gb (the bounds are
     // strictly increasing and within half a share of total c / nce: a guess and a short walk)
     int clo = min(max((int)((float)ga * c_per_cost), 0), nce - 1);
@@ -842,16 +852,6 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
       pre_a = load_words(w_a, n_a);
       n_b = claim_size(w_a);
       if (lane == 0) raw_b = atomicAdd(cnt_ptr, n_b);
-    }
-    // A operand: Q rows of the group's heads (rows >= G are zero)
-    uint32_t qa[D / 16][2];
-    {
-      const uint32_t* qp = reinterpret_cast<const uint32_t*>(q + ((size_t)b * Hq + (size_t)g * G + min(g4, G - 1)) * D);
-#pragma unroll
-      for (int ks = 0; ks < D / 16; ++ks) {
-        qa[ks][0] = (g4 < G) ? qp[8 * ks + t4] : 0u;
-        qa[ks][1] = (g4 < G) ? qp[8 * ks + 4 + t4] : 0u;
-      }
     }
     if (tid == 0) RBQ_STAMP(gather_probe, 10);
     float m_run = -INFINITY, l_run = 0.0f;
