@@ -276,7 +276,7 @@ __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(TP_THREADS, TP_THRE
 topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key, const int32_t* __restrict__ n_indexed,
             int Hq, int Lcap, int wpr, float p_f, uint32_t* __restrict__ sel_bits, int32_t* __restrict__ sel_idx,
             int32_t* __restrict__ sel_cnt) {
-  rbq_pdl_trigger();                                          // the wait for S5 comes after the shared-memory set-up
+  rbq_pdl_trigger();                                          // (dependents: the gather cannot be resident beside this kernel anyway)
   TP_STAMP(0);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TpSmall& sh = *reinterpret_cast<TpSmall*>(smem_raw);
@@ -321,15 +321,14 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
   auto peer = [&](int r) -> const TpSmall* { return CS == 1 ? &sh : cluster.map_shared_rank(&sh, r); };
 
   // ---- pass 1: load the slice (read once) and histogram it ---------------------------------------------
+  // A CTA of 1 024 threads x 64 registers becomes resident only when its SM has drained, i.e. at the very end of S5: the
+  // set-up below is not hidden behind the predecessor.  So the wait comes first, the slice copies go out right behind it and
+  // the histogram is zeroed while they are in flight.
   const double tabv = tid < TP_NC + 32 ? g_tp_tab[tid] : 0.0;    // written at rbq_create, not by a kernel of the chain
-  for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
-  if (tid < TP_OFS) { hist[2 * TP_NB + tid] = 0u; hist[3 * TP_NB + tid] = 0u; }   // overflow slots (candidate area, free until S1)
-  if (tid == 0) { sh.lcount = 0; sh.found = 0; }
   rbq_pdl_wait();                                             // scores and row maxima of S5
   TP_STAMP(1);
   const float jof_f = tp_overflow_bin(n, p_f);
   const int jof = (int)jof_f;
-  __syncthreads();
   float m, ms_;                                               // row maximum: loaded behind the slice copies (one latency, not two)
   {
     const float4* src = reinterpret_cast<const float4*>(scores + rbase + lo);
@@ -343,10 +342,16 @@ topp_kernel(const float* __restrict__ scores, uint32_t* __restrict__ rowmax_key,
       for (int i4 = tid; i4 < n4; i4 += TP_THREADS)
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst + 16u * (uint32_t)i4), "l"(src + i4) : "memory");
       asm volatile("cp.async.commit_group;" ::: "memory");
-      m = __fadd_rn(rbq_fkey_inv(rowmax_key[row]), 0.0f);
-      ms_ = __fmul_rn(m, TP_SCALE);
+      const uint32_t mkey = rowmax_key[row];
+      for (int i = tid; i < 2 * TP_NB; i += TP_THREADS) hist[i] = 0u;
+      if (tid < TP_OFS) { hist[2 * TP_NB + tid] = 0u; hist[3 * TP_NB + tid] = 0u; }   // overflow slots (candidate area, free until S1)
+      if (tid == 0) { sh.lcount = 0; sh.found = 0; }
+      __syncthreads();                                         // histogram zeroed by all before anybody adds to it (the copies are still
+                                                               // in flight: every thread then starts on its own groups as they land)
       if (tid < TP_NC) sh.tabA[tid] = tabv;                    // fp64 tables: loaded at kernel entry, first used after the pass
       else if (tid < TP_NC + 32) sh.tabB[tid - TP_NC] = tabv;
+      m = __fadd_rn(rbq_fkey_inv(mkey), 0.0f);
+      ms_ = __fmul_rn(m, TP_SCALE);
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     TP_STAMP(10);
