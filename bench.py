@@ -384,6 +384,9 @@ def run_b200(args):
                 "traffic_source": f"static: {NCU_SUMMARY} (committed ncu --set full capture, not measured in this run)",
                 "frac_at_ncu_duration": (alg[dom] / (ncu[dom][2] * 1e-6) / 1e9 / peak) if dom in ncu else None,
                 "peak_source": peak_src,
+                "kernel_note": ("attn_gather = the whole S7 stage in ONE kernel (attn_gather_bits_kernel: expands the selection "
+                                "bitmaps, gathers, contracts, merges); until the middle of round 2 S7 was attn_plan + attn_gather "
+                                "and this entry was the second of the two kernels only") if dom == "attn_gather" else None,
                 "algorithmic_bytes": alg[dom], "us_per_launch": stages[dom]["us"], "stages": stages,
                 "attended_rows_union": uni, "attended_rows_per_head_sum": per_head,
                 "attn_per_head_bytes_gbs": per_head * 2 * w.D * esz / (stages["attn_gather"]["us"] * 1e-6) / 1e9
