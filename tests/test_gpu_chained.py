@@ -81,6 +81,34 @@ def test_decode_step_chained_both_gather_paths(orc, rot128, cfg, kw, p, force, m
     _chained(orc, U.workload(cfg, **kw), rot128[0], ROT_DENSE, p)
 
 
+def test_plan_path_is_bit_reproducible_and_matches_default(rot128, monkeypatch):
+    """RBQ_GATHER_PLAN=1 (static partition over union lists) gives the same bits on every run; the default path (dynamic
+    hand-out) agrees with it to the accumulation-order bound, run after run, also while its union-size history (rho) settles
+    over the first steps and after the query has changed."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    w = U.workload(2, L=9000, n_heavy=32)
+    pool = synth.query_pool(w, 3)
+    outs = {}
+    for force in ("1", "0"):
+        monkeypatch.setenv("RBQ_GATHER_PLAN", force)
+        c = U.make_cache(w, rot128[0])
+        c.encode_keys(U.to_dev(w.seq_lens))
+        res = []
+        for i in range(6):
+            q = U.to_dev(pool[i % 3], U.torch_dtype(w))
+            o = c.new_out()
+            c.decode_step(q, 0.9, o)
+            torch.cuda.synchronize()
+            res.append(o.cpu().numpy())
+        outs[force] = res
+        c.close()
+    for i in range(3):                                    # same query three steps later: same bits on the static path
+        assert (outs["1"][i].view(np.uint32) == outs["1"][i + 3].view(np.uint32)).all()
+    for i in range(6):
+        U.assert_same_step_output(outs["0"][i], outs["1"][i], f"default path differs from the plan path at step {i}")
+
+
 @pytest.mark.parametrize("kind", [ROT_DENSE, ROT_WH])
 @pytest.mark.parametrize("cfg,kw,D", [(1, dict(L=5003), 128), (3, dict(L=3001, B=3), 128), (1, dict(L=3001), 64), (2, dict(L=4100, n_heavy=32), 256)])
 def test_decode_step_chained_f16_factors(orc, cfg, kw, D, kind):
