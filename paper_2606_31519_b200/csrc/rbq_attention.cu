@@ -604,7 +604,7 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 //     into out / lse, stores the group's exact-to-estimated union ratio for the next step and resets the counters.
 // The accumulation order of a group's rows therefore depends on the hand-out: results are reproducible to rounding (~1e-6
 // relative), not bit for bit; RBQ_GATHER_PLAN=1 selects the static plan + union-list path below, which is.
-// Measured at config 2: plan 8-10 us + gather 55 us -> 56 us, step 90.9 -> 83.4 us (profiles/r02_ncu.md).
+// Measured at config 2 (stage events): plan 10.3 us + gather 55.2 us -> 56.3 us; step 90.9 -> 82.8 us (profiles/r02_ncu.md).
 constexpr int GB_CW = 8;                                     // bitmap words (32 tokens each) per claim at most: one word per lane and head
 constexpr int GB_CW0 = 4;                                    // words of a warp's static first claim
 constexpr int GB_RING = 512;                                 // entries per warp ring (>= 15 left over + one claim)
@@ -678,13 +678,6 @@ __device__ void build_cost_table(const int32_t* __restrict__ sel_cnt, const floa
   }
   if (tid == 0) s_start[ngroups] = total;
   __syncthreads();
-}
-
-// first estimated row of CTA c of nce (total >= nce >= 1): floor(total * c / nce), strictly increasing in c
-__device__ __forceinline__ int gb_begin(unsigned total, int c, int nce) {
-  if (c >= nce) return (int)total;
-  const unsigned q0 = total / (unsigned)nce, r0 = total - q0 * (unsigned)nce;
-  return (int)(q0 * (unsigned)c + (r0 * (unsigned)c) / (unsigned)nce);
 }
 
 // CTA boundaries in the cost space, snapped: s_bound[c] = floor(total c / nce), and the boundary nearest to the border
