@@ -243,6 +243,35 @@ def test_append_flush_state_machine(orc, rot128, use_side, kind):
     c.close()
 
 
+@pytest.mark.parametrize("force", ["0", "1"])
+def test_large_pending_window_both_gather_paths(orc, rot128, force, monkeypatch):
+    """A pending window of several hundred rows (W = 1024: nothing is flushed), appended 100 / 200 / 61 rows at a time: the
+    pending rows follow the bitmap words of a KV group as many words of 32 rows, claims straddle the border between the two,
+    the last pending word is ragged.  Output against the oracle's step after each append, on both S7 paths."""
+    import torch
+    from paper_2606_31519_b200 import synth
+    monkeypatch.setenv("RBQ_GATHER_PLAN", force)
+    W = 1024
+    w = U.workload(3, L=1700, B=3, extra_cap=512)
+    lazy = orc.LazyIndex(w.K, w.V, w.seq_lens, ROT_DENSE, rot128[0], W)
+    c = U.make_cache(w, rot128[0], flush_tokens=W)
+    c.encode_keys(U.to_dev(w.seq_lens))
+    pool = synth.query_pool(w, 3)
+    out = c.new_out()
+    for s, n_new in enumerate((100, 200, 61)):
+        k_new, v_new = synth.append_rows(3, 40 + s, w.B, w.Hkv, n_new)
+        lazy.append(k_new, v_new)
+        c.append_tokens(U.to_dev(k_new, torch.bfloat16), U.to_dev(v_new, torch.bfloat16))
+        c.decode_step(U.to_dev(pool[s], torch.bfloat16), 0.9, out)
+        torch.cuda.synchronize()
+        assert (c.n_indexed.cpu().numpy() == lazy.n_indexed).all() and (c.n_total.cpu().numpy() == lazy.n_total).all()
+        assert int((lazy.n_total - lazy.n_indexed).min()) == sum((100, 200, 61)[:s + 1])
+        ref = orc.decode_step(pool[s], lazy.K, lazy.V, lazy.codes, lazy.f_scale, None, lazy.c_k, None, lazy.n_indexed,
+                              lazy.n_total, ROT_DENSE, rot128[0], 0.9, U.SM_SCALE)
+        U.assert_attention_close(out.cpu().numpy(), ref["out"], "bf16")
+    c.close()
+
+
 def test_append_flush_enc_fast(orc, rot128):
     """Lazy flush through RBQ_ENC_FAST (tcgen05 encode with per-sequence t_begin / t_count, tiles far from full): the
     flushed rows carry the oracle's codes up to the guard band (|y_j| <= 1e-5 ||x||) and its factors within 1e-5."""
