@@ -74,7 +74,9 @@ def test_decode_step_chained(orc, rot128, cfg, kw, p, kind):
                                       (4, dict(L=4099, B=2), 0.95),
                                       (1, dict(L=3001, Hq=8, Hkv=8), 0.9),      # G = 1: one bitmap row per group
                                       (1, dict(L=4100, Hq=12, Hkv=6), 0.9),     # G = 2
-                                      (3, dict(L=1500, B=5, Hq=4, Hkv=1), 0.8)])
+                                      (3, dict(L=1500, B=5, Hq=4, Hkv=1), 0.8),
+                                      (1, dict(L=70, Hq=4, Hkv=2), 0.6),        # fewer attended rows than CTAs
+                                      (1, dict(L=33, n_heavy=4), 0.9)])         # two bitmap words, the second with one token
 def test_decode_step_chained_both_gather_paths(orc, rot128, cfg, kw, p, force, monkeypatch):
     """S7 has two paths for bf16 K/V: straight from the selection bitmaps (dynamic hand-out of a group's bitmap words, work
     partition by estimated union sizes; the default) and through attn_plan_kernel + union lists (RBQ_GATHER_PLAN=1).  Both
