@@ -611,6 +611,9 @@ constexpr int GB_RING = 512;                                 // entries per warp
 #ifndef RBQ_GB_TOKDIV
 #define RBQ_GB_TOKDIV 14                                     // cost of a group = union rows + tokens / RBQ_GB_TOKDIV (scan + sparse-row penalty)
 #endif
+#ifndef RBQ_GB_BYTEPAR
+#define RBQ_GB_BYTEPAR 5                                     // n > 0: byte-parallel expansion of the claims of groups whose claims exceed n words (see fill)
+#endif
 #ifndef RBQ_GB_SNAP
 #define RBQ_GB_SNAP 6                                        // CTA boundaries snap to boundaries between groups worth >= this many CTAs each
 #endif
@@ -808,6 +811,9 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     const int dyn_base = max(0, chi - cfl + 1) * GA_WARPS * GB_CW0;   // words below it are the static first claims
     // words per claim: ~64 attended rows while plenty is left, down to one word at the end of the group
     const int cw_max = min(GB_CW, max(GB_CW0, (int)(2.0f * (float)max(nidx, 1) / (float)max(gb - ga, 1))));
+#if RBQ_GB_BYTEPAR
+    const bool bytepar = cw_max > RBQ_GB_BYTEPAR;              // warp-uniform, per group
+#endif
     const __nv_bfloat16* Kb = K + (long long)b * sb + (long long)g * sh;
     const __nv_bfloat16* Vb = V + (long long)b * sb + (long long)g * sh;
     // lane l loads word (l & 7) of head (l >> 3) of a claim
@@ -857,7 +863,41 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     auto fill = [&]() {
       while (tail - head < GA_TILE && n_a > 0) {
         consumed += (n_a * 32) / RBQ_GB_TOKDIV - tail;
+#if RBQ_GB_BYTEPAR
+        // sparse groups (claims of more than RBQ_GB_BYTEPAR words): all bitmap words of the claim at once: lane 4 j + s owns byte s of word j (8 tokens): the four heads' bytes side by
+        // side in P, a warp scan of the bytes' popcounts, then every lane writes its <= 8 entries (head mask of bit b =
+        // bits b, 8 + b, 16 + b, 24 + b of P, moved to bits 28 .. 31 by one multiplication)
+        const int nbw = bytepar ? min(n_a, nw - w_a) : 0;
+        if (nbw > 0) {
+          const int j = lane >> 2, sB = lane & 3;
+          const uint32_t w0 = __shfl_sync(0xffffffffu, pre_a, j), w1 = __shfl_sync(0xffffffffu, pre_a, 8 + j);
+          const uint32_t w2 = __shfl_sync(0xffffffffu, pre_a, 16 + j), w3 = __shfl_sync(0xffffffffu, pre_a, 24 + j);
+          const uint32_t selr = (uint32_t)sB | ((uint32_t)(4 + sB) << 4);
+          const uint32_t P = __byte_perm(__byte_perm(w0, w1, selr), __byte_perm(w2, w3, selr), 0x5410);
+          uint32_t u8 = (P | (P >> 8) | (P >> 16) | (P >> 24)) & 0xFFu;
+          const int cnt = __popc(u8);
+          int incl = cnt;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+          }
+          const int tot = __shfl_sync(0xffffffffu, incl, 31);
+          int pos = tail + incl - cnt;
+          const uint32_t tokb = (uint32_t)((w_a + j) * 32 + 8 * sB);
+          while (u8) {
+            const int bp = __ffs(u8) - 1;
+            u8 &= u8 - 1u;
+            ring[pos & (GB_RING - 1)] = (tokb + (uint32_t)bp) | ((((P >> bp) & 0x01010101u) * 0x10204080u) & 0xF0000000u);
+            ++pos;
+          }
+          __syncwarp();
+          tail += tot;
+        }
+        for (int k = max(nbw, 0); k < n_a; ++k) {
+#else
         for (int k = 0; k < n_a; ++k) {
+#endif
           const int w = w_a + k;
           if (w < nw) {
             uint32_t u = 0u, mask = 0u;
