@@ -611,6 +611,9 @@ constexpr int GB_RING = 512;                                 // entries per warp
 #ifndef RBQ_GB_TOKDIV
 #define RBQ_GB_TOKDIV 14                                     // cost of a group = union rows + tokens / RBQ_GB_TOKDIV (scan + sparse-row penalty)
 #endif
+#ifndef RBQ_GB_PEN
+#define RBQ_GB_PEN 800                                       // fixed cost of a group (one visit: prologue, drain, merge, arrival) in row units
+#endif
 #ifndef RBQ_GB_BYTEPAR
 #define RBQ_GB_BYTEPAR 5                                     // n > 0: byte-parallel expansion of the claims of groups whose claims exceed n words (see fill)
 #endif
@@ -656,7 +659,7 @@ __device__ void build_cost_table(const int32_t* __restrict__ sel_cnt, const floa
       est = (int)(ind * (r > 0.0f ? r : 1.0f) + 0.5f);
       est = min(max(est, mx), (int)min((long long)ni, sum));
     }
-    const int cost = (est + np > 0) ? est + np + ni / RBQ_GB_TOKDIV : 0;   // rows + what scanning the bitmaps of ni tokens costs
+    const int cost = (est + np > 0) ? est + np + ni / RBQ_GB_TOKDIV + RBQ_GB_PEN : 0;   // rows + scanning the bitmaps of ni tokens + one visit
     s_nidx[gi] = ni;
     s_npend[gi] = np;
     s_ind[gi] = ind;
@@ -825,7 +828,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     // alone in a small group at first (its neighbour still busy with its own first group) would take all of it.
     const bool leave_early = (int)blockIdx.x == chi && chi > clo && r1 > gb;
     const int limit = leave_early ? max(1, (gb - max(r0, ga)) / GA_WARPS) : 0x7fffffff;
-    int consumed = 0;
+    int consumed = RBQ_GB_PEN / GA_WARPS;                      // this visit's own fixed cost counts towards the share
 
     if (tid == 0) RBQ_STAMP(gather_probe, 12);
     // claim stream of this warp: [w_a, w_a + n_a) = words to expand next (bitmap words in pre_a); raw_b / n_b = the claim after
