@@ -590,10 +590,12 @@ attn_gather_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __r
 // ---- gather attention straight from the selection bitmaps (no plan kernel, no union list in global memory) ----------------
 // The union of a KV group's G selection bitmaps is expanded where it is consumed.  Work unit: a CLAIM of 1 .. GB_CW
 // consecutive bitmap words (32 tokens each) of one group, all G rows; the pending-window rows follow the bitmap words as
-// words of 32 rows.  A warp expands a claim into its private ring of entries (token | head mask << 28) in shared memory;
+// words of 32 rows.  A warp expands a claim into its private ring of entries (token | head mask << 28) in shared memory
+// (dense groups: one word per step, lane = token; sparse groups: all words of the claim at once, lane = one byte of one word);
 // its cp.async pipeline takes 16-entry tiles from the ring and runs on across claim boundaries.
 //   * across groups the CTAs are placed by the groups' COSTS = union rows + tokens / RBQ_GB_TOKDIV (sparse groups stream
-//     slower per row: more bitmap to scan, isolated 512-byte rows), the union size being an estimate (build_cost_table):
+//     slower per row: more bitmap to scan, isolated 512-byte rows) + RBQ_GB_PEN (every visit of a group costs a prologue, a
+//     pipeline drain, a merge and an arrival), the union size being an estimate (build_cost_table):
 //     equal contiguous ranges of the concatenated costs, one per CTA, boundaries snapped to the borders of large groups.  A
 //     wrong estimate costs balance only, never correctness;
 //   * inside a group the words are handed out dynamically: one atomicAdd per claim on the group's counter, issued one claim
