@@ -400,9 +400,11 @@ int rbq_decode_step_host(rbq_ctx* ctx, const void* q_host, const rbq_kv* cache, 
     cudaGetLastError();
     return nullptr;
   };
-  void* out_mapped = mapped(out_host);
-  const void* q_mapped = mapped(q_host);                       // S3 reads q over PCIe and leaves the device copy for S7
-  auto direct = [&]() -> int {
+  void* out_mapped = nullptr;
+  const void* q_mapped = nullptr;                              // S3 reads q over PCIe and leaves the device copy for S7
+  bool looked_up = false;                                      // (two driver calls: not on the replay path, where the CPU-side
+  auto direct = [&]() -> int {                                 //  latency of the launch is part of every step)
+    if (!looked_up) { out_mapped = mapped(out_host); q_mapped = mapped(q_host); looked_up = true; }
     if (!q_mapped) RBQ_CUDA_OK(ctx, cudaMemcpyAsync(dq, q_host, qb, cudaMemcpyHostToDevice, s));
     RBQ_TRY(decode_step_impl(ctx, q_mapped ? q_mapped : dq, q_mapped ? dq : nullptr, cache, idx, p, out_mapped ? out_mapped : dout,
                              nullptr, nullptr, stream));
