@@ -749,7 +749,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
   __syncthreads();
 #endif
   rbq_pdl_wait();                                             // selection bitmaps and counts of S6
-  if (tid == 0) RBQ_STAMP(gather_probe, 1);
+  if (tid == 0) { RBQ_STAMP(gather_probe, 1); s_rows = 0; }    // (barriers inside the table builders below)
 
   build_cost_table(sel_cnt, rho, n_indexed, n_total, ngroups, Hq, Hkv, s_start, s_warp, GA_THREADS, s_nidx, s_npend, s_ind);
   if (tid == 0) RBQ_STAMP(gather_probe, 2);
@@ -1035,12 +1035,12 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
     l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
 
-    // merge the warps of the CTA (staging area aliases the drained pipeline buffers)
-    if (tid == 0) s_rows = 0;
-    __syncthreads();
-    float* stg = reinterpret_cast<float*>(ga_smem);            // [GA_WARPS][G][GA_PART]
+    // merge the warps of the CTA.  Every warp stages its partial in its OWN drained pipeline buffers (no barrier in front:
+    // nobody else touches them), [G][GA_PART] floats at the start of the warp's region; s_rows is zero here (below)
+    float* stg = reinterpret_cast<float*>(ga_smem);            // staging of warp w at stg + w * WSTG floats
+    constexpr int WSTG = GA_STAGES * GA_STAGE_BYTES / 4;
     if (g4 < G) {
-      float* dst = stg + ((size_t)warp * G + g4) * GA_PART;
+      float* dst = stg + (size_t)warp * WSTG + (size_t)g4 * GA_PART;
 #pragma unroll
       for (int nt = 0; nt < D / 8; ++nt) { dst[8 * nt + 2 * t4] = o[nt][0]; dst[8 * nt + 2 * t4 + 1] = o[nt][1]; }
       if (t4 == 0) { dst[D] = m_run; dst[D + 1] = l_run; }
@@ -1053,11 +1053,11 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
       const int h = idx / D, d = idx % D;
       float mm = -INFINITY;
 #pragma unroll
-      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[((size_t)w * G + h) * GA_PART + D]);
+      for (int w = 0; w < GA_WARPS; ++w) mm = fmaxf(mm, stg[(size_t)w * WSTG + (size_t)h * GA_PART + D]);
       float oo = 0.0f, ll = 0.0f;
 #pragma unroll
       for (int w = 0; w < GA_WARPS; ++w) {
-        const float* sp = stg + ((size_t)w * G + h) * GA_PART;
+        const float* sp = stg + (size_t)w * WSTG + (size_t)h * GA_PART;
         const float f = (sp[D] == -INFINITY) ? 0.0f : exp2f(sp[D] - mm);
         oo = fmaf(f, sp[d], oo);
         ll = fmaf(f, sp[D + 1], ll);
@@ -1071,6 +1071,7 @@ attn_gather_bits_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     const bool touches = tid >= clo && tid <= chi;
     const int expected = chi - clo + 1;
     __syncthreads();                                           // staging area free, partial stores fenced
+    if (tid == 0) s_rows = 0;                                  // (read above, before this barrier; next used after the barriers below)
     if (tid == 0) s_last = (atomicAdd(&gdone[gi], 1) == expected - 1);
     __syncthreads();
     if (tid == 0) RBQ_STAMP(gather_probe, 7);
