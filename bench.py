@@ -288,6 +288,10 @@ def run_b200(args):
         r = i % R
         caches[r].decode_step(q_dev, w.p, outs[r], None, sels[r][1])     # selection stays a bitmap in the workspace
 
+    # ---- set-up, untimed: every replica decodes twice (S7 sizes its work partition with the union sizes it counted in the
+    #      previous step of the same cache: the first step after rbq_set_workspace runs without that history) ------------
+    for i in range(2 * R):
+        step(i)
     # ---- device-timed region: W warm-ups, then exactly K steps ---------------------------------------------
     for i in range(args.warmup):
         step(i)
@@ -410,7 +414,9 @@ def run_b200(args):
                            f"({R * (2 * w.K.size * esz + alg['estimator']) / 2**30:.1f} GiB resident, L2 is 126 MB)",
                            "parallelism": f"{world} independent layer replica set(s), no data-path collective",
                            "budget_tokens": {"min": int(budgets.min()), "mean": float(budgets.mean()), "max": int(budgets.max())},
-                           "value_note": "us per decode step per layer = max-over-ranks step time / n_gpus"},
+                           "value_note": "us per decode step per layer = max-over-ranks step time / n_gpus",
+                           "setup_note": "every layer replica decodes twice, untimed, before the W warm-up steps (steady state of a "
+                                         "decode loop: S7 partitions its work with the union sizes counted in the replica's previous step)"},
                 "clocks": clocks, "gpu_launches": int(gpu_launches),
                 "step_us": {"p10": float(np.percentile(per_step, 10)), "median": float(np.median(per_step)),
                             "p90": float(np.percentile(per_step, 90))},
@@ -487,7 +493,7 @@ def step_profile(rb, caches, q_dev, p, steps, warm=5):
     import torch
     R = len(caches)
     outs = [c.new_out() for c in caches]
-    us = ev_time_us(lambda i: caches[i % R].decode_step(q_dev, p, outs[i % R]), steps, warm)
+    us = ev_time_us(lambda i: caches[i % R].decode_step(q_dev, p, outs[i % R]), steps, max(warm, 2 * R))   # >= 2 steps per replica first
     for c in caches:
         c.profile_enable(True)
     for i in range(min(steps, 128)):
